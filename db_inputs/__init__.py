@@ -1,0 +1,132 @@
+"""Seeded synthetic inputs shared by the CUDA path and the oracle.
+
+This module holds NONE of the method's arithmetic: only parameter values (the
+recipe of DESIGN.md "Inputs") and numpy-random tiny networks for the
+`db_create_from_csr` tests.  The CUDA binding and the oracle binding each
+translate these plain dicts into their own structs.
+
+Units: ms, mV; C = 1 so that g_L = 1/tau_m (R13: the paper prints no
+numeric neuron constants, Supp. Table 5 P:L816-832 gives names only).
+"""
+from __future__ import annotations
+
+import copy
+
+import numpy as np
+
+GEN_SEED = 20221115   # network generation
+DYN_SEED = 1          # dynamics (V0, Poisson background)
+
+RECEPTORS = ("AMPA", "NMDA", "GABA_A", "GABA_B")
+
+# background weight -> target mean rate (Hz), calibrated with the oracle on
+# config 0; mean-field is size independent at
+# fixed in-degree, so the same values serve configs 1, 2, 4.
+BG_WEIGHT_FOR_RATE = {7: 0.0072, 15: 0.0110, 30: 0.0240}
+
+
+def type_params(bg_weight: float = BG_WEIGHT_FOR_RATE[7], bg_rate_hz: float = 1000.0,
+                g_scale: float = 1.0) -> dict:
+    """One neuron type (paper property table, Supp. Table 5)."""
+    return dict(
+        C=1.0, gL=0.03, VL=-75.0, Vth=-50.0, Vreset=-65.0, Tref_ms=5.0, Iext=0.0,
+        G=[1.0 * g_scale, 0.25 * g_scale, 1.0 * g_scale, 1.0 * g_scale],
+        E=[0.0, 0.0, -70.0, -100.0],
+        tau_ms=[2.0, 40.0, 10.0, 50.0],
+        bg_rate_hz=bg_rate_hz, bg_weight=bg_weight,
+    )
+
+
+def sim_params(dt_ms: float = 0.1, S: int = 22, D: int = 32, window_steps: int = 10,
+               rate_hz: int = 7, g_scale: float = 1.0, types: list | None = None) -> dict:
+    if types is None:
+        # G scales with 100/K (R20); the background enters through G_AMPA too, so its
+        # weight is divided by the same factor to keep the drive fixed.
+        t = type_params(BG_WEIGHT_FOR_RATE[rate_hz] / g_scale, g_scale=g_scale)
+        types = [t, copy.deepcopy(t)]            # exc and inh share constants (R13)
+    return dict(dt_ms=dt_ms, S=S, D=D, window_steps=window_steps, types=types)
+
+
+def _net(**kw) -> dict:
+    base = dict(
+        N=0, n_regions=1, region_size_sigma=0.0, exc_frac=0.8, mode=0, K=100,
+        intra_frac=1.0, region_matrix_sigma=1.0,
+        outdeg_mean=500.0, outdeg_sigma=1.0, outdeg_cap=20000,
+        w_mu=-1.0, w_sigma=0.5, w_scale=0.01, inh_mult=4.0, slow_frac=0.2,
+        delay_intra_min=1, delay_intra_max=20, delay_inter_min=20, delay_inter_max=200,
+        weight_fp16=0,
+    )
+    base.update(kw)
+    return base
+
+
+def config(idx: int, rate_hz: int | None = None, scale: float = 1.0) -> dict:
+    """BASELINE.json configs[idx] as {"net": ..., "sim": ..., "steps": ...}.
+
+    `scale` < 1 shrinks N (same structure) for parity cases the oracle can
+    finish in seconds.
+    """
+    if idx == 0:
+        net = _net(N=int(10_000 * scale), K=100)
+        return dict(name="config0", net=net, sim=sim_params(rate_hz=rate_hz or 7), steps=1000)
+    if idx == 1:
+        net = _net(N=int(1_000_000 * scale), K=100)
+        return dict(name="config1", net=net, sim=sim_params(rate_hz=rate_hz or 7), steps=10_000)
+    if idx == 2:
+        net = _net(N=int(5_000_000 * scale), n_regions=200, region_size_sigma=0.7, K=200,
+                   intra_frac=0.8)
+        # 200 inputs per neuron: hold the mean input of K=100 fixed (R20)
+        return dict(name="config2", net=net,
+                    sim=sim_params(rate_hz=rate_hz or 7, D=256, g_scale=0.5), steps=10_000)
+    if idx == 3:
+        net = _net(N=int(10_000_000 * scale), n_regions=200, region_size_sigma=0.7, K=1000,
+                   intra_frac=0.8, weight_fp16=1)
+        return dict(name="config3", net=net,
+                    sim=sim_params(rate_hz=rate_hz or 15, D=256, g_scale=0.1), steps=1000)
+    if idx == 4:
+        net = _net(N=int(2_000_000 * scale), mode=1, K=0)
+        return dict(name="config4", net=net,
+                    sim=sim_params(rate_hz=rate_hz or 30, g_scale=0.2), steps=10_000)
+    raise ValueError(idx)
+
+
+def random_csr(N: int, mean_outdeg: float, seed: int, max_delay: int = 20, n_regions: int = 1,
+               exc_frac: float = 0.8, fp16: bool = False, heavy_rows: dict | None = None) -> dict:
+    """Tiny numpy-random network for from-CSR tests (unique (src, tgt) pairs).
+
+    heavy_rows: {row: out_degree} to force long rows (load-balance edge cases).
+    """
+    rng = np.random.default_rng(seed)
+    n_exc = int(round(exc_frac * N))
+    ntype = np.zeros(N, np.uint8)
+    bounds = np.linspace(0, N, n_regions + 1).astype(np.int64)
+    for r in range(n_regions):
+        lo, hi = bounds[r], bounds[r + 1]
+        ne = int(round(exc_frac * (hi - lo)))
+        ntype[lo + ne:hi] = 1
+    if n_regions == 1:
+        ntype[:] = 0
+        ntype[n_exc:] = 1
+    deg = rng.poisson(mean_outdeg, N).astype(np.int64)
+    if heavy_rows:
+        for r, d in heavy_rows.items():
+            deg[r] = d
+    deg = np.minimum(deg, N - 1)
+    row_ptr = np.zeros(N + 1, np.int64)
+    row_ptr[1:] = np.cumsum(deg)
+    E = int(row_ptr[-1])
+    tgt = np.empty(E, np.int32)
+    for j in range(N):
+        t = rng.choice(N - 1, size=int(deg[j]), replace=False)
+        t = np.sort(t + (t >= j))
+        tgt[row_ptr[j]:row_ptr[j + 1]] = t
+    w = (0.01 * rng.lognormal(-1.0, 0.5, E)).astype(np.float32)
+    src_type = np.repeat(ntype, deg)
+    w = np.where(src_type == 1, w * np.float32(4.0), w).astype(np.float32)
+    if fp16:
+        w = w.astype(np.float16).astype(np.float32)
+    delay = rng.integers(1, max_delay + 1, E).astype(np.uint8)
+    slow = (rng.random(E) < 0.2).astype(np.uint8)
+    rec = (2 * src_type + slow).astype(np.uint8)
+    return dict(N=N, E=E, n_regions=n_regions, region_start=bounds, ntype=ntype,
+                row_ptr=row_ptr, tgt=tgt, w=w, delay=delay, rec=rec)

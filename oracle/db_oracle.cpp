@@ -1,0 +1,735 @@
+// =============================================================================
+// db_oracle.cpp -- ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+//
+// Plain, slow, single-threaded CPU implementation of the per-time-step hot path
+// of the Digital Brain spiking-network simulator (arXiv 2211.15963), written
+// from /root/reference/PAPER.md ("P:L<n>" = line n of that file) and the
+// readings listed in DESIGN.md ("R<n>").  It shares NO code with the CUDA path
+// under paper_2211_15963_b200/: no headers, helpers, tables or generators.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+// reference legs may load this library.
+//
+// What is here
+//   1. Philox4x32-10 counter-based generator (Salmon et al., SC'11) + the
+//      keyed draws the method uses (V0, Poisson background, generator).
+//   2. Integer Poisson inverse-CDF thresholds (background drive).
+//   3. The synthetic network generator (stand-in for the paper's HRGCME
+//      generator): fixed in-degree / lognormal
+//      out-degree, regions, no autapses, no multapses.
+//   4. The simulator: one iteration = SI Eq.(3) conductances,
+//      SI Eq.(5) membrane step read with the CV equation,
+//      threshold / reset / refractory, push-based spike
+//      delivery (Supp. Alg. 2) into a delayed fixed-point ring.
+//   5. Dense brute-force delivery (plain definition of the delivered sums).
+//
+// Pins (tests/, -m "not gpu"): Philox known-answer vectors; Poisson moments;
+// discrete + continuous LIF closed forms, first-spike time, ISI = n*+R;
+// single-event conductance kernel; PSP shape; dense brute force + event
+// conservation; generator degree/no-dup/receptor/moment checks and a second
+// independent (Python) implementation of the draws.
+// Parity unpinned: the numeric neuron constants (paper prints none, R13) and
+// the absolute firing rates they produce.
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -fno-fast-math -shared -fPIC
+//        (no FMA contraction: the fp32 mode is an arithmetic contract, R-FP).
+// =============================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <algorithm>
+#include <vector>
+
+namespace {
+
+// ----------------------------------------------------------------------------
+// 1. Philox4x32-10 (Salmon, Moraes, Dror, Shaw: "Parallel random numbers: as
+//    easy as 1, 2, 3", SC'11).  10 rounds; multipliers / Weyl constants as
+//    published.  counter c[4], key k[2] -> 4 output words.
+// ----------------------------------------------------------------------------
+struct u32x4 { uint32_t w[4]; };
+
+u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                    uint32_t k0, uint32_t k1) {
+    const uint64_t M0 = 0xD2511F53ull, M1 = 0xCD9E8D57ull;
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = M0 * (uint64_t)c0;
+        uint64_t p1 = M1 * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    u32x4 o; o.w[0] = c0; o.w[1] = c1; o.w[2] = c2; o.w[3] = c3;
+    return o;
+}
+
+// Keyed draw used everywhere (R-RNG): key = seed, counter =
+// (a_lo, a_hi | stream<<24, b_lo, b_hi); a < 2^56 is an entity id, b a second
+// index (time step, slot).
+enum : uint32_t {
+    STREAM_V0 = 1,     // initial membrane potential
+    STREAM_BG = 2,     // Poisson background counts
+    STREAM_SRC = 3,    // permutation round keys (source / target selection)
+    STREAM_SYN = 4,    // per-synapse weight / delay / receptor
+    STREAM_REGION = 5, // region sizes and region matrix (host-side normals)
+    STREAM_INTER = 6,  // source-region choice of an inter-region input
+    STREAM_DEG = 7     // out-degree of a neuron (out-degree mode)
+};
+
+u32x4 draw(uint64_t seed, uint32_t stream, uint64_t a, uint64_t b) {
+    return philox4x32_10((uint32_t)a, (uint32_t)(a >> 32) | (stream << 24),
+                         (uint32_t)b, (uint32_t)(b >> 32),
+                         (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// ----------------------------------------------------------------------------
+// 2. Poisson inverse CDF on a 32-bit uniform (background drive: "independent
+//    homogeneous Poisson spike trains"; R14).
+//    T_m = floor(CDF(m; lambda) * 2^32), k = #{m : u >= T_m}.
+// ----------------------------------------------------------------------------
+const int POISSON_MAX = 32;
+
+int poisson_thresholds(double lambda, uint32_t* T /*[POISSON_MAX]*/) {
+    double pm = std::exp(-lambda);   // P(0)
+    double cdf = 0.0;
+    int M = 0;
+    for (int m = 0; m < POISSON_MAX; ++m) {
+        cdf += pm;
+        double t = std::floor(cdf * 4294967296.0);
+        if (t >= 4294967295.0) break;          // CDF saturated at 32-bit resolution
+        T[M++] = (uint32_t)t;
+        pm = pm * lambda / (double)(m + 1);
+    }
+    return M;
+}
+
+int poisson_count(uint32_t u, const uint32_t* T, int M) {
+    int k = 0;
+    for (int m = 0; m < M; ++m) if (u >= T[m]) ++k;
+    return k;
+}
+
+// ----------------------------------------------------------------------------
+// 3a. Keyed pseudo-random permutation of [0, M): 8-round alternating Feistel
+//     network on nb = max(2, ceil(log2 M)) bits with cycle walking (round r
+//     uses key[r & 3] + (r >> 2) * 0x9E3779B9).  Taking
+//     perm(0), perm(1), ... gives sources "sampled with equal probability
+//     without replacement" with no rejection state.
+// ----------------------------------------------------------------------------
+uint32_t fmix32(uint32_t h) {      // MurmurHash3 finaliser (public domain)
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+
+uint32_t prp(uint32_t x, uint32_t M, const uint32_t key[4]) {
+    if (M <= 1) return 0;
+    int nb = 2;
+    while (nb < 32 && (1ull << nb) < (uint64_t)M) ++nb;
+    const int a = nb / 2, b = nb - a;           // left a bits, right b bits
+    do {
+        uint32_t L = x >> b, R = x & ((1u << b) - 1u);
+        int nl = a, nr = b;
+        for (int r = 0; r < 8; ++r) {
+            uint32_t rk = key[r & 3] + (uint32_t)(r >> 2) * 0x9E3779B9u;
+            uint32_t F = fmix32(R + rk) & ((1u << nl) - 1u);
+            uint32_t newR = L ^ F;              // nl bits
+            L = R; R = newR;
+            int t = nl; nl = nr; nr = t;
+        }
+        x = (L << nr) | R;                      // even round count: (nl, nr) == (a, b) again
+    } while (x >= M);
+    return x;
+}
+
+// ----------------------------------------------------------------------------
+// 3b. Host-side helpers for distribution tables.
+// ----------------------------------------------------------------------------
+double norm_cdf(double z) { return 0.5 * std::erfc(-z / std::sqrt(2.0)); }
+
+double norm_ppf(double p) {                      // bisection on the CDF
+    double lo = -40.0, hi = 40.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (norm_cdf(mid) < p) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+// IEEE binary16 round-to-nearest-even of a float, returned as float.
+float round_to_half(float f) {
+    uint32_t x; std::memcpy(&x, &f, 4);
+    uint32_t sign = x & 0x80000000u;
+    uint32_t ax = x & 0x7FFFFFFFu;
+    float r;
+    if (ax >= 0x7F800000u) return f;                      // inf / nan
+    float af; std::memcpy(&af, &ax, 4);
+    if (af >= 65520.0f) { uint32_t inf = sign | 0x7F800000u; std::memcpy(&r, &inf, 4); return r; }
+    if (af < 6.103515625e-05f) {                          // subnormal half: multiples of 2^-24
+        float q = std::nearbyintf(af * 16777216.0f) / 16777216.0f;
+        uint32_t qb; std::memcpy(&qb, &q, 4); qb |= sign; std::memcpy(&r, &qb, 4); return r;
+    }
+    uint32_t rem = ax & 0x1FFFu, base = ax & ~0x1FFFu;    // drop 13 mantissa bits
+    if (rem > 0x1000u || (rem == 0x1000u && (base & 0x2000u))) base += 0x2000u;
+    base |= sign; std::memcpy(&r, &base, 4);
+    return r;
+}
+
+}  // namespace
+
+// =============================================================================
+// C interface (ctypes).  All structs are plain data.
+// =============================================================================
+extern "C" {
+
+// Per neuron type (0 = excitatory, 1 = inhibitory).  Names follow the paper's
+// property table (Supp. Table 5).  Units: ms, mV; C = 1 makes
+// g_L = 1/tau_m.
+struct orc_type_params {
+    double C, gL, VL, Vth, Vreset, Tref_ms, Iext;
+    double G[4];        // g_u: maximal conductance per receptor
+    double E[4];        // V_u: reversal potential
+    double tau_ms[4];   // tau_u
+    double bg_rate_hz;  // Poisson background rate per neuron (R14)
+    double bg_weight;   // its weight, delivered to AMPA
+};
+
+struct orc_sim_params {
+    double dt_ms;
+    int32_t S;            // fixed-point shift of the ring (R28)
+    int32_t D;            // ring depth, power of two, > max delay
+    int32_t window_steps; // region-rate window (R24)
+    int32_t n_types;
+    orc_type_params type[4];
+};
+
+struct orc_net_spec {
+    int64_t N;
+    int32_t n_regions;
+    double region_size_sigma;    // region sizes ~ lognormal(0, sigma), normalised
+    double exc_frac;             // 0.8
+    int32_t mode;                // 0 fixed in-degree, 1 lognormal out-degree
+    int32_t K;                   // in-degree (mode 0)
+    double intra_frac;           // fraction of K from the own region (n_regions > 1)
+    double region_matrix_sigma;  // inter-region weights ~ lognormal(0, sigma), zero diag, row-normalised
+    double outdeg_mean, outdeg_sigma; int32_t outdeg_cap;   // mode 1 (R27)
+    double w_mu, w_sigma, w_scale, inh_mult, slow_frac;     // weights (R11), receptors (R12)
+    int32_t delay_intra_min, delay_intra_max, delay_inter_min, delay_inter_max; // steps
+    int32_t weight_fp16;
+};
+
+// ---- raw generator access for the pins --------------------------------------
+void orc_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                uint32_t k0, uint32_t k1, uint32_t* out4) {
+    u32x4 o = philox4x32_10(c0, c1, c2, c3, k0, k1);
+    for (int i = 0; i < 4; ++i) out4[i] = o.w[i];
+}
+void orc_draw(uint64_t seed, uint32_t stream, uint64_t a, uint64_t b, uint32_t* out4) {
+    u32x4 o = draw(seed, stream, a, b);
+    for (int i = 0; i < 4; ++i) out4[i] = o.w[i];
+}
+int32_t orc_poisson_thresholds(double lambda, uint32_t* T) { return poisson_thresholds(lambda, T); }
+int32_t orc_poisson_count(uint32_t u, const uint32_t* T, int32_t M) { return poisson_count(u, T, M); }
+uint32_t orc_prp(uint32_t x, uint32_t M, const uint32_t* key4) { return prp(x, M, key4); }
+double orc_norm_ppf(double p) { return norm_ppf(p); }
+float orc_round_to_half(float f) { return round_to_half(f); }
+
+// =============================================================================
+// 3c. Network generator.  Output: presynaptic-major CSR (one row per source
+//     neuron = the paper's per-neuron destination-address list), rows
+//     sorted by (target, receptor).  Regions are contiguous id ranges,
+//     excitatory neurons first inside each region.
+// =============================================================================
+struct orc_network {
+    int64_t N, E;
+    int32_t n_regions;
+    int64_t* region_start;   // [n_regions+1]
+    int64_t* region_nexc;    // [n_regions]
+    uint8_t* ntype;          // [N] 0 exc / 1 inh
+    int64_t* row_ptr;        // [N+1]
+    int32_t* tgt;            // [E]
+    float* w;                // [E] (already rounded to binary16 if weight_fp16)
+    uint8_t* delay;          // [E] steps
+    uint8_t* rec;            // [E] receptor 0..3
+};
+
+void orc_network_free(orc_network* n) {
+    if (!n) return;
+    std::free(n->region_start); std::free(n->region_nexc); std::free(n->ntype);
+    std::free(n->row_ptr); std::free(n->tgt); std::free(n->w); std::free(n->delay); std::free(n->rec);
+    std::free(n);
+}
+
+namespace {
+struct Edge { int32_t src, tgt; float w; uint8_t delay, rec; };
+
+// Standard normal from two 32-bit words (Box-Muller, double); host tables only.
+double normal_from(uint32_t u0, uint32_t u1) {
+    double a = ((double)u0 + 0.5) / 4294967296.0;
+    double b = ((double)u1 + 0.5) / 4294967296.0;
+    return std::sqrt(-2.0 * std::log(a)) * std::cos(2.0 * M_PI * b);
+}
+
+// Largest-remainder apportionment of `total` into parts proportional to x[].
+std::vector<int64_t> apportion(const std::vector<double>& x, int64_t total) {
+    size_t n = x.size();
+    double s = 0; for (double v : x) s += v;
+    std::vector<int64_t> out(n);
+    std::vector<std::pair<double, size_t>> frac(n);
+    int64_t used = 0;
+    for (size_t i = 0; i < n; ++i) {
+        double q = x[i] / s * (double)total;
+        out[i] = (int64_t)std::floor(q);
+        frac[i] = { -(q - std::floor(q)), i };   // sort: largest remainder first, then index
+        used += out[i];
+    }
+    std::sort(frac.begin(), frac.end());
+    for (int64_t r = 0; r < total - used; ++r) out[frac[(size_t)r].second] += 1;
+    return out;
+}
+
+int region_of(const int64_t* region_start, int n_regions, int64_t i) {
+    int r = 0;
+    while (r + 1 < n_regions && region_start[r + 1] <= i) ++r;   // plain linear scan
+    return r;
+}
+}  // namespace
+
+// Weight quantile table (65536 entries): w_q = scale * exp(mu + sigma * Phi^-1((q+0.5)/65536)).
+void orc_weight_table(double mu, double sigma, double scale, float* tab /*[65536]*/) {
+    for (int q = 0; q < 65536; ++q) {
+        double z = norm_ppf(((double)q + 0.5) / 65536.0);
+        tab[q] = (float)(scale * std::exp(mu + sigma * z));
+    }
+}
+
+// Out-degree quantile table (mode 1, R27): mean of the lognormal = outdeg_mean.
+void orc_outdeg_table(double mean, double sigma, int32_t cap, int32_t* tab /*[65536]*/) {
+    double mu = std::log(mean) - 0.5 * sigma * sigma;
+    for (int q = 0; q < 65536; ++q) {
+        double z = norm_ppf(((double)q + 0.5) / 65536.0);
+        double d = std::floor(std::exp(mu + sigma * z) + 0.5);
+        if (d < 1) d = 1;
+        if (d > cap) d = cap;
+        tab[q] = (int32_t)d;
+    }
+}
+
+// Region sizes (lognormal, normalised, largest remainder) -- config 2 / 3.
+void orc_region_sizes(uint64_t seed, int64_t N, int32_t R, double sigma, int64_t* sizes) {
+    std::vector<double> x((size_t)R);
+    for (int r = 0; r < R; ++r) {
+        u32x4 o = draw(seed, STREAM_REGION, (uint64_t)r, 0);
+        x[(size_t)r] = std::exp(sigma * normal_from(o.w[0], o.w[1]));
+    }
+    std::vector<int64_t> s = apportion(x, N);
+    for (int r = 0; r < R; ++r) sizes[r] = s[(size_t)r];
+}
+
+// Inter-region cumulative thresholds: row r holds R-1 uint32 thresholds; the
+// source region of a draw u is #{m : u >= T[r][m]}.
+void orc_region_cdf(uint64_t seed, int32_t R, double sigma, uint32_t* T /*[R][R-1]*/) {
+    for (int r = 0; r < R; ++r) {
+        std::vector<double> p((size_t)R);
+        double s = 0;
+        for (int c = 0; c < R; ++c) {
+            u32x4 o = draw(seed, STREAM_REGION, (uint64_t)r * (uint64_t)R + (uint64_t)c, 1);
+            p[(size_t)c] = (c == r) ? 0.0 : std::exp(sigma * normal_from(o.w[0], o.w[1]));
+            s += p[(size_t)c];
+        }
+        double cum = 0;
+        for (int c = 0; c < R - 1; ++c) {
+            cum += p[(size_t)c] / s;
+            double t = std::floor(cum * 4294967296.0);
+            if (t > 4294967295.0) t = 4294967295.0;
+            T[(size_t)r * (size_t)(R - 1) + (size_t)c] = (uint32_t)t;
+        }
+    }
+}
+
+orc_network* orc_generate(const orc_net_spec* sp, uint64_t seed) {
+    const int64_t N = sp->N;
+    const int R = sp->n_regions;
+    orc_network* net = (orc_network*)std::calloc(1, sizeof(orc_network));
+    net->N = N; net->n_regions = R;
+    net->region_start = (int64_t*)std::calloc((size_t)R + 1, sizeof(int64_t));
+    net->region_nexc = (int64_t*)std::calloc((size_t)R, sizeof(int64_t));
+    net->ntype = (uint8_t*)std::calloc((size_t)N, 1);
+
+    // regions and types -------------------------------------------------------
+    std::vector<int64_t> sizes((size_t)R);
+    if (R == 1) sizes[0] = N; else orc_region_sizes(seed, N, R, sp->region_size_sigma, sizes.data());
+    for (int r = 0; r < R; ++r) {
+        net->region_start[r + 1] = net->region_start[r] + sizes[(size_t)r];
+        net->region_nexc[r] = (int64_t)std::floor(sp->exc_frac * (double)sizes[(size_t)r] + 0.5);
+        for (int64_t l = 0; l < sizes[(size_t)r]; ++l)
+            net->ntype[net->region_start[r] + l] = (l < net->region_nexc[r]) ? 0 : 1;
+    }
+
+    std::vector<float> wtab(65536);
+    orc_weight_table(sp->w_mu, sp->w_sigma, sp->w_scale, wtab.data());
+    const uint32_t slow_thr = (uint32_t)std::floor(sp->slow_frac * 4294967296.0);
+    const float inh_mult = (float)sp->inh_mult;
+
+    // attributes of the synapse drawn as (owner, slot): weight, delay, receptor
+    auto make_edge = [&](int64_t owner, int64_t slot, int64_t src, int64_t tgt, bool inter) {
+        u32x4 o = draw(seed, STREAM_SYN, (uint64_t)owner, (uint64_t)slot);
+        Edge e;
+        e.src = (int32_t)src; e.tgt = (int32_t)tgt;
+        bool inh = net->ntype[src] != 0;
+        float w = wtab[o.w[0] >> 16];
+        if (inh) w = w * inh_mult;
+        if (sp->weight_fp16) w = round_to_half(w);
+        e.w = w;
+        int dmin = inter ? sp->delay_inter_min : sp->delay_intra_min;
+        int dmax = inter ? sp->delay_inter_max : sp->delay_intra_max;
+        e.delay = (uint8_t)(dmin + (int)(((uint64_t)o.w[1] * (uint64_t)(dmax - dmin + 1)) >> 32));
+        int slow = (o.w[2] < slow_thr) ? 1 : 0;      // NMDA / GABA_B w.p. slow_frac (R12)
+        e.rec = (uint8_t)((inh ? 2 : 0) + slow);      // receptor class follows the SOURCE type
+        return e;
+    };
+
+    std::vector<Edge> edges;
+    if (sp->mode == 0) {
+        // fixed in-degree K per target ("for each neuron, the number of
+        // synaptic inputs from each neuron population ...").
+        std::vector<uint32_t> cdf;
+        int K_intra = sp->K, K_inter = 0;
+        if (R > 1) {
+            K_intra = (int)std::floor(sp->intra_frac * (double)sp->K + 0.5);
+            K_inter = sp->K - K_intra;
+            cdf.resize((size_t)R * (size_t)(R - 1));
+            orc_region_cdf(seed, R, sp->region_matrix_sigma, cdf.data());
+        }
+        edges.reserve((size_t)N * (size_t)sp->K);
+        for (int64_t i = 0; i < N; ++i) {
+            int r = region_of(net->region_start, R, i);
+            int64_t base = net->region_start[r];
+            int64_t size = net->region_start[r + 1] - base;
+            int64_t li = i - base;
+            u32x4 k0 = draw(seed, STREAM_SRC, (uint64_t)i, 0);
+            for (int k = 0; k < K_intra; ++k) {        // own region, any type, not self
+                uint32_t j = prp((uint32_t)k, (uint32_t)(size - 1), k0.w);
+                if ((int64_t)j >= li) j += 1;          // skip self: no autapse
+                edges.push_back(make_edge(i, k, base + j, i, false));
+            }
+            u32x4 k1 = draw(seed, STREAM_SRC, (uint64_t)i, 1);
+            for (int s = 0; s < K_inter; ++s) {        // other regions, excitatory only
+                uint32_t u = draw(seed, STREAM_INTER, (uint64_t)i, (uint64_t)s).w[0];
+                const uint32_t* T = &cdf[(size_t)r * (size_t)(R - 1)];
+                int rs = 0;
+                for (int m = 0; m < R - 1; ++m) if (u >= T[m]) ++rs;
+                // distinct slots s map to distinct neurons of region rs (prp is injective)
+                uint32_t j = prp((uint32_t)s, (uint32_t)net->region_nexc[rs], k1.w);
+                edges.push_back(make_edge(i, K_intra + s, net->region_start[rs] + j, i, true));
+            }
+        }
+    } else {
+        // lognormal out-degree per source, targets uniform without replacement (R27)
+        std::vector<int32_t> dtab(65536);
+        orc_outdeg_table(sp->outdeg_mean, sp->outdeg_sigma, sp->outdeg_cap, dtab.data());
+        for (int64_t j = 0; j < N; ++j) {
+            int32_t deg = dtab[draw(seed, STREAM_DEG, (uint64_t)j, 0).w[0] >> 16];
+            if ((int64_t)deg > N - 1) deg = (int32_t)(N - 1);
+            u32x4 k0 = draw(seed, STREAM_SRC, (uint64_t)j, 0);
+            for (int m = 0; m < deg; ++m) {
+                uint32_t t = prp((uint32_t)m, (uint32_t)(N - 1), k0.w);
+                if ((int64_t)t >= j) t += 1;
+                edges.push_back(make_edge(j, m, j, t, false));
+            }
+        }
+    }
+
+    // presynaptic-major CSR, rows sorted by target ---------------------------------
+    std::sort(edges.begin(), edges.end(), [](const Edge& a, const Edge& b) {
+        if (a.src != b.src) return a.src < b.src;
+        if (a.tgt != b.tgt) return a.tgt < b.tgt;
+        return a.rec < b.rec;
+    });
+    const int64_t E = (int64_t)edges.size();
+    net->E = E;
+    net->row_ptr = (int64_t*)std::calloc((size_t)N + 1, sizeof(int64_t));
+    net->tgt = (int32_t*)std::malloc(sizeof(int32_t) * (size_t)std::max<int64_t>(E, 1));
+    net->w = (float*)std::malloc(sizeof(float) * (size_t)std::max<int64_t>(E, 1));
+    net->delay = (uint8_t*)std::malloc((size_t)std::max<int64_t>(E, 1));
+    net->rec = (uint8_t*)std::malloc((size_t)std::max<int64_t>(E, 1));
+    for (int64_t e = 0; e < E; ++e) {
+        net->row_ptr[edges[(size_t)e].src + 1] += 1;
+        net->tgt[e] = edges[(size_t)e].tgt; net->w[e] = edges[(size_t)e].w;
+        net->delay[e] = edges[(size_t)e].delay; net->rec[e] = edges[(size_t)e].rec;
+    }
+    for (int64_t i = 0; i < N; ++i) net->row_ptr[i + 1] += net->row_ptr[i];
+    return net;
+}
+
+// =============================================================================
+// 4. The simulator.  `real` = float is the parity mode (fp32, fixed operation
+//    order, no FMA: R-FP); `real` = double is used only for closed-form and
+//    dt-convergence pins.
+// =============================================================================
+}  // extern "C"
+
+namespace {
+
+template <typename real>
+struct TypeConst {
+    real gL, VL, Vth, Vreset, kappa, Iext;
+    real G[4], E[4], alpha[4];
+    int32_t R;              // refractory steps
+    int32_t wq_bg;
+    uint32_t T[POISSON_MAX]; int M;
+};
+
+template <typename real>
+struct Sim {
+    int64_t N = 0, E = 0;
+    int D = 0, S = 0, window = 0, n_regions = 1;
+    uint64_t seed = 0;
+    uint64_t step = 0;
+    std::vector<TypeConst<real>> tc;
+    std::vector<uint8_t> ntype;
+    std::vector<int64_t> region_start;
+    // network (borrowed copies)
+    std::vector<int64_t> row_ptr; std::vector<int32_t> tgt; std::vector<float> w;
+    std::vector<uint8_t> delay, rec;
+    // state
+    std::vector<real> V, g;           // g[4*i+u]
+    std::vector<int32_t> ref;
+    std::vector<int32_t> ring;        // ring[(slot*N + i)*4 + u]
+    // outputs
+    std::vector<uint64_t> spike_step; std::vector<int32_t> spike_id;
+    std::vector<uint32_t> region_count;   // [window][region]
+    uint64_t n_events = 0, n_bg = 0;
+    int32_t overflow = 0;
+    bool log_arrivals = false;            // pins only: what step 1 consumed, [n][i][u]
+    std::vector<int32_t> arrivals_log;
+
+    void one_step() {
+        const uint64_t n = step;
+        const real scale = (real)std::ldexp(1.0, -S);
+        int32_t* slot = &ring[(size_t)(n % (uint64_t)D) * (size_t)N * 4];
+        std::vector<int32_t> L;                           // SpikeList (Alg. 2 line 2)
+        for (int64_t i = 0; i < N; ++i) {
+            const TypeConst<real>& c = tc[ntype[(size_t)i]];
+            // 1. arrivals due now; the slot is consumed
+            int32_t a[4];
+            for (int u = 0; u < 4; ++u) { a[u] = slot[i * 4 + u]; slot[i * 4 + u] = 0; }
+            if (log_arrivals) for (int u = 0; u < 4; ++u) arrivals_log.push_back(a[u]);
+            for (int u = 0; u < 4; ++u)
+                if (a[u] > (1 << 30) || a[u] < -(1 << 30)) overflow = 1;
+            // 2. Poisson background into AMPA (R14); one Philox block serves 4 neurons
+            uint32_t uu = draw(seed, STREAM_BG, (uint64_t)(i >> 2), n).w[i & 3];
+            int k = poisson_count(uu, c.T, c.M);
+            a[0] = (int32_t)((uint32_t)a[0] + (uint32_t)k * (uint32_t)c.wq_bg);
+            n_bg += (uint64_t)k;
+            // 3. fixed point -> real
+            real x[4];
+            for (int u = 0; u < 4; ++u) x[u] = (real)a[u] * scale;
+            // 4. synaptic current I_u = g_u (V_u - V) J_u, fixed summation order
+            real v = V[(size_t)i];
+            real* gi = &g[(size_t)i * 4];
+            real t0 = (c.G[0] * gi[0]) * (c.E[0] - v);
+            real t1 = (c.G[1] * gi[1]) * (c.E[1] - v);
+            real t2 = (c.G[2] * gi[2]) * (c.E[2] - v);
+            real t3 = (c.G[3] * gi[3]) * (c.E[3] - v);
+            real I = (((t0 + t1) + t2) + t3) + c.Iext;
+            // 5. membrane step: CV equation with Euler step (SI Eq.(5); R1)
+            real leak = (-c.gL) * (v - c.VL);
+            real vn = v + c.kappa * (leak + I);
+            // 6. conductances: exact exponential decay + arrivals (SI Eq.(3))
+            for (int u = 0; u < 4; ++u) gi[u] = gi[u] * c.alpha[u] + x[u];
+            // 7. refractory clamp / threshold / reset (R5, R6)
+            int spike = 0;
+            if (ref[(size_t)i] > 0) { vn = c.Vreset; ref[(size_t)i] -= 1; }
+            else if (vn >= c.Vth) { spike = 1; vn = c.Vreset; ref[(size_t)i] = c.R; }
+            V[(size_t)i] = vn;
+            if (spike) L.push_back((int32_t)i);
+        }
+        // 8. record + region counts
+        const size_t win = (size_t)(n / (uint64_t)window);
+        if (region_count.size() < (win + 1) * (size_t)n_regions) region_count.resize((win + 1) * (size_t)n_regions, 0);
+        for (int32_t j : L) {
+            spike_step.push_back(n); spike_id.push_back(j);
+            int r = 0;
+            while (r + 1 < n_regions && region_start[(size_t)r + 1] <= j) ++r;
+            region_count[win * (size_t)n_regions + (size_t)r] += 1;
+        }
+        // 9. push delivery along the destination list (Alg. 2 lines 3-4)
+        for (int32_t j : L) {
+            for (int64_t s = row_ptr[(size_t)j]; s < row_ptr[(size_t)j + 1]; ++s) {
+                int32_t wq = (int32_t)std::lrintf(w[(size_t)s] * (float)std::ldexp(1.0, S));
+                size_t sl = (size_t)((n + delay[(size_t)s]) % (uint64_t)D);
+                int32_t* cell = &ring[(sl * (size_t)N + (size_t)tgt[(size_t)s]) * 4 + rec[(size_t)s]];
+                *cell = (int32_t)((uint32_t)*cell + (uint32_t)wq);      // two's-complement wrap
+            }
+            n_events += (uint64_t)(row_ptr[(size_t)j + 1] - row_ptr[(size_t)j]);
+        }
+        step += 1;
+    }
+};
+
+template <typename real>
+Sim<real>* sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
+                      int32_t n_regions, const int64_t* region_start,
+                      const int64_t* row_ptr, const int32_t* tgt, const float* w,
+                      const uint8_t* delay, const uint8_t* rec, uint64_t seed) {
+    Sim<real>* s = new Sim<real>();
+    s->N = N; s->E = row_ptr[N]; s->D = p->D; s->S = p->S; s->window = p->window_steps;
+    s->seed = seed; s->n_regions = n_regions;
+    s->ntype.assign(ntype, ntype + N);
+    s->region_start.assign(region_start, region_start + n_regions + 1);
+    s->row_ptr.assign(row_ptr, row_ptr + N + 1);
+    s->tgt.assign(tgt, tgt + s->E); s->w.assign(w, w + s->E);
+    s->delay.assign(delay, delay + s->E); s->rec.assign(rec, rec + s->E);
+    for (int t = 0; t < p->n_types; ++t) {
+        const orc_type_params& q = p->type[t];
+        TypeConst<real> c;
+        // constants are formed in double, then rounded once to `real`
+        c.gL = (real)q.gL; c.VL = (real)q.VL; c.Vth = (real)q.Vth; c.Vreset = (real)q.Vreset;
+        c.kappa = (real)(p->dt_ms / q.C); c.Iext = (real)q.Iext;
+        for (int u = 0; u < 4; ++u) {
+            c.G[u] = (real)q.G[u]; c.E[u] = (real)q.E[u];
+            c.alpha[u] = (real)std::exp(-p->dt_ms / q.tau_ms[u]);
+        }
+        c.R = (int32_t)std::lrint(q.Tref_ms / p->dt_ms);
+        c.wq_bg = (int32_t)std::lrint(q.bg_weight * std::ldexp(1.0, p->S));
+        c.M = poisson_thresholds(q.bg_rate_hz * p->dt_ms * 1e-3, c.T);
+        s->tc.push_back(c);
+    }
+    s->V.resize((size_t)N); s->g.assign((size_t)N * 4, (real)0); s->ref.assign((size_t)N, 0);
+    s->ring.assign((size_t)p->D * (size_t)N * 4, 0);
+    for (int64_t i = 0; i < N; ++i) {
+        const TypeConst<real>& c = s->tc[ntype[i]];
+        uint32_t u = draw(seed, STREAM_V0, (uint64_t)i, 0).w[0];
+        real U = (real)(u >> 8) * (real)std::ldexp(1.0, -24);
+        s->V[(size_t)i] = c.Vreset + (c.Vth - c.Vreset) * U;
+    }
+    return s;
+}
+
+struct Handle { int fp64; Sim<float>* f; Sim<double>* d; };
+
+}  // namespace
+
+extern "C" {
+
+void* orc_sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
+                     int32_t n_regions, const int64_t* region_start,
+                     const int64_t* row_ptr, const int32_t* tgt, const float* w,
+                     const uint8_t* delay, const uint8_t* rec, uint64_t seed, int32_t fp64) {
+    Handle* h = new Handle{fp64, nullptr, nullptr};
+    if (fp64) h->d = sim_create<double>(p, N, ntype, n_regions, region_start, row_ptr, tgt, w, delay, rec, seed);
+    else      h->f = sim_create<float>(p, N, ntype, n_regions, region_start, row_ptr, tgt, w, delay, rec, seed);
+    return h;
+}
+void orc_sim_destroy(void* hv) { Handle* h = (Handle*)hv; delete h->f; delete h->d; delete h; }
+
+void orc_sim_step(void* hv, int64_t n_steps) {
+    Handle* h = (Handle*)hv;
+    for (int64_t k = 0; k < n_steps; ++k) { if (h->fp64) h->d->one_step(); else h->f->one_step(); }
+}
+
+#define BOTH(expr_f, expr_d) (h->fp64 ? (expr_d) : (expr_f))
+
+uint64_t orc_sim_step_index(void* hv) { Handle* h = (Handle*)hv; return BOTH(h->f->step, h->d->step); }
+uint64_t orc_sim_n_spikes(void* hv) { Handle* h = (Handle*)hv; return BOTH(h->f->spike_id.size(), h->d->spike_id.size()); }
+uint64_t orc_sim_n_events(void* hv) { Handle* h = (Handle*)hv; return BOTH(h->f->n_events, h->d->n_events); }
+uint64_t orc_sim_n_bg(void* hv) { Handle* h = (Handle*)hv; return BOTH(h->f->n_bg, h->d->n_bg); }
+int32_t orc_sim_overflow(void* hv) { Handle* h = (Handle*)hv; return BOTH(h->f->overflow, h->d->overflow); }
+
+void orc_sim_get_spikes(void* hv, uint64_t* steps, int32_t* ids) {
+    Handle* h = (Handle*)hv;
+    const std::vector<uint64_t>& st = h->fp64 ? h->d->spike_step : h->f->spike_step;
+    const std::vector<int32_t>& id = h->fp64 ? h->d->spike_id : h->f->spike_id;
+    std::copy(st.begin(), st.end(), steps); std::copy(id.begin(), id.end(), ids);
+}
+
+void orc_sim_log_arrivals(void* hv, int32_t on) { Handle* h = (Handle*)hv; if (h->fp64) h->d->log_arrivals = on; else h->f->log_arrivals = on; }
+uint64_t orc_sim_get_arrivals(void* hv, int32_t* out) {     // [steps][N][4]; returns element count
+    Handle* h = (Handle*)hv;
+    const std::vector<int32_t>& a = h->fp64 ? h->d->arrivals_log : h->f->arrivals_log;
+    if (out) std::copy(a.begin(), a.end(), out);
+    return a.size();
+}
+
+// state as double (exact for the fp32 mode): V[N], g[N][4]; ref[N]
+void orc_sim_get_state(void* hv, double* V, double* g, int32_t* ref) {
+    Handle* h = (Handle*)hv;
+    int64_t N = BOTH(h->f->N, h->d->N);
+    for (int64_t i = 0; i < N; ++i) {
+        V[i] = BOTH((double)h->f->V[(size_t)i], h->d->V[(size_t)i]);
+        for (int u = 0; u < 4; ++u) g[i * 4 + u] = BOTH((double)h->f->g[(size_t)i * 4 + u], h->d->g[(size_t)i * 4 + u]);
+        ref[i] = BOTH(h->f->ref[(size_t)i], h->d->ref[(size_t)i]);
+    }
+}
+void orc_sim_set_state(void* hv, const double* V, const double* g, const int32_t* ref) {
+    Handle* h = (Handle*)hv;
+    int64_t N = BOTH(h->f->N, h->d->N);
+    for (int64_t i = 0; i < N; ++i) {
+        if (h->fp64) h->d->V[(size_t)i] = V[i]; else h->f->V[(size_t)i] = (float)V[i];
+        for (int u = 0; u < 4; ++u) {
+            if (h->fp64) h->d->g[(size_t)i * 4 + u] = g[i * 4 + u]; else h->f->g[(size_t)i * 4 + u] = (float)g[i * 4 + u];
+        }
+        if (h->fp64) h->d->ref[(size_t)i] = ref[i]; else h->f->ref[(size_t)i] = ref[i];
+    }
+}
+// ring[D][N][4] int32
+void orc_sim_get_ring(void* hv, int32_t* out) {
+    Handle* h = (Handle*)hv;
+    const std::vector<int32_t>& r = h->fp64 ? h->d->ring : h->f->ring;
+    std::copy(r.begin(), r.end(), out);
+}
+void orc_sim_set_ring(void* hv, const int32_t* in) {
+    Handle* h = (Handle*)hv;
+    std::vector<int32_t>& r = h->fp64 ? h->d->ring : h->f->ring;
+    std::copy(in, in + r.size(), r.begin());
+}
+// spike counts per (window, region); returns number of windows available
+int64_t orc_sim_region_counts(void* hv, uint32_t* out, int64_t cap_windows) {
+    Handle* h = (Handle*)hv;
+    const std::vector<uint32_t>& rc = h->fp64 ? h->d->region_count : h->f->region_count;
+    int R = BOTH(h->f->n_regions, h->d->n_regions);
+    int64_t nw = (int64_t)(rc.size() / (size_t)R);
+    int64_t m = std::min(nw, cap_windows);
+    if (out) std::copy(rc.begin(), rc.begin() + (size_t)(m * R), out);
+    return nw;
+}
+
+// =============================================================================
+// 5. Dense brute force: the plain definition of what delivery sums (R-DENSE).
+//    arrivals[n][i][u] = sum_j Wq[u][i][j] * spike_j(n - d[i][j]), with the
+//    dense matrices built from the CSR and spikes given as a [T][N] 0/1 array.
+//    Integer arithmetic; must equal what the ring delivered, exactly.
+// =============================================================================
+void orc_dense_arrivals(int64_t N, int64_t T, int32_t S, const int64_t* row_ptr, const int32_t* tgt,
+                        const float* w, const uint8_t* delay, const uint8_t* rec,
+                        const uint8_t* spikes /*[T][N]*/, int64_t* arrivals /*[T][N][4]*/) {
+    std::vector<int64_t> Wq((size_t)4 * (size_t)N * (size_t)N, 0);
+    std::vector<int32_t> dd((size_t)N * (size_t)N, 0);
+    for (int64_t j = 0; j < N; ++j)
+        for (int64_t s = row_ptr[j]; s < row_ptr[j + 1]; ++s) {
+            int64_t i = tgt[s];
+            Wq[((size_t)rec[s] * (size_t)N + (size_t)i) * (size_t)N + (size_t)j] +=
+                (int64_t)std::lrintf(w[s] * (float)std::ldexp(1.0, S));
+            dd[(size_t)i * (size_t)N + (size_t)j] = delay[s];
+        }
+    for (int64_t n = 0; n < T; ++n)
+        for (int64_t i = 0; i < N; ++i)
+            for (int u = 0; u < 4; ++u) {
+                int64_t acc = 0;
+                for (int64_t j = 0; j < N; ++j) {
+                    int64_t d = dd[(size_t)i * (size_t)N + (size_t)j];
+                    if (d == 0 || n - d < 0) continue;
+                    acc += Wq[((size_t)u * (size_t)N + (size_t)i) * (size_t)N + (size_t)j] *
+                           (int64_t)spikes[(size_t)(n - d) * (size_t)N + (size_t)j];
+                }
+                arrivals[((size_t)n * (size_t)N + (size_t)i) * 4 + (size_t)u] = acc;
+            }
+}
+
+}  // extern "C"
