@@ -1,0 +1,217 @@
+/* ============================================================================
+ * db_b200.h -- C ABI of the B200-native single-GPU step loop of the Digital
+ * Brain spiking-network simulator (arXiv 2211.15963).
+ *
+ * "P:L<n>" = line n of PAPER.md; "R<n>" = reading n in DESIGN.md.
+ *
+ * One iteration (SI "Numerical method" P:L469-490, Supp. Alg. 2
+ * P:L869-884):
+ *   neuron update   conductances  J_u(t+dt) = exp(-dt/tau_u) J_u(t) + arrivals   (SI Eq.(3))
+ *                   membrane      C dV/dt = -g_L (V - V_L) + sum_u g_u (V_u - V) J_u + I_bg + I_ext
+ *                                 stepped with first-order Euler (SI Eq.(5), R1)
+ *                   threshold / reset / refractory clamp
+ *   spike list      stack the spiking neurons                                    (Alg. 2 line 2)
+ *   delivery        push each spike along its destination list into the delayed,
+ *                   fixed-point per-receptor ring buffer with integer atomics    (Alg. 2 l.3-4)
+ *   region rates    firing rate of neuron groups
+ *
+ * Conventions
+ *   - Every function returns int32_t: DB_OK (0) or a negative DB_E* code; text
+ *     is available from db_last_error().  Nothing throws or aborts across the ABI.
+ *   - `db_sim` is opaque and owned by the library; db_destroy() frees it and all
+ *     device memory it obtained (through db_runtime.alloc/free when given, else
+ *     cudaMalloc/cudaFree).
+ *   - All pointer arguments are HOST pointers unless the name ends in `_dev`.
+ *     Output buffers are caller-allocated with a capacity in elements; the call
+ *     writes at most that many and reports the total available.
+ *   - All device work is enqueued on db_runtime.stream (a cudaStream_t; NULL =
+ *     the legacy default stream).  db_step() is asynchronous; every db_read_* /
+ *     db_get_* / db_export_* call synchronises that stream first.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - There is no CPU fallback: without a CUDA device every create call fails
+ *     with DB_ECUDA.
+ * ==========================================================================*/
+#ifndef DB_B200_H
+#define DB_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DB_OK       0
+#define DB_EINVAL  (-1)   /* bad argument / spec out of the supported range */
+#define DB_ENOMEM  (-2)   /* host or device allocation failed */
+#define DB_ECUDA   (-3)   /* CUDA runtime error (no device, launch failure, ...) */
+#define DB_ERANGE  (-4)   /* requested steps / elements are not (or no longer) available */
+#define DB_ESTATE  (-5)   /* call not valid in the current state of the handle */
+
+#define DB_MAX_TYPES 4    /* neuron types; 0 = excitatory, 1 = inhibitory */
+#define DB_N_RECEPTORS 4  /* 0 AMPA, 1 NMDA, 2 GABA_A, 3 GABA_B */
+
+typedef struct db_sim db_sim;
+
+/* Per neuron type constants: the paper's property table (Supp. Table 5,
+ * P:L816-832), held per type instead of per neuron (R-D1).  Units ms / mV;
+ * with C = 1, g_L = 1/tau_m. */
+typedef struct db_type_params {
+    double C, gL, VL, Vth, Vreset, Tref_ms, Iext;
+    double G[DB_N_RECEPTORS];       /* g_u, maximal conductance */
+    double E[DB_N_RECEPTORS];       /* V_u, reversal potential */
+    double tau_ms[DB_N_RECEPTORS];  /* tau_u */
+    double bg_rate_hz;              /* Poisson background rate per neuron (R14) */
+    double bg_weight;               /* its weight; delivered to AMPA */
+} db_type_params;
+
+/* Execution mode of db_step(). */
+#define DB_EXEC_AUTO       0   /* library picks */
+#define DB_EXEC_KERNELS    1   /* two kernels per step (update+compaction, delivery), CUDA-graph replayed */
+#define DB_EXEC_PERSISTENT 2   /* one cooperative persistent kernel looping over the steps */
+
+typedef struct db_sim_params {
+    uint32_t struct_size;     /* = sizeof(db_sim_params) */
+    double   dt_ms;           /* 0.1 or 1 */
+    int32_t  S;               /* fixed-point shift of the ring: increment = lrintf(w * 2^S) (R28) */
+    int32_t  D;               /* ring depth in steps: power of two, > largest delay */
+    int32_t  window_steps;    /* region-rate window in steps (R24) */
+    int32_t  n_types;         /* 1..DB_MAX_TYPES */
+    db_type_params type[DB_MAX_TYPES];
+    uint64_t dyn_seed;        /* keys V0 and the Poisson background */
+    uint64_t raster_capacity; /* spikes kept for db_read_spikes (0 = default); older ones are overwritten */
+    uint32_t max_windows;     /* region-rate windows kept (0 = default 4096) */
+    int32_t  exec_mode;       /* DB_EXEC_* */
+} db_sim_params;
+
+/* Device memory and stream plumbing supplied by the caller (the Python binding
+ * backs alloc/free with torch tensors and passes torch's current stream). */
+typedef struct db_runtime {
+    void* (*alloc)(size_t bytes, void* user);   /* returns a DEVICE pointer, 256-byte aligned, or NULL */
+    void  (*free)(void* dev_ptr, void* user);
+    void*  user;
+    void*  stream;                               /* cudaStream_t */
+    int32_t device;                              /* CUDA device ordinal */
+} db_runtime;
+
+/* Synthetic network (stand-in for the paper's HRGCME generator, P:L408-439,
+ * P:L322-331; recipe in DESIGN.md "Generator"). */
+#define DB_MODE_FIXED_INDEGREE  0
+#define DB_MODE_OUTDEG_LOGNORMAL 1
+typedef struct db_network_spec {
+    uint32_t struct_size;        /* = sizeof(db_network_spec) */
+    int64_t  N;                  /* neurons, 2 <= N < 2^30 */
+    int32_t  n_regions;          /* contiguous id ranges; excitatory neurons first in each */
+    double   region_size_sigma;  /* sizes ~ lognormal(0, sigma), normalised to N */
+    double   exc_frac;           /* 0.8 */
+    int32_t  mode;               /* DB_MODE_* */
+    int32_t  K;                  /* in-degree per neuron (mode 0) */
+    double   intra_frac;         /* share of K drawn inside the own region (n_regions > 1) */
+    double   region_matrix_sigma;/* inter-region matrix ~ lognormal(0, sigma), zero diagonal, row-normalised */
+    double   outdeg_mean, outdeg_sigma; int32_t outdeg_cap;   /* mode 1 (R27) */
+    double   w_mu, w_sigma, w_scale, inh_mult, slow_frac;     /* weights (R11), NMDA / GABA_B share (R12) */
+    int32_t  delay_intra_min, delay_intra_max, delay_inter_min, delay_inter_max;  /* steps, 1..255 */
+    int32_t  weight_fp16;        /* store weights as binary16 (config 3) instead of fp32 */
+    db_sim_params sim;
+    const db_runtime* runtime;   /* may be NULL */
+} db_network_spec;
+
+/* A presynaptic-major CSR on the HOST: row j = destination list of neuron j. */
+typedef struct db_csr_view {
+    int64_t N, E;
+    int32_t n_regions;
+    const int64_t* region_start; /* [n_regions + 1] */
+    const uint8_t* ntype;        /* [N] neuron type index */
+    const int64_t* row_ptr;      /* [N + 1] */
+    const int32_t* tgt;          /* [E] target neuron */
+    const float*   w;            /* [E] weight */
+    const uint8_t* delay;        /* [E] delay in steps, 1 <= delay < D */
+    const uint8_t* rec;          /* [E] receptor 0..3 */
+    int32_t weight_fp16;         /* store on the device as binary16 (w must already be representable) */
+} db_csr_view;
+
+/* Library-allocated host copy of the network (db_export_csr); release with db_free_csr. */
+typedef struct db_csr_host {
+    int64_t N, E;
+    int32_t n_regions;
+    int64_t* region_start; uint8_t* ntype; int64_t* row_ptr;
+    int32_t* tgt; float* w; uint8_t* delay; uint8_t* rec;   /* rows sorted by (target, receptor) */
+} db_csr_host;
+
+typedef struct db_counters {
+    uint64_t steps;        /* time steps done */
+    uint64_t spikes;       /* spikes emitted */
+    uint64_t events;       /* synaptic events delivered = sum of out-degrees of spiking neurons */
+    uint64_t bg_events;    /* background Poisson events drawn */
+    uint32_t ring_overflow;/* sticky: some consumed ring cell exceeded 2^30 in magnitude (R28) */
+    uint32_t exec_mode;    /* DB_EXEC_* actually in use */
+} db_counters;
+
+/* Per-phase device time of the last db_step_profiled() call, in milliseconds. */
+typedef struct db_phase_times {
+    double update_ms;      /* neuron update + compaction (a1 + a2 + a4) */
+    double deliver_ms;     /* spike delivery (a3) */
+    double total_ms;       /* whole call on the stream */
+    uint64_t steps, spikes, events;   /* work done inside the call */
+} db_phase_times;
+
+#define DB_FIELD_V      0  /* float  [count] */
+#define DB_FIELD_G_AMPA 1  /* float  [count] */
+#define DB_FIELD_G_NMDA 2
+#define DB_FIELD_G_GABAA 3
+#define DB_FIELD_G_GABAB 4
+#define DB_FIELD_REF    5  /* int32  [count], refractory steps left */
+#define DB_FIELD_TYPE   6  /* uint8  [count] */
+#define DB_FIELD_RING   7  /* int32  [D][count][4] fixed-point arrivals, slot = step mod D */
+
+/* a0: generate the network on the device from `spec` (seed keys every draw of
+ * the generator), build the CSR and initialise the state (V0 keyed by
+ * spec->sim.dyn_seed). */
+int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out);
+
+/* Same, from a host CSR (tests, tiny networks, externally built networks). */
+int32_t db_create_from_csr(const db_sim_params* sim, const db_csr_view* csr,
+                           const db_runtime* runtime, db_sim** out);
+
+int32_t db_destroy(db_sim* sim);
+
+/* a1-a4 for n_steps consecutive time steps; asynchronous on the stream. */
+int32_t db_step(db_sim* sim, uint32_t n_steps);
+
+/* Same in DB_EXEC_KERNELS mode with CUDA events around every kernel; blocks
+ * until done.  For per-kernel roofline measurement. */
+int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out);
+
+/* Spikes with step_begin <= step < step_end, sorted by (step, id).  Writes at
+ * most `cap` pairs, *n_out = number available.  DB_ERANGE if part of the range
+ * was already overwritten in the raster ring or lies in the future. */
+int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end,
+                       uint64_t* steps, int32_t* ids, uint64_t cap, uint64_t* n_out);
+
+/* State of neurons [first, first+count) into dst (layout per DB_FIELD_*). */
+int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, void* dst);
+/* Test hook: overwrite state (identical-state one-step parity). */
+int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, const void* src);
+
+/* Firing rate in Hz per (window, region) for the completed windows still kept:
+ * spikes / (region size * window seconds) (R24).  rates_hz[w * n_regions + r];
+ * *first_window = index of the first window returned. */
+int32_t db_region_rates(db_sim* sim, float* rates_hz, uint64_t cap_windows,
+                        uint64_t* n_windows, uint64_t* first_window);
+/* The integer counts behind them (same indexing). */
+int32_t db_region_counts(db_sim* sim, uint32_t* counts, uint64_t cap_windows,
+                         uint64_t* n_windows, uint64_t* first_window);
+
+int32_t db_export_csr(db_sim* sim, db_csr_host* out);
+int32_t db_free_csr(db_csr_host* csr);
+
+int32_t db_get_counters(db_sim* sim, db_counters* out);
+int32_t db_synchronize(db_sim* sim);
+
+/* Text of the last error on this handle (sim == NULL: last create error of this thread). */
+const char* db_last_error(const db_sim* sim);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DB_B200_H */

@@ -62,6 +62,11 @@ def lib():
         L.orc_generate.restype = C.POINTER(Network)
         L.orc_generate.argtypes = [C.POINTER(NetSpec), C.c_uint64]
         L.orc_network_free.argtypes = [C.POINTER(Network)]
+        L.orc_gen_create.restype = C.c_void_p
+        L.orc_gen_create.argtypes = [C.POINTER(NetSpec), C.c_uint64]
+        L.orc_gen_destroy.argtypes = [C.c_void_p]
+        L.orc_gen_owner_edges.restype = C.c_int64
+        L.orc_gen_owner_edges.argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 5
         L.orc_sim_create.restype = C.c_void_p
         L.orc_sim_create.argtypes = [C.POINTER(SimParams), C.c_int64, C.c_void_p, C.c_int32, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -189,6 +194,35 @@ def generate(net: dict, seed: int) -> dict:
     )
     L.orc_network_free(h)
     return out
+
+
+class OwnerEdges:
+    """The synapses owned by single neurons (their K inputs, or in out-degree mode their
+    outputs), without building the whole network: sampled parity at full size."""
+
+    def __init__(self, net: dict, seed: int):
+        sp = _net_spec(net)
+        self.h = lib().orc_gen_create(C.byref(sp), int(seed))
+        self.cap = max(int(net["K"]), int(net["outdeg_cap"])) + 1
+
+    def __call__(self, i: int) -> dict:
+        cap = self.cap
+        src, tgt = np.zeros(cap, np.int32), np.zeros(cap, np.int32)
+        w, d, r = np.zeros(cap, np.float32), np.zeros(cap, np.uint8), np.zeros(cap, np.uint8)
+        n = lib().orc_gen_owner_edges(self.h, int(i), cap, _p(src), _p(tgt), _p(w), _p(d), _p(r))
+        assert n <= cap
+        return dict(src=src[:n], tgt=tgt[:n], w=w[:n], delay=d[:n], rec=r[:n])
+
+    def close(self):
+        if self.h:
+            lib().orc_gen_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 # ---- simulator ------------------------------------------------------------------

@@ -352,65 +352,47 @@ void orc_region_cdf(uint64_t seed, int32_t R, double sigma, uint32_t* T /*[R][R-
     }
 }
 
-orc_network* orc_generate(const orc_net_spec* sp, uint64_t seed) {
-    const int64_t N = sp->N;
-    const int R = sp->n_regions;
-    orc_network* net = (orc_network*)std::calloc(1, sizeof(orc_network));
-    net->N = N; net->n_regions = R;
-    net->region_start = (int64_t*)std::calloc((size_t)R + 1, sizeof(int64_t));
-    net->region_nexc = (int64_t*)std::calloc((size_t)R, sizeof(int64_t));
-    net->ntype = (uint8_t*)std::calloc((size_t)N, 1);
+// Tables and per-neuron draws of the generator.  `owner_edges(i)` appends the
+// synapses owned by neuron i: its K inputs (mode 0) or its outputs (mode 1).
+struct orc_gen {
+    orc_net_spec sp; uint64_t seed;
+    std::vector<int64_t> region_start, region_nexc;
+    std::vector<uint32_t> cdf;
+    std::vector<float> wtab;
+    std::vector<int32_t> dtab;
+    int K_intra, K_inter;
 
-    // regions and types -------------------------------------------------------
-    std::vector<int64_t> sizes((size_t)R);
-    if (R == 1) sizes[0] = N; else orc_region_sizes(seed, N, R, sp->region_size_sigma, sizes.data());
-    for (int r = 0; r < R; ++r) {
-        net->region_start[r + 1] = net->region_start[r] + sizes[(size_t)r];
-        net->region_nexc[r] = (int64_t)std::floor(sp->exc_frac * (double)sizes[(size_t)r] + 0.5);
-        for (int64_t l = 0; l < sizes[(size_t)r]; ++l)
-            net->ntype[net->region_start[r] + l] = (l < net->region_nexc[r]) ? 0 : 1;
+    bool is_inh(int64_t j) const {
+        int r = region_of(region_start.data(), sp.n_regions, j);
+        return (j - region_start[(size_t)r]) >= region_nexc[(size_t)r];
     }
-
-    std::vector<float> wtab(65536);
-    orc_weight_table(sp->w_mu, sp->w_sigma, sp->w_scale, wtab.data());
-    const uint32_t slow_thr = (uint32_t)std::floor(sp->slow_frac * 4294967296.0);
-    const float inh_mult = (float)sp->inh_mult;
-
     // attributes of the synapse drawn as (owner, slot): weight, delay, receptor
-    auto make_edge = [&](int64_t owner, int64_t slot, int64_t src, int64_t tgt, bool inter) {
+    Edge make_edge(int64_t owner, int64_t slot, int64_t src, int64_t tgt, bool inter) const {
         u32x4 o = draw(seed, STREAM_SYN, (uint64_t)owner, (uint64_t)slot);
         Edge e;
         e.src = (int32_t)src; e.tgt = (int32_t)tgt;
-        bool inh = net->ntype[src] != 0;
+        bool inh = is_inh(src);
         float w = wtab[o.w[0] >> 16];
-        if (inh) w = w * inh_mult;
-        if (sp->weight_fp16) w = round_to_half(w);
+        if (inh) w = w * (float)sp.inh_mult;
+        if (sp.weight_fp16) w = round_to_half(w);
         e.w = w;
-        int dmin = inter ? sp->delay_inter_min : sp->delay_intra_min;
-        int dmax = inter ? sp->delay_inter_max : sp->delay_intra_max;
+        int dmin = inter ? sp.delay_inter_min : sp.delay_intra_min;
+        int dmax = inter ? sp.delay_inter_max : sp.delay_intra_max;
         e.delay = (uint8_t)(dmin + (int)(((uint64_t)o.w[1] * (uint64_t)(dmax - dmin + 1)) >> 32));
-        int slow = (o.w[2] < slow_thr) ? 1 : 0;      // NMDA / GABA_B w.p. slow_frac (R12)
-        e.rec = (uint8_t)((inh ? 2 : 0) + slow);      // receptor class follows the SOURCE type
+        uint32_t slow_thr = (uint32_t)std::floor(sp.slow_frac * 4294967296.0);
+        int slow = (o.w[2] < slow_thr) ? 1 : 0;       // NMDA / GABA_B w.p. slow_frac (R12)
+        e.rec = (uint8_t)((inh ? 2 : 0) + slow);       // receptor class follows the SOURCE type
         return e;
-    };
-
-    std::vector<Edge> edges;
-    if (sp->mode == 0) {
-        // fixed in-degree K per target ("for each neuron, the number of
-        // synaptic inputs from each neuron population ...").
-        std::vector<uint32_t> cdf;
-        int K_intra = sp->K, K_inter = 0;
-        if (R > 1) {
-            K_intra = (int)std::floor(sp->intra_frac * (double)sp->K + 0.5);
-            K_inter = sp->K - K_intra;
-            cdf.resize((size_t)R * (size_t)(R - 1));
-            orc_region_cdf(seed, R, sp->region_matrix_sigma, cdf.data());
-        }
-        edges.reserve((size_t)N * (size_t)sp->K);
-        for (int64_t i = 0; i < N; ++i) {
-            int r = region_of(net->region_start, R, i);
-            int64_t base = net->region_start[r];
-            int64_t size = net->region_start[r + 1] - base;
+    }
+    void owner_edges(int64_t i, std::vector<Edge>& edges) const {
+        const int R = sp.n_regions;
+        const int64_t N = sp.N;
+        if (sp.mode == 0) {
+            // fixed in-degree K per target ("for each neuron, the number of
+            // synaptic inputs from each neuron population ...")
+            int r = region_of(region_start.data(), R, i);
+            int64_t base = region_start[(size_t)r];
+            int64_t size = region_start[(size_t)r + 1] - base;
             int64_t li = i - base;
             u32x4 k0 = draw(seed, STREAM_SRC, (uint64_t)i, 0);
             for (int k = 0; k < K_intra; ++k) {        // own region, any type, not self
@@ -425,25 +407,82 @@ orc_network* orc_generate(const orc_net_spec* sp, uint64_t seed) {
                 int rs = 0;
                 for (int m = 0; m < R - 1; ++m) if (u >= T[m]) ++rs;
                 // distinct slots s map to distinct neurons of region rs (prp is injective)
-                uint32_t j = prp((uint32_t)s, (uint32_t)net->region_nexc[rs], k1.w);
-                edges.push_back(make_edge(i, K_intra + s, net->region_start[rs] + j, i, true));
+                uint32_t j = prp((uint32_t)s, (uint32_t)region_nexc[(size_t)rs], k1.w);
+                edges.push_back(make_edge(i, K_intra + s, region_start[(size_t)rs] + j, i, true));
             }
-        }
-    } else {
-        // lognormal out-degree per source, targets uniform without replacement (R27)
-        std::vector<int32_t> dtab(65536);
-        orc_outdeg_table(sp->outdeg_mean, sp->outdeg_sigma, sp->outdeg_cap, dtab.data());
-        for (int64_t j = 0; j < N; ++j) {
-            int32_t deg = dtab[draw(seed, STREAM_DEG, (uint64_t)j, 0).w[0] >> 16];
+        } else {
+            // lognormal out-degree per source, targets uniform without replacement (R27)
+            int32_t deg = dtab[draw(seed, STREAM_DEG, (uint64_t)i, 0).w[0] >> 16];
             if ((int64_t)deg > N - 1) deg = (int32_t)(N - 1);
-            u32x4 k0 = draw(seed, STREAM_SRC, (uint64_t)j, 0);
+            u32x4 k0 = draw(seed, STREAM_SRC, (uint64_t)i, 0);
             for (int m = 0; m < deg; ++m) {
                 uint32_t t = prp((uint32_t)m, (uint32_t)(N - 1), k0.w);
-                if ((int64_t)t >= j) t += 1;
-                edges.push_back(make_edge(j, m, j, t, false));
+                if ((int64_t)t >= i) t += 1;
+                edges.push_back(make_edge(i, m, i, t, false));
             }
         }
     }
+};
+
+orc_gen* orc_gen_create(const orc_net_spec* sp, uint64_t seed) {
+    orc_gen* g = new orc_gen();
+    g->sp = *sp; g->seed = seed;
+    const int64_t N = sp->N;
+    const int R = sp->n_regions;
+    std::vector<int64_t> sizes((size_t)R);
+    if (R == 1) sizes[0] = N; else orc_region_sizes(seed, N, R, sp->region_size_sigma, sizes.data());
+    g->region_start.assign((size_t)R + 1, 0);
+    g->region_nexc.assign((size_t)R, 0);
+    for (int r = 0; r < R; ++r) {
+        g->region_start[(size_t)r + 1] = g->region_start[(size_t)r] + sizes[(size_t)r];
+        g->region_nexc[(size_t)r] = (int64_t)std::floor(sp->exc_frac * (double)sizes[(size_t)r] + 0.5);
+    }
+    g->wtab.resize(65536);
+    orc_weight_table(sp->w_mu, sp->w_sigma, sp->w_scale, g->wtab.data());
+    g->K_intra = sp->K; g->K_inter = 0;
+    if (sp->mode == 0 && R > 1) {
+        g->K_intra = (int)std::floor(sp->intra_frac * (double)sp->K + 0.5);
+        g->K_inter = sp->K - g->K_intra;
+        g->cdf.resize((size_t)R * (size_t)(R - 1));
+        orc_region_cdf(seed, R, sp->region_matrix_sigma, g->cdf.data());
+    }
+    if (sp->mode == 1) {
+        g->dtab.resize(65536);
+        orc_outdeg_table(sp->outdeg_mean, sp->outdeg_sigma, sp->outdeg_cap, g->dtab.data());
+    }
+    return g;
+}
+void orc_gen_destroy(orc_gen* g) { delete g; }
+
+// The synapses owned by neuron i, in slot order (sampled parity at full size).
+// Returns the count; writes at most cap entries.
+int64_t orc_gen_owner_edges(const orc_gen* g, int64_t i, int64_t cap, int32_t* src, int32_t* tgt,
+                            float* w, uint8_t* delay, uint8_t* rec) {
+    std::vector<Edge> e;
+    g->owner_edges(i, e);
+    for (int64_t k = 0; k < (int64_t)e.size() && k < cap; ++k) {
+        src[k] = e[(size_t)k].src; tgt[k] = e[(size_t)k].tgt; w[k] = e[(size_t)k].w;
+        delay[k] = e[(size_t)k].delay; rec[k] = e[(size_t)k].rec;
+    }
+    return (int64_t)e.size();
+}
+
+orc_network* orc_generate(const orc_net_spec* sp, uint64_t seed) {
+    const int64_t N = sp->N;
+    const int R = sp->n_regions;
+    orc_gen* g = orc_gen_create(sp, seed);
+    orc_network* net = (orc_network*)std::calloc(1, sizeof(orc_network));
+    net->N = N; net->n_regions = R;
+    net->region_start = (int64_t*)std::calloc((size_t)R + 1, sizeof(int64_t));
+    net->region_nexc = (int64_t*)std::calloc((size_t)R, sizeof(int64_t));
+    net->ntype = (uint8_t*)std::calloc((size_t)N, 1);
+    for (int r = 0; r <= R; ++r) net->region_start[r] = g->region_start[(size_t)r];
+    for (int r = 0; r < R; ++r) net->region_nexc[r] = g->region_nexc[(size_t)r];
+    for (int64_t i = 0; i < N; ++i) net->ntype[i] = g->is_inh(i) ? 1 : 0;
+
+    std::vector<Edge> edges;
+    for (int64_t i = 0; i < N; ++i) g->owner_edges(i, edges);
+    orc_gen_destroy(g);
 
     // presynaptic-major CSR, rows sorted by target ---------------------------------
     std::sort(edges.begin(), edges.end(), [](const Edge& a, const Edge& b) {

@@ -1,0 +1,692 @@
+// C ABI of the library (include/db_b200.h): handle management, host-side
+// constant tables, CSR upload, step scheduling (CUDA graph / persistent
+// kernel) and read-back.  All simulation work is done by the kernels in
+// db_step.cu and db_gen.cu; nothing here computes on the CPU what the step
+// path computes.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include "../../include/db_b200.h"
+#include "db_device.cuh"
+#include "db_host.h"
+
+using namespace dbk;
+
+static thread_local std::string g_create_error;
+
+struct db_sim {
+    SimDev dev{};
+    db_sim_params params{};
+    db_runtime rt{};
+    bool have_rt = false;
+    cudaStream_t stream = nullptr;
+    int device = 0, n_sm = 0;
+    std::vector<void*> allocs;
+    int64_t E = 0, Epad = 0;
+    uint64_t spike_cap = 0, work_cap = 0;
+    std::vector<int64_t> region_start;
+    uint8_t* ntype_dev = nullptr;
+    int exec_mode = DB_EXEC_KERNELS;
+    int deliver_grid = 0, persistent_grid = 0;
+    cudaGraphExec_t graph_exec = nullptr;
+    int graph_steps = 0;
+    std::vector<cudaEvent_t> prof_events;
+    std::string err;
+};
+
+namespace {
+
+#define CK(call)                                                                         \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            return fail(sim, DB_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+        }                                                                                \
+    } while (0)
+
+int32_t fail(db_sim* sim, int32_t code, const std::string& msg) {
+    if (sim) sim->err = msg;
+    g_create_error = msg;
+    return code;
+}
+
+void* dev_alloc(db_sim* sim, size_t bytes) {
+    if (bytes == 0) bytes = 256;
+    void* p = nullptr;
+    if (sim->have_rt && sim->rt.alloc) p = sim->rt.alloc(bytes, sim->rt.user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+    if (p) sim->allocs.push_back(p);
+    return p;
+}
+
+void dev_free_all(db_sim* sim) {
+    for (void* p : sim->allocs) {
+        if (sim->have_rt && sim->rt.free) sim->rt.free(p, sim->rt.user);
+        else cudaFree(p);
+    }
+    sim->allocs.clear();
+}
+
+template <typename T>
+int32_t alloc_zero(db_sim* sim, T** out, size_t count) {
+    *out = static_cast<T*>(dev_alloc(sim, count * sizeof(T)));
+    if (!*out) return fail(sim, DB_ENOMEM, "device allocation of " + std::to_string(count * sizeof(T)) + " bytes failed");
+    CK(cudaMemsetAsync(*out, 0, std::max<size_t>(count * sizeof(T), 1), sim->stream));
+    return DB_OK;
+}
+
+uint64_t next_pow2(uint64_t x) { uint64_t p = 1; while (p < x) p <<= 1; return p; }
+
+// Per-type constants, formed in double and rounded once to fp32 (DESIGN.md
+// "Arithmetic contract").  Poisson thresholds: c_m = c_{m-1} + p_m with
+// p_0 = exp(-lambda), p_m = (p_{m-1} * lambda) / m; T_m = floor(c_m * 2^32);
+// the table ends where it saturates.
+int32_t make_type_consts(db_sim* sim, const db_sim_params& sp, TypeConst* tc) {
+    for (int t = 0; t < sp.n_types; ++t) {
+        const db_type_params& q = sp.type[t];
+        if (!(q.C > 0) || !(q.gL >= 0) || !(q.Tref_ms >= 0) || !(q.bg_rate_hz >= 0))
+            return fail(sim, DB_EINVAL, "type parameters out of range");
+        TypeConst c{};
+        c.neg_gL = -(float)q.gL; c.VL = (float)q.VL; c.Vth = (float)q.Vth; c.Vreset = (float)q.Vreset;
+        c.kappa = (float)(sp.dt_ms / q.C); c.Iext = (float)q.Iext;
+        for (int u = 0; u < 4; ++u) {
+            if (!(q.tau_ms[u] > 0)) return fail(sim, DB_EINVAL, "tau_ms must be positive");
+            c.G[u] = (float)q.G[u]; c.E[u] = (float)q.E[u];
+            c.alpha[u] = (float)std::exp(-sp.dt_ms / q.tau_ms[u]);
+        }
+        const long R = std::lrint(q.Tref_ms / sp.dt_ms);
+        if (R < 0 || R > kRefMask) return fail(sim, DB_EINVAL, "Tref/dt must be within 0..4095 steps");
+        c.R = (int32_t)R;
+        const double wq = std::rint(q.bg_weight * std::ldexp(1.0, sp.S));
+        if (std::fabs(wq) > 1073741824.0) return fail(sim, DB_EINVAL, "bg_weight * 2^S overflows");
+        c.wq_bg = (int32_t)wq;
+        const double lambda = q.bg_rate_hz * sp.dt_ms * 1e-3;
+        double term = std::exp(-lambda), cum = 0.0;
+        int M = 0;
+        bool saturated = false;
+        for (int m = 0; m < kPoissonMax; ++m) {
+            cum += term;
+            const double thr = std::floor(cum * 4294967296.0);
+            if (thr >= 4294967295.0) { saturated = true; break; }
+            c.T[M++] = (uint32_t)thr;
+            term = term * lambda / (double)(m + 1);
+        }
+        if (!saturated) return fail(sim, DB_EINVAL, "bg_rate_hz * dt too large for the Poisson table");
+        c.M = M;
+        tc[t] = c;
+    }
+    return DB_OK;
+}
+
+int32_t check_sim_params(db_sim* sim, const db_sim_params* sp) {
+    if (!sp || sp->struct_size != sizeof(db_sim_params)) return fail(sim, DB_EINVAL, "db_sim_params.struct_size mismatch");
+    if (!(sp->dt_ms > 0)) return fail(sim, DB_EINVAL, "dt_ms must be positive");
+    if (sp->S < 0 || sp->S > 30) return fail(sim, DB_EINVAL, "S must be within 0..30");
+    if (sp->D < 2 || sp->D > 65536 || (sp->D & (sp->D - 1))) return fail(sim, DB_EINVAL, "D must be a power of two in 2..65536");
+    if (sp->window_steps < 1) return fail(sim, DB_EINVAL, "window_steps must be >= 1");
+    if (sp->n_types < 1 || sp->n_types > DB_MAX_TYPES) return fail(sim, DB_EINVAL, "n_types must be 1..4");
+    if (sp->exec_mode < DB_EXEC_AUTO || sp->exec_mode > DB_EXEC_PERSISTENT) return fail(sim, DB_EINVAL, "bad exec_mode");
+    return DB_OK;
+}
+
+int32_t open_device(db_sim* sim, const db_runtime* rt) {
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0)
+        return fail(sim, DB_ECUDA, "no CUDA device: this library has no CPU path");
+    if (rt) { sim->rt = *rt; sim->have_rt = true; sim->device = rt->device; sim->stream = (cudaStream_t)rt->stream; }
+    if (sim->device < 0 || sim->device >= n_dev) return fail(sim, DB_EINVAL, "bad device ordinal");
+    CK(cudaSetDevice(sim->device));
+    cudaDeviceProp prop{};
+    CK(cudaGetDeviceProperties(&prop, sim->device));
+    sim->n_sm = prop.multiProcessorCount;
+    return DB_OK;
+}
+
+// Everything except the CSR arrays: state, ring, lists, counters.
+int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_regions,
+                     const int64_t* region_start) {
+    SimDev& d = sim->dev;
+    sim->params = *sp;
+    if (N < 1 || N >= (1ll << 30)) return fail(sim, DB_EINVAL, "N must be within 1..2^30-1");
+    if (n_regions < 1 || n_regions > 65536) return fail(sim, DB_EINVAL, "n_regions must be 1..65536");
+    d.N = (int32_t)N;
+    d.Npad = (int32_t)(((N + kNeuronPad - 1) / kNeuronPad) * kNeuronPad);
+    d.D = sp->D; d.S = sp->S;
+    d.scale = (float)std::ldexp(1.0, -sp->S);
+    d.wscale = (float)std::ldexp(1.0, sp->S);
+    d.seed_lo = (uint32_t)sp->dyn_seed; d.seed_hi = (uint32_t)(sp->dyn_seed >> 32);
+    d.window_steps = sp->window_steps;
+    d.max_windows = sp->max_windows ? sp->max_windows : 4096u;
+    if (d.max_windows < 4) return fail(sim, DB_EINVAL, "max_windows must be >= 4");
+    d.n_regions = n_regions;
+    int32_t rc = make_type_consts(sim, *sp, d.tc);
+    if (rc) return rc;
+
+    sim->region_start.assign(region_start, region_start + n_regions + 1);
+    if (sim->region_start.front() != 0 || sim->region_start.back() != N)
+        return fail(sim, DB_EINVAL, "region_start must run from 0 to N");
+    std::vector<int32_t> rs32((size_t)n_regions + 1);
+    for (int r = 0; r <= n_regions; ++r) {
+        if (r && sim->region_start[(size_t)r] < sim->region_start[(size_t)r - 1])
+            return fail(sim, DB_EINVAL, "region_start must be non-decreasing");
+        rs32[(size_t)r] = (int32_t)sim->region_start[(size_t)r];
+    }
+
+    const size_t Np = (size_t)d.Npad;
+    if ((rc = alloc_zero(sim, &d.V, Np))) return rc;
+    if ((rc = alloc_zero(sim, &d.g, 4 * Np))) return rc;
+    if ((rc = alloc_zero(sim, &d.rt, Np))) return rc;
+    if ((rc = alloc_zero(sim, &d.ring, (size_t)d.D * 4 * Np))) return rc;
+    uint64_t cap = sp->raster_capacity ? sp->raster_capacity : (1ull << 24);
+    cap = next_pow2(std::max<uint64_t>(cap, (uint64_t)N));
+    sim->spike_cap = cap;
+    d.spike_mask = cap - 1;
+    if ((rc = alloc_zero(sim, &d.spike_ids, (size_t)cap))) return rc;
+    d.step_log_mask = (1u << 16) - 1u;
+    if ((rc = alloc_zero(sim, &d.step_end, (size_t)d.step_log_mask + 1))) return rc;
+    int32_t* rs_dev = nullptr;
+    if ((rc = alloc_zero(sim, &rs_dev, (size_t)n_regions + 1))) return rc;
+    CK(cudaMemcpyAsync(rs_dev, rs32.data(), rs32.size() * sizeof(int32_t), cudaMemcpyHostToDevice, sim->stream));
+    d.region_start = rs_dev;
+    if ((rc = alloc_zero(sim, &d.region_counts, (size_t)d.max_windows * (size_t)n_regions))) return rc;
+    if ((rc = alloc_zero(sim, &d.bg_parts, (size_t)kBgParts))) return rc;
+    if ((rc = alloc_zero(sim, &d.ctl, 1))) return rc;
+    if ((rc = alloc_zero(sim, &sim->ntype_dev, Np))) return rc;
+    return DB_OK;
+}
+
+// After the CSR is on the device: work list, execution mode, initial state.
+int32_t finish_setup(db_sim* sim, uint64_t work_cap) {
+    SimDev& d = sim->dev;
+    int32_t rc;
+    sim->work_cap = std::max<uint64_t>(work_cap, 1);
+    if ((rc = alloc_zero(sim, &d.work, (size_t)sim->work_cap))) return rc;
+    CK(launch_init_state(d, sim->ntype_dev, sim->stream));
+    sim->deliver_grid = sim->n_sm * 4;
+    CK(persistent_max_grid(d, sim->n_sm, &sim->persistent_grid));
+    int coop = 0;
+    CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device));
+    int mode = sim->params.exec_mode;
+    if (mode == DB_EXEC_AUTO) mode = DB_EXEC_KERNELS;
+    if (mode == DB_EXEC_PERSISTENT && (!coop || sim->persistent_grid < 1))
+        return fail(sim, DB_ECUDA, "cooperative launch not available for the persistent mode");
+    sim->exec_mode = mode;
+    CK(cudaStreamSynchronize(sim->stream));
+    return DB_OK;
+}
+
+int32_t build_graph(db_sim* sim) {
+    const int steps = 32;
+    cudaGraph_t graph = nullptr;
+    cudaStream_t cap = nullptr;
+    CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    CK(cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
+    for (int s = 0; s < steps; ++s) {
+        launch_update(sim->dev, cap);
+        launch_deliver(sim->dev, sim->deliver_grid, cap);
+    }
+    cudaError_t e = cudaStreamEndCapture(cap, &graph);
+    if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail(sim, DB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
+    e = cudaGraphInstantiate(&sim->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess) return fail(sim, DB_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
+    sim->graph_steps = steps;
+    return DB_OK;
+}
+
+int32_t read_ctl(db_sim* sim, Ctl* out) {
+    CK(cudaStreamSynchronize(sim->stream));
+    CK(cudaMemcpy(out, sim->dev.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost));
+    return DB_OK;
+}
+
+}  // namespace
+
+// ===========================================================================
+extern "C" {
+
+const char* db_last_error(const db_sim* sim) { return sim ? sim->err.c_str() : g_create_error.c_str(); }
+
+int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, const db_runtime* rt, db_sim** out) {
+    if (!out) return fail(nullptr, DB_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!csr || !csr->row_ptr || !csr->ntype || !csr->region_start) return fail(nullptr, DB_EINVAL, "csr is incomplete");
+    db_sim* sim = new (std::nothrow) db_sim();
+    if (!sim) return fail(nullptr, DB_ENOMEM, "host allocation failed");
+    auto bail = [&](int32_t rc) { g_create_error = sim->err; dev_free_all(sim); delete sim; return rc; };
+    int32_t rc;
+    if ((rc = check_sim_params(sim, sp))) return bail(rc);
+    if ((rc = open_device(sim, rt))) return bail(rc);
+    const int64_t N = csr->N, E = csr->E;
+    if (E < 0 || csr->row_ptr[0] != 0 || csr->row_ptr[N] != E) return bail(fail(sim, DB_EINVAL, "row_ptr must run from 0 to E"));
+    if (E > 0 && (!csr->tgt || !csr->w || !csr->delay || !csr->rec)) return bail(fail(sim, DB_EINVAL, "csr arrays missing"));
+    if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start))) return bail(rc);
+    SimDev& d = sim->dev;
+
+    // padded row layout + validation
+    std::vector<int64_t> row_begin((size_t)N);
+    std::vector<int32_t> row_len((size_t)N);
+    int64_t pos = 0;
+    uint64_t work_cap = 0;
+    for (int64_t j = 0; j < N; ++j) {
+        const int64_t len = csr->row_ptr[j + 1] - csr->row_ptr[j];
+        if (len < 0 || len > 0x7FFFFFFF) return bail(fail(sim, DB_EINVAL, "row_ptr must be non-decreasing"));
+        if (csr->ntype[j] >= sp->n_types) return bail(fail(sim, DB_EINVAL, "ntype out of range"));
+        row_begin[(size_t)j] = pos; row_len[(size_t)j] = (int32_t)len;
+        pos += (len + kRowAlign - 1) / kRowAlign * kRowAlign;
+        work_cap += (uint64_t)((len + kChunk - 1) / kChunk);
+    }
+    const int64_t Epad = pos + kRowAlign;
+    sim->E = E; sim->Epad = Epad;
+    std::vector<uint32_t> tr((size_t)Epad, 0u);
+    std::vector<uint8_t> dl((size_t)Epad, 1);
+    std::vector<float> wf;
+    std::vector<__half> wh;
+    if (csr->weight_fp16) wh.assign((size_t)Epad, __float2half(0.0f)); else wf.assign((size_t)Epad, 0.0f);
+    for (int64_t j = 0; j < N; ++j) {
+        int64_t o = row_begin[(size_t)j];
+        for (int64_t s = csr->row_ptr[j]; s < csr->row_ptr[j + 1]; ++s, ++o) {
+            if (csr->tgt[s] < 0 || csr->tgt[s] >= N) return bail(fail(sim, DB_EINVAL, "target out of range"));
+            if (csr->rec[s] > 3) return bail(fail(sim, DB_EINVAL, "receptor out of range"));
+            if (csr->delay[s] < 1 || csr->delay[s] >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
+            tr[(size_t)o] = ((uint32_t)csr->rec[s] << 30) | (uint32_t)csr->tgt[s];
+            dl[(size_t)o] = csr->delay[s];
+            if (csr->weight_fp16) wh[(size_t)o] = __float2half_rn(csr->w[s]); else wf[(size_t)o] = csr->w[s];
+        }
+    }
+    int64_t* rb_dev; int32_t* rl_dev; uint32_t* tr_dev; uint8_t* dl_dev; void* w_dev;
+    if ((rc = alloc_zero(sim, &rb_dev, (size_t)N))) return bail(rc);
+    if ((rc = alloc_zero(sim, &rl_dev, (size_t)N))) return bail(rc);
+    if ((rc = alloc_zero(sim, &tr_dev, (size_t)Epad))) return bail(rc);
+    if ((rc = alloc_zero(sim, &dl_dev, (size_t)Epad))) return bail(rc);
+    const size_t wbytes = (size_t)Epad * (csr->weight_fp16 ? 2 : 4);
+    uint8_t* wraw;
+    if ((rc = alloc_zero(sim, &wraw, wbytes))) return bail(rc);
+    w_dev = wraw;
+    auto up = [&](void* dst, const void* src, size_t bytes) {
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, sim->stream);
+    };
+    if (up(rb_dev, row_begin.data(), (size_t)N * 8) != cudaSuccess || up(rl_dev, row_len.data(), (size_t)N * 4) != cudaSuccess ||
+        up(tr_dev, tr.data(), (size_t)Epad * 4) != cudaSuccess || up(dl_dev, dl.data(), (size_t)Epad) != cudaSuccess ||
+        up(w_dev, csr->weight_fp16 ? (const void*)wh.data() : (const void*)wf.data(), wbytes) != cudaSuccess ||
+        up(sim->ntype_dev, csr->ntype, (size_t)N) != cudaSuccess || cudaStreamSynchronize(sim->stream) != cudaSuccess)
+        return bail(fail(sim, DB_ECUDA, std::string("CSR upload: ") + cudaGetErrorString(cudaGetLastError())));
+    d.row_begin = rb_dev; d.row_len = rl_dev; d.tgt_rec = tr_dev; d.delay = dl_dev; d.w = w_dev;
+    d.w_fp16 = csr->weight_fp16 ? 1 : 0;
+    if ((rc = finish_setup(sim, work_cap))) return bail(rc);
+    *out = sim;
+    return DB_OK;
+}
+
+int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
+    if (!out) return fail(nullptr, DB_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!spec || spec->struct_size != sizeof(db_network_spec)) return fail(nullptr, DB_EINVAL, "db_network_spec.struct_size mismatch");
+    db_sim* sim = new (std::nothrow) db_sim();
+    if (!sim) return fail(nullptr, DB_ENOMEM, "host allocation failed");
+    auto bail = [&](int32_t rc) { g_create_error = sim->err; dev_free_all(sim); delete sim; return rc; };
+    int32_t rc;
+    if ((rc = check_sim_params(sim, &spec->sim))) return bail(rc);
+    if ((rc = open_device(sim, spec->runtime))) return bail(rc);
+
+    GenHostTables tabs;
+    std::string gerr;
+    if (!gen_host_tables(*spec, seed, &tabs, &gerr)) return bail(fail(sim, DB_EINVAL, gerr));
+    if ((rc = setup_common(sim, &spec->sim, spec->N, spec->n_regions, tabs.region_start.data()))) return bail(rc);
+
+    GenAlloc ga;
+    ga.user = sim;
+    ga.alloc = [](void* u, size_t bytes) { return dev_alloc(static_cast<db_sim*>(u), bytes); };
+    GenResult gr;
+    cudaError_t ce = generate_network(*spec, seed, tabs, ga, sim->stream, sim->dev.Npad, sim->ntype_dev, &gr, &gerr);
+    if (ce != cudaSuccess) return bail(fail(sim, DB_ECUDA, "generator: " + gerr + " (" + cudaGetErrorString(ce) + ")"));
+    if (!gerr.empty()) return bail(fail(sim, gr.oom ? DB_ENOMEM : DB_EINVAL, "generator: " + gerr));
+    SimDev& d = sim->dev;
+    d.row_begin = gr.row_begin; d.row_len = gr.row_len; d.tgt_rec = gr.tgt_rec; d.delay = gr.delay; d.w = gr.w;
+    d.w_fp16 = spec->weight_fp16 ? 1 : 0;
+    sim->E = gr.E; sim->Epad = gr.Epad;
+    if (gr.max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
+    if ((rc = finish_setup(sim, gr.work_cap))) return bail(rc);
+    *out = sim;
+    return DB_OK;
+}
+
+int32_t db_destroy(db_sim* sim) {
+    if (!sim) return DB_EINVAL;
+    cudaSetDevice(sim->device);
+    cudaStreamSynchronize(sim->stream);
+    if (sim->graph_exec) cudaGraphExecDestroy(sim->graph_exec);
+    for (cudaEvent_t e : sim->prof_events) cudaEventDestroy(e);
+    dev_free_all(sim);
+    delete sim;
+    return DB_OK;
+}
+
+int32_t db_step(db_sim* sim, uint32_t n_steps) {
+    if (!sim) return DB_EINVAL;
+    if (n_steps == 0) return DB_OK;
+    CK(cudaSetDevice(sim->device));
+    if (sim->exec_mode == DB_EXEC_PERSISTENT) {
+        CK(launch_persistent(sim->dev, n_steps, sim->persistent_grid, sim->stream));
+        return DB_OK;
+    }
+    if (!sim->graph_exec && n_steps >= 32) { int32_t rc = build_graph(sim); if (rc) return rc; }
+    uint32_t left = n_steps;
+    while (sim->graph_exec && left >= (uint32_t)sim->graph_steps) {
+        CK(cudaGraphLaunch(sim->graph_exec, sim->stream));
+        left -= (uint32_t)sim->graph_steps;
+    }
+    for (; left; --left) {
+        CK(launch_update(sim->dev, sim->stream));
+        CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
+    }
+    return DB_OK;
+}
+
+int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
+    if (!sim || !out) return DB_EINVAL;
+    CK(cudaSetDevice(sim->device));
+    Ctl c0, c1;
+    int32_t rc;
+    if ((rc = read_ctl(sim, &c0))) return rc;
+    std::memset(out, 0, sizeof(*out));
+    const uint32_t batch = 256;
+    while (sim->prof_events.size() < 2 * batch + 1) {
+        cudaEvent_t e; CK(cudaEventCreate(&e)); sim->prof_events.push_back(e);
+    }
+    uint32_t left = n_steps;
+    while (left) {
+        const uint32_t b = std::min(left, batch);
+        CK(cudaEventRecord(sim->prof_events[0], sim->stream));
+        for (uint32_t s = 0; s < b; ++s) {
+            CK(launch_update(sim->dev, sim->stream));
+            CK(cudaEventRecord(sim->prof_events[2 * s + 1], sim->stream));
+            CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
+            CK(cudaEventRecord(sim->prof_events[2 * s + 2], sim->stream));
+        }
+        CK(cudaStreamSynchronize(sim->stream));
+        for (uint32_t s = 0; s < b; ++s) {
+            float a = 0, d = 0;
+            CK(cudaEventElapsedTime(&a, sim->prof_events[2 * s], sim->prof_events[2 * s + 1]));
+            CK(cudaEventElapsedTime(&d, sim->prof_events[2 * s + 1], sim->prof_events[2 * s + 2]));
+            out->update_ms += a; out->deliver_ms += d;
+        }
+        float t = 0;
+        CK(cudaEventElapsedTime(&t, sim->prof_events[0], sim->prof_events[2 * b]));
+        out->total_ms += t;
+        left -= b;
+    }
+    if ((rc = read_ctl(sim, &c1))) return rc;
+    out->steps = c1.step - c0.step; out->spikes = c1.spike_begin - c0.spike_begin; out->events = c1.events - c0.events;
+    return DB_OK;
+}
+
+int32_t db_synchronize(db_sim* sim) {
+    if (!sim) return DB_EINVAL;
+    CK(cudaStreamSynchronize(sim->stream));
+    return DB_OK;
+}
+
+int32_t db_get_counters(db_sim* sim, db_counters* out) {
+    if (!sim || !out) return DB_EINVAL;
+    Ctl c;
+    int32_t rc = read_ctl(sim, &c);
+    if (rc) return rc;
+    std::vector<unsigned long long> parts(kBgParts);
+    CK(cudaMemcpy(parts.data(), sim->dev.bg_parts, kBgParts * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    uint64_t bg = 0;
+    for (auto v : parts) bg += v;
+    out->steps = c.step; out->spikes = c.spike_begin; out->events = c.events; out->bg_events = bg;
+    out->ring_overflow = c.overflow; out->exec_mode = (uint32_t)sim->exec_mode;
+    return DB_OK;
+}
+
+int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint64_t* steps, int32_t* ids,
+                       uint64_t cap, uint64_t* n_out) {
+    if (!sim || !n_out) return DB_EINVAL;
+    *n_out = 0;
+    Ctl c;
+    int32_t rc = read_ctl(sim, &c);
+    if (rc) return rc;
+    if (step_begin > step_end) return fail(sim, DB_EINVAL, "step_begin > step_end");
+    if (step_end > c.step) return fail(sim, DB_ERANGE, "steps not simulated yet");
+    if (step_begin == step_end) return DB_OK;
+    const uint64_t log_cap = (uint64_t)sim->dev.step_log_mask + 1;
+    const uint64_t first_log = step_begin ? step_begin - 1 : 0;      // first log entry needed
+    if (c.step - first_log > log_cap) return fail(sim, DB_ERANGE, "steps older than the step log");
+    const uint64_t n_log = step_end - first_log;                     // entries first_log .. step_end-1
+    std::vector<unsigned long long> ends((size_t)n_log);
+    for (uint64_t k = 0; k < n_log;) {                               // circular copy
+        const uint64_t idx = (first_log + k) & sim->dev.step_log_mask;
+        const uint64_t run = std::min<uint64_t>(n_log - k, log_cap - idx);
+        CK(cudaMemcpy(ends.data() + k, sim->dev.step_end + idx, (size_t)run * 8, cudaMemcpyDeviceToHost));
+        k += run;
+    }
+    const uint64_t seg_begin = step_begin ? ends[0] : 0ull;
+    const uint64_t seg_end = ends.back();
+    if (c.spike_begin - seg_begin > sim->spike_cap) return fail(sim, DB_ERANGE, "spikes already overwritten in the raster ring");
+    const uint64_t n = seg_end - seg_begin;
+    *n_out = n;
+    if (n == 0 || cap == 0) return DB_OK;
+    std::vector<int32_t> tmp((size_t)n);
+    for (uint64_t k = 0; k < n;) {
+        const uint64_t idx = (seg_begin + k) & sim->dev.spike_mask;
+        const uint64_t run = std::min<uint64_t>(n - k, sim->spike_cap - idx);
+        CK(cudaMemcpy(tmp.data() + k, sim->dev.spike_ids + idx, (size_t)run * 4, cudaMemcpyDeviceToHost));
+        k += run;
+    }
+    uint64_t o = 0, prev = seg_begin;
+    for (uint64_t s = step_begin; s < step_end && o < cap; ++s) {
+        const uint64_t e = ends[(size_t)(s - first_log)];
+        std::sort(tmp.begin() + (size_t)(prev - seg_begin), tmp.begin() + (size_t)(e - seg_begin));
+        for (uint64_t k = prev; k < e && o < cap; ++k, ++o) {
+            if (steps) steps[o] = s;
+            if (ids) ids[o] = tmp[(size_t)(k - seg_begin)];
+        }
+        prev = e;
+    }
+    return DB_OK;
+}
+
+int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, void* dst) {
+    if (!sim || !dst) return DB_EINVAL;
+    const SimDev& d = sim->dev;
+    if (first < 0 || count < 0 || first + count > d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds");
+    CK(cudaStreamSynchronize(sim->stream));
+    if (count == 0) return DB_OK;
+    const size_t Np = (size_t)d.Npad;
+    switch (field) {
+    case DB_FIELD_V:
+        CK(cudaMemcpy(dst, d.V + first, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;
+    case DB_FIELD_G_AMPA: case DB_FIELD_G_NMDA: case DB_FIELD_G_GABAA: case DB_FIELD_G_GABAB:
+        CK(cudaMemcpy(dst, d.g + (field - DB_FIELD_G_AMPA) * Np + first, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;
+    case DB_FIELD_REF: case DB_FIELD_TYPE: {
+        std::vector<uint16_t> t((size_t)count);
+        CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));
+        for (int64_t i = 0; i < count; ++i) {
+            if (field == DB_FIELD_REF) static_cast<int32_t*>(dst)[i] = t[(size_t)i] & kRefMask;
+            else static_cast<uint8_t*>(dst)[i] = (uint8_t)(t[(size_t)i] >> 12);
+        }
+        break;
+    }
+    case DB_FIELD_RING: {
+        std::vector<int32_t> t((size_t)count);
+        int32_t* o = static_cast<int32_t*>(dst);
+        for (int s = 0; s < d.D; ++s)
+            for (int u = 0; u < 4; ++u) {
+                CK(cudaMemcpy(t.data(), d.ring + ((size_t)s * 4 + u) * Np + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
+                for (int64_t i = 0; i < count; ++i) o[((size_t)s * (size_t)count + (size_t)i) * 4 + u] = t[(size_t)i];
+            }
+        break;
+    }
+    default: return fail(sim, DB_EINVAL, "unknown field");
+    }
+    return DB_OK;
+}
+
+int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, const void* src) {
+    if (!sim || !src) return DB_EINVAL;
+    const SimDev& d = sim->dev;
+    if (first < 0 || count < 0 || first + count > d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds");
+    CK(cudaStreamSynchronize(sim->stream));
+    if (count == 0) return DB_OK;
+    const size_t Np = (size_t)d.Npad;
+    switch (field) {
+    case DB_FIELD_V:
+        CK(cudaMemcpy(d.V + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
+    case DB_FIELD_G_AMPA: case DB_FIELD_G_NMDA: case DB_FIELD_G_GABAA: case DB_FIELD_G_GABAB:
+        CK(cudaMemcpy(d.g + (field - DB_FIELD_G_AMPA) * Np + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
+    case DB_FIELD_REF: {
+        std::vector<uint16_t> t((size_t)count);
+        CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));
+        for (int64_t i = 0; i < count; ++i) {
+            const int32_t r = static_cast<const int32_t*>(src)[i];
+            if (r < 0 || r > kRefMask) return fail(sim, DB_EINVAL, "ref out of range");
+            t[(size_t)i] = (uint16_t)((t[(size_t)i] & ~kRefMask) | r);
+        }
+        CK(cudaMemcpy(d.rt + first, t.data(), (size_t)count * 2, cudaMemcpyHostToDevice));
+        break;
+    }
+    case DB_FIELD_RING: {
+        std::vector<int32_t> t((size_t)count);
+        const int32_t* in = static_cast<const int32_t*>(src);
+        for (int s = 0; s < d.D; ++s)
+            for (int u = 0; u < 4; ++u) {
+                for (int64_t i = 0; i < count; ++i) t[(size_t)i] = in[((size_t)s * (size_t)count + (size_t)i) * 4 + u];
+                CK(cudaMemcpy(d.ring + ((size_t)s * 4 + u) * Np + first, t.data(), (size_t)count * 4, cudaMemcpyHostToDevice));
+            }
+        break;
+    }
+    default: return fail(sim, DB_EINVAL, "field is not writable");
+    }
+    return DB_OK;
+}
+
+static int32_t region_windows(db_sim* sim, std::vector<uint32_t>* counts, uint64_t cap_windows,
+                              uint64_t* n_windows, uint64_t* first_window) {
+    Ctl c;
+    int32_t rc = read_ctl(sim, &c);
+    if (rc) return rc;
+    const SimDev& d = sim->dev;
+    const uint64_t done = c.step / (uint64_t)d.window_steps;           // completed windows
+    const uint64_t keep = (uint64_t)d.max_windows - 2;                  // the two newest slots may be in flux
+    const uint64_t first = done > keep ? done - keep : 0;
+    uint64_t n = done - first;
+    if (first_window) *first_window = first;
+    if (n_windows) *n_windows = n;
+    n = std::min(n, cap_windows);
+    counts->resize((size_t)n * (size_t)d.n_regions);
+    for (uint64_t k = 0; k < n;) {
+        const uint64_t idx = (first + k) % d.max_windows;
+        const uint64_t run = std::min<uint64_t>(n - k, d.max_windows - idx);
+        CK(cudaMemcpy(counts->data() + (size_t)k * d.n_regions, d.region_counts + (size_t)idx * d.n_regions,
+                      (size_t)run * d.n_regions * 4, cudaMemcpyDeviceToHost));
+        k += run;
+    }
+    return DB_OK;
+}
+
+int32_t db_region_counts(db_sim* sim, uint32_t* counts, uint64_t cap_windows, uint64_t* n_windows, uint64_t* first_window) {
+    if (!sim) return DB_EINVAL;
+    std::vector<uint32_t> c;
+    int32_t rc = region_windows(sim, &c, counts ? cap_windows : 0, n_windows, first_window);
+    if (rc) return rc;
+    if (counts) std::copy(c.begin(), c.end(), counts);
+    return DB_OK;
+}
+
+int32_t db_region_rates(db_sim* sim, float* rates_hz, uint64_t cap_windows, uint64_t* n_windows, uint64_t* first_window) {
+    if (!sim) return DB_EINVAL;
+    std::vector<uint32_t> c;
+    int32_t rc = region_windows(sim, &c, rates_hz ? cap_windows : 0, n_windows, first_window);
+    if (rc) return rc;
+    if (!rates_hz) return DB_OK;
+    const int R = sim->dev.n_regions;
+    const double win_s = (double)sim->dev.window_steps * sim->params.dt_ms * 1e-3;
+    for (size_t k = 0; k < c.size(); ++k) {
+        const int r = (int)(k % (size_t)R);
+        const double size = (double)(sim->region_start[(size_t)r + 1] - sim->region_start[(size_t)r]);
+        rates_hz[k] = size > 0 ? (float)((double)c[k] / (size * win_s)) : 0.0f;
+    }
+    return DB_OK;
+}
+
+int32_t db_export_csr(db_sim* sim, db_csr_host* out) {
+    if (!sim || !out) return DB_EINVAL;
+    std::memset(out, 0, sizeof(*out));
+    const SimDev& d = sim->dev;
+    CK(cudaStreamSynchronize(sim->stream));
+    const int64_t N = d.N;
+    std::vector<int64_t> rb((size_t)N);
+    std::vector<int32_t> rl((size_t)N);
+    CK(cudaMemcpy(rb.data(), d.row_begin, (size_t)N * 8, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(rl.data(), d.row_len, (size_t)N * 4, cudaMemcpyDeviceToHost));
+    std::vector<uint32_t> tr((size_t)sim->Epad);
+    std::vector<uint8_t> dl((size_t)sim->Epad);
+    CK(cudaMemcpy(tr.data(), d.tgt_rec, (size_t)sim->Epad * 4, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(dl.data(), d.delay, (size_t)sim->Epad, cudaMemcpyDeviceToHost));
+    std::vector<float> wf((size_t)sim->Epad);
+    if (d.w_fp16) {
+        std::vector<__half> wh((size_t)sim->Epad);
+        CK(cudaMemcpy(wh.data(), d.w, (size_t)sim->Epad * 2, cudaMemcpyDeviceToHost));
+        for (size_t k = 0; k < wh.size(); ++k) wf[k] = __half2float(wh[k]);
+    } else {
+        CK(cudaMemcpy(wf.data(), d.w, (size_t)sim->Epad * 4, cudaMemcpyDeviceToHost));
+    }
+    int64_t E = 0;
+    for (int64_t j = 0; j < N; ++j) E += rl[(size_t)j];
+    out->N = N; out->E = E; out->n_regions = d.n_regions;
+    out->region_start = (int64_t*)std::malloc(sizeof(int64_t) * ((size_t)d.n_regions + 1));
+    out->ntype = (uint8_t*)std::malloc((size_t)N);
+    out->row_ptr = (int64_t*)std::malloc(sizeof(int64_t) * ((size_t)N + 1));
+    const size_t En = (size_t)std::max<int64_t>(E, 1);
+    out->tgt = (int32_t*)std::malloc(4 * En); out->w = (float*)std::malloc(4 * En);
+    out->delay = (uint8_t*)std::malloc(En); out->rec = (uint8_t*)std::malloc(En);
+    if (!out->region_start || !out->ntype || !out->row_ptr || !out->tgt || !out->w || !out->delay || !out->rec) {
+        db_free_csr(out);
+        return fail(sim, DB_ENOMEM, "host allocation failed");
+    }
+    std::copy(sim->region_start.begin(), sim->region_start.end(), out->region_start);
+    CK(cudaMemcpy(out->ntype, sim->ntype_dev, (size_t)N, cudaMemcpyDeviceToHost));
+    std::vector<int32_t> order;
+    int64_t o = 0;
+    out->row_ptr[0] = 0;
+    for (int64_t j = 0; j < N; ++j) {
+        const int64_t b = rb[(size_t)j];
+        const int32_t len = rl[(size_t)j];
+        order.resize((size_t)len);
+        for (int32_t k = 0; k < len; ++k) order[(size_t)k] = k;
+        std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {   // canonical: by (target, receptor)
+            const uint32_t a = tr[(size_t)(b + x)], c = tr[(size_t)(b + y)];
+            const uint32_t ta = a & 0x3FFFFFFFu, tc = c & 0x3FFFFFFFu;
+            if (ta != tc) return ta < tc;
+            return (a >> 30) < (c >> 30);
+        });
+        for (int32_t k = 0; k < len; ++k, ++o) {
+            const size_t s = (size_t)(b + order[(size_t)k]);
+            out->tgt[o] = (int32_t)(tr[s] & 0x3FFFFFFFu); out->rec[o] = (uint8_t)(tr[s] >> 30);
+            out->w[o] = wf[s]; out->delay[o] = dl[s];
+        }
+        out->row_ptr[j + 1] = o;
+    }
+    return DB_OK;
+}
+
+int32_t db_free_csr(db_csr_host* c) {
+    if (!c) return DB_EINVAL;
+    std::free(c->region_start); std::free(c->ntype); std::free(c->row_ptr);
+    std::free(c->tgt); std::free(c->w); std::free(c->delay); std::free(c->rec);
+    std::memset(c, 0, sizeof(*c));
+    return DB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,78 @@
+// Device-side data layout of one simulation (HBM), shared by the step kernels,
+// the generator and the C ABI.  See DESIGN.md "Data layout".
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace dbk {
+
+constexpr int kMaxTypes = 4;
+constexpr int kPoissonMax = 32;
+constexpr int kNeuronPad = 1024;     // Npad is a multiple of this: whole warps, 128-bit accesses
+constexpr int kRowAlign = 4;         // CSR rows start on a multiple of 4 synapses (128-bit target loads)
+constexpr int kChunk = 512;          // synapses per delivery work item (one warp)
+constexpr int kRefMask = 0x0FFF;     // rt = type << 12 | refractory steps left
+
+// Philox streams
+constexpr uint32_t kStreamV0 = 1, kStreamBG = 2, kStreamSRC = 3, kStreamSYN = 4,
+                   kStreamREGION = 5, kStreamINTER = 6, kStreamDEG = 7;
+
+struct TypeConst {                   // per neuron type, rounded once on the host
+    float neg_gL, VL, Vth, Vreset, kappa, Iext;
+    float G[4], E[4], alpha[4];
+    int32_t R;                       // refractory steps
+    int32_t wq_bg;                   // fixed-point background weight
+    int32_t M;                       // number of Poisson thresholds
+    uint32_t T[kPoissonMax];
+};
+
+struct Ctl {                         // device-resident control block
+    unsigned long long step;         // current time step n
+    unsigned long long spike_begin;  // spikes emitted before step n
+    unsigned long long step_counts[2];  // [n & 1] of step n: high 32 = spikes, low 32 = work items (one atomic)
+    unsigned long long events;       // synaptic events delivered so far
+    unsigned int overflow;           // sticky ring overflow flag
+    unsigned int done_blocks;        // delivery kernel: finished-block ticket
+    unsigned int bar_count;          // persistent kernel: grid barrier arrivals
+    unsigned int pad;
+    unsigned long long t_update, t_deliver;   // persistent kernel: accumulated phase time (ns, block 0)
+};
+
+constexpr int kBgParts = 1024;       // background-event counter is spread over this many cells
+
+struct SimDev {                      // passed by value to every kernel
+    int32_t N, Npad;
+    int32_t D, S;
+    float scale;                     // 2^-S
+    float wscale;                    // 2^S
+    uint32_t seed_lo, seed_hi;
+    // neuron state, structure of arrays
+    float* V;                        // [Npad]
+    float* g;                        // [4][Npad]
+    uint16_t* rt;                    // [Npad] type << 12 | ref
+    int32_t* ring;                   // [D][4][Npad] fixed-point arrivals
+    // presynaptic-major CSR
+    const int64_t* row_begin;        // [N] first synapse of row j (multiple of kRowAlign)
+    const int32_t* row_len;          // [N]
+    const uint32_t* tgt_rec;         // [Epad] receptor << 30 | target
+    const void* w;                   // [Epad] float or __half
+    const uint8_t* delay;            // [Epad]
+    int32_t w_fp16;
+    // spike list = raster ring; per-step work list
+    int32_t* spike_ids;              // [spike_cap] circular
+    unsigned long long spike_mask;
+    int2* work;                      // [work_cap] (neuron, chunk) of this step
+    unsigned long long* step_end;    // [step_log_cap] circular: spikes emitted up to and including step n
+    uint32_t step_log_mask;
+    // regions
+    const int32_t* region_start;     // [n_regions + 1]
+    int32_t n_regions;
+    uint32_t* region_counts;         // [max_windows][n_regions] circular
+    int32_t window_steps;
+    uint32_t max_windows;
+    unsigned long long* bg_parts;    // [kBgParts]
+    Ctl* ctl;
+    TypeConst tc[kMaxTypes];
+};
+
+}  // namespace dbk

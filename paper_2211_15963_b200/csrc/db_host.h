@@ -1,0 +1,48 @@
+// Host-side interfaces between the translation units of the library.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+#include <cuda_runtime.h>
+#include "../../include/db_b200.h"
+#include "db_device.cuh"
+
+namespace dbk {
+
+// ---- db_step.cu ------------------------------------------------------------
+cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
+cudaError_t launch_update(const SimDev& p, cudaStream_t st);
+cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);
+cudaError_t persistent_max_grid(const SimDev& p, int n_sm, int* grid);
+cudaError_t launch_persistent(const SimDev& p, unsigned n_steps, int grid, cudaStream_t st);
+
+// ---- db_gen.cu -------------------------------------------------------------
+struct GenHostTables {                 // distribution tables formed on the host in double
+    std::vector<int64_t> region_start; // [R + 1]
+    std::vector<int32_t> region_nexc;  // [R]
+    std::vector<uint32_t> region_cdf;  // [R][R - 1] cumulative thresholds of the inter-region matrix
+    std::vector<float> weight_tab;     // [65536] lognormal quantiles
+    std::vector<int32_t> outdeg_tab;   // [65536] (mode 1)
+    int32_t K_intra = 0, K_inter = 0;
+};
+
+bool gen_host_tables(const db_network_spec& spec, uint64_t seed, GenHostTables* out, std::string* err);
+
+struct GenAlloc { void* user; void* (*alloc)(void* user, size_t bytes); };
+
+struct GenResult {
+    int64_t* row_begin = nullptr; int32_t* row_len = nullptr;
+    uint32_t* tgt_rec = nullptr; void* w = nullptr; uint8_t* delay = nullptr;
+    int64_t E = 0, Epad = 0;
+    uint64_t work_cap = 0;
+    int32_t max_delay = 0;
+    bool oom = false;
+};
+
+// Builds the presynaptic-major CSR on the device.  Returns a CUDA error, or
+// cudaSuccess with *err non-empty for spec / memory problems.
+cudaError_t generate_network(const db_network_spec& spec, uint64_t seed, const GenHostTables& tabs,
+                             const GenAlloc& ga, cudaStream_t st, int32_t Npad, uint8_t* ntype_dev,
+                             GenResult* out, std::string* err);
+
+}  // namespace dbk

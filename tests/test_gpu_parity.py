@@ -1,0 +1,238 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, element by element,
+on the same seeded inputs.  Bars (BASELINE.json north_star): ring buffers bit-exact;
+one-step fp32 state within 1e-5 relative; identical raster for the first 200 steps of
+config 0; long-run rates within 2 %."""
+import numpy as np
+import pytest
+
+import db_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def db():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2211_15963_b200 as m
+    m.load()
+    return m
+
+
+def _ring_oracle_layout(sim):
+    return sim.db_read_state(7)            # [D][N][4], same layout as the oracle's ring()
+
+
+def _compare_state(g, o, rel=1e-5):
+    Vg, gg, rg = g.state()
+    Vo, go, ro = o.state()
+    assert np.array_equal(rg, ro)
+    assert np.all(np.abs(Vg - Vo) <= rel * np.abs(Vo))
+    assert np.all(np.abs(gg - go) <= rel * np.abs(go))
+    return float(np.max(np.abs(Vg - Vo))), float(np.max(np.abs(gg - go)))
+
+
+def _compare_raster(g, o, step_end, step_begin=0):
+    sg, ig = g.db_read_spikes(step_begin, step_end)
+    so, io = o.spikes()
+    m = (so >= step_begin) & (so < step_end)
+    so, io = so[m], io[m]
+    order = np.lexsort((io, so))
+    assert np.array_equal(sg, so[order]) and np.array_equal(ig, io[order])
+    return len(ig)
+
+
+def _pair(db, oracle_mod, sim, net, mode, seed=db_inputs.DYN_SEED, fp16=False, **kw):
+    g = db.Sim.db_create_from_csr(sim, net, dyn_seed=seed, exec_mode=mode, fp16=fp16, **kw)
+    o = oracle_mod.OracleSim(sim, net, seed)
+    return g, o
+
+
+MODES = [1, 2]   # DB_EXEC_KERNELS, DB_EXEC_PERSISTENT
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_initial_state_matches(db, oracle_mod, mode):
+    net = db_inputs.random_csr(N=3000, mean_outdeg=20, seed=1)
+    g, o = _pair(db, oracle_mod, db_inputs.sim_params(), net, mode)
+    dv, dg = _compare_state(g, o, rel=0.0)
+    assert dv == 0.0 and dg == 0.0
+    assert np.array_equal(g.db_read_state(6), net["ntype"])
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_one_step_from_identical_random_state(db, oracle_mod, mode):
+    # identical arbitrary state on both sides (incl. a random ring), one step, compare everything
+    N = 5000 + 37                                   # several tiles and a ragged tail
+    net = db_inputs.random_csr(N=N, mean_outdeg=25, seed=3)
+    sim = db_inputs.sim_params()
+    g, o = _pair(db, oracle_mod, sim, net, mode)
+    rng = np.random.default_rng(0)
+    V = rng.uniform(-75.0, -49.0, N).astype(np.float32)          # some already above threshold
+    gg = rng.gamma(1.0, 0.05, (N, 4)).astype(np.float32)
+    ref = np.where(rng.random(N) < 0.1, rng.integers(1, 50, N), 0).astype(np.int32)
+    ring = np.where(rng.random((sim["D"], N, 4)) < 0.2, rng.integers(-50000, 200000, (sim["D"], N, 4)), 0).astype(np.int32)
+    g.set_state(V, gg, ref); g.db_write_state(7, ring)
+    o.set_state(V, gg, ref); o.set_ring(ring)
+    assert np.array_equal(_ring_oracle_layout(g), ring)
+    g.db_step(1); o.step(1)
+    dv, dg = _compare_state(g, o)                                  # bar: 1e-5 relative
+    assert dv == 0.0 and dg == 0.0                                 # the contract gives bit-equality
+    assert np.array_equal(_ring_oracle_layout(g), o.ring())        # bit-exact fixed point
+    n = _compare_raster(g, o, 1)
+    assert n > 50
+    cg, co = g.db_get_counters(), o.counters()
+    for k in ("steps", "spikes", "events", "bg_events"):
+        assert cg[k] == co[k], k
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_config0_raster_identical_200_steps_and_ring_bit_exact(db, oracle_mod, mode):
+    cfg = db_inputs.config(0)
+    net = oracle_mod.generate(cfg["net"], db_inputs.GEN_SEED)
+    g, o = _pair(db, oracle_mod, cfg["sim"], net, mode)
+    for upto in (1, 7, 50, 200):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        assert np.array_equal(_ring_oracle_layout(g), o.ring())
+        _compare_state(g, o)
+    n = _compare_raster(g, o, 200)
+    assert n > 500
+    # longer run: the whole config-0 raster, rates within 2 % (they are in fact identical)
+    g.db_step(800); o.step(800)
+    n = _compare_raster(g, o, 1000)
+    assert np.array_equal(_ring_oracle_layout(g), o.ring())
+    cg, co = g.db_get_counters(), o.counters()
+    assert cg["events"] == co["events"] and cg["bg_events"] == co["bg_events"] and cg["ring_overflow"] == 0
+    rate = n / cfg["net"]["N"] / (1000 * cfg["sim"]["dt_ms"] * 1e-3)
+    assert 4.0 < rate < 11.0                                       # the ~7 Hz workload
+    cnt, first = g.db_region_counts()
+    oc = o.region_counts()
+    assert first == 0 and np.array_equal(cnt, oc[:len(cnt)]) and len(cnt) == 100
+    rates, _ = g.db_region_rates()
+    want = o.region_rates([cfg["net"]["N"]])[:len(rates)]
+    assert np.all(np.abs(rates - want) <= 0.02 * np.maximum(want, 1e-9))
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("case", ["empty", "one", "ragged", "heavy", "regions_fp16", "maxdelay"])
+def test_edge_cases(db, oracle_mod, mode, case):
+    sim = db_inputs.sim_params()
+    strong = db_inputs.type_params(bg_weight=0.03)
+    sim["types"] = [strong, dict(strong)]
+    fp16 = False
+    steps = 120
+    if case == "empty":                       # no synapses at all
+        net = db_inputs.random_csr(N=700, mean_outdeg=0, seed=1)
+        assert net["E"] == 0
+    elif case == "one":                       # a single neuron
+        net = db_inputs.random_csr(N=1, mean_outdeg=0, seed=1)
+    elif case == "ragged":                    # N not a multiple of anything
+        net = db_inputs.random_csr(N=1025 + 511, mean_outdeg=12, seed=5)
+    elif case == "heavy":                     # rows spanning several delivery chunks next to empty rows
+        net = db_inputs.random_csr(N=4000, mean_outdeg=3, seed=6, heavy_rows={0: 3999, 17: 1500, 3999: 513, 5: 512, 6: 0})
+    elif case == "regions_fp16":              # region counters + binary16 weights
+        net = db_inputs.random_csr(N=2500, mean_outdeg=30, seed=7, n_regions=7, fp16=True)
+        fp16 = True
+        sim["window_steps"] = 7
+    else:                                     # delays 1 and D-1 both present
+        net = db_inputs.random_csr(N=900, mean_outdeg=20, seed=8, max_delay=sim["D"] - 1)
+        assert net["delay"].min() == 1 and net["delay"].max() == sim["D"] - 1
+    g, o = _pair(db, oracle_mod, sim, net, mode, fp16=fp16)
+    if case == "heavy":                       # make the heavy rows fire in step 0
+        V, gg, ref = o.state()
+        V[[0, 17, 3999, 5, 6]] = -40.0
+        o.set_state(V, gg, ref); g.set_state(V.astype(np.float32), gg.astype(np.float32), ref)
+    g.db_step(steps); o.step(steps)
+    _compare_state(g, o)
+    assert np.array_equal(_ring_oracle_layout(g), o.ring())
+    n = _compare_raster(g, o, steps)
+    if case not in ("one",):
+        assert n > 0
+    cg, co = g.db_get_counters(), o.counters()
+    for k in ("steps", "spikes", "events", "bg_events"):
+        assert cg[k] == co[k], k
+    cnt, first = g.db_region_counts()
+    assert np.array_equal(cnt, o.region_counts()[first:first + len(cnt)])
+    assert len(cnt) == steps // sim["window_steps"]
+
+
+def test_modes_agree_and_split_stepping(db):
+    # kernels vs persistent, and db_step(a); db_step(b) == db_step(a + b) (graph replay + remainder)
+    cfg = db_inputs.config(0, scale=0.3)
+    a = db.Sim.db_create(cfg["net"], cfg["sim"], seed=5, dyn_seed=2, exec_mode=1)
+    b = db.Sim.db_create(cfg["net"], cfg["sim"], seed=5, dyn_seed=2, exec_mode=2)
+    a.db_step(100)
+    for n in (1, 31, 33, 35):
+        b.db_step(n)
+    assert np.array_equal(a.state()[0], b.state()[0])
+    assert np.array_equal(a.db_read_state(7), b.db_read_state(7))
+    sa, ia = a.db_read_spikes(0, 100); sb, ib = b.db_read_spikes(0, 100)
+    assert np.array_equal(sa, sb) and np.array_equal(ia, ib) and len(ia) > 20
+
+
+def test_read_spikes_ranges_and_errors(db):
+    cfg = db_inputs.config(0, scale=0.2)
+    s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=1, raster_capacity=1)   # capacity rounds up to N
+    s.db_step(300)
+    st, ids = s.db_read_spikes(100, 200)
+    assert np.all((st >= 100) & (st < 200)) and len(st) > 0
+    assert np.all(np.diff(st.astype(np.int64)) >= 0)
+    same = st[1:] == st[:-1]
+    assert np.all(np.diff(ids)[same] > 0)
+    assert len(s.db_read_spikes(250, 250)[0]) == 0
+    with pytest.raises(db.DbError) as e:
+        s.db_read_spikes(0, 301)
+    assert e.value.code == db.binding.DB_ERANGE
+    s.db_step(20000)                                  # the small raster ring wraps
+    with pytest.raises(db.DbError) as e:
+        s.db_read_spikes(0, 100)
+    assert e.value.code == db.binding.DB_ERANGE
+    assert len(s.db_read_spikes(20250, 20300)[0]) > 0
+    with pytest.raises(db.DbError):
+        s.db_read_state(0, first=0, count=s.N + 1)
+
+
+def test_bad_arguments_are_rejected(db):
+    sim = db_inputs.sim_params()
+    net = db_inputs.random_csr(N=100, mean_outdeg=5, seed=1)
+    bad = dict(net, delay=np.full_like(net["delay"], sim["D"]))
+    with pytest.raises(db.DbError) as e:
+        db.Sim.db_create_from_csr(sim, bad)
+    assert e.value.code == db.binding.DB_EINVAL
+    with pytest.raises(db.DbError):
+        db.Sim.db_create_from_csr(dict(sim, D=24), net)
+    with pytest.raises(db.DbError):
+        db.Sim.db_create(dict(db_inputs.config(0)["net"], N=50, K=100), sim, seed=1)
+
+
+# ------------------------------------------------------------------ generator parity
+def _assert_same_network(a, b):
+    for k in ("N", "E", "n_regions"):
+        assert a[k] == b[k], k
+    for k in ("region_start", "ntype", "row_ptr", "tgt", "rec", "delay", "w"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+@pytest.mark.parametrize("which", ["config0", "regions", "regions_fp16", "outdeg"])
+def test_generator_matches_oracle_generator(db, oracle_mod, which):
+    if which == "config0":
+        cfg = db_inputs.config(0)
+    elif which == "regions":
+        cfg = db_inputs.config(2, scale=0.01)             # 50,000 neurons, 200 regions
+    elif which == "regions_fp16":
+        cfg = db_inputs.config(3, scale=0.001)
+        cfg["net"].update(N=20_000, n_regions=12, K=300)
+    else:
+        cfg = db_inputs.config(4, scale=0.01)             # 20,000 neurons, lognormal out-degree
+        cfg["net"].update(outdeg_mean=120.0, outdeg_cap=3000)
+    want = oracle_mod.generate(cfg["net"], db_inputs.GEN_SEED)
+    s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED)
+    got = s.db_export_csr()
+    _assert_same_network(got, want)
+    # and the dynamics on the generated network follow the oracle on ITS network
+    o = oracle_mod.OracleSim(cfg["sim"], want, db_inputs.DYN_SEED)
+    s.db_step(150); o.step(150)
+    _compare_raster(s, o, 150)
+    assert np.array_equal(_ring_oracle_layout(s), o.ring())
+    cnt, first = s.db_region_counts()
+    assert np.array_equal(cnt, o.region_counts()[first:first + len(cnt)])

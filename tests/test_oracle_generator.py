@@ -209,3 +209,18 @@ def test_second_implementation_reproduces_small_network(oracle_mod):
     assert [e[2] for e in edges] == [float(x) for x in net["w"]]
     assert [e[3] for e in edges] == net["delay"].tolist()
     assert [e[4] for e in edges] == net["rec"].tolist()
+
+
+def test_owner_edges_match_full_generation(oracle_mod, net_regions):
+    spec, net = net_regions
+    oe = oracle_mod.OwnerEdges(spec, db_inputs.GEN_SEED)
+    src_all = _src_of(net)
+    for i in (0, 1, 777, spec["N"] - 1):
+        e = oe(i)
+        assert np.all(e["tgt"] == i) and len(e["src"]) == spec["K"]
+        m = net["tgt"] == i
+        order = np.argsort(e["src"], kind="stable")
+        assert np.array_equal(src_all[m], e["src"][order])
+        assert np.array_equal(net["w"][m], e["w"][order])
+        assert np.array_equal(net["delay"][m], e["delay"][order])
+        assert np.array_equal(net["rec"][m], e["rec"][order])
