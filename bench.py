@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (a1 update, a2 compaction, a3 delivery, a4 region
+rates) on BASELINE.json configs[1]: 1,000,000 LIF neurons, in-degree 100
+(1e8 synapses), dt = 0.1 ms, background tuned for ~7 Hz (``--rate 15|30`` for the other two).
+
+One bench "step" = one ``db_step(sim_steps)`` call = ``--sim-steps`` (default 1000) consecutive
+simulation time steps = 0.1 s of biological time.  The default run (``--steps 10``) is therefore
+the 10,000 steps / 1 s biological that configs[1] names, after ``--warmup`` (default 3) untimed
+bench steps that also carry the network past its start-up transient.
+
+Prints ONE JSON line (rank 0):
+  value         synaptic events/s (sum of out-degrees of spiking neurons / device time), whole job
+  e2e           same metric through the C ABI with HOST buffers: every bench step restores the neuron
+                state from pinned host memory (db_write_state), steps, and reads the raster, the
+                region rates and V back to the host (db_read_spikes / db_region_rates / db_read_state)
+  roofline      the dominant kernel (k_update) against the measured HBM copy peak
+  cpu_baseline  the oracle (oracle/, as it stands) on the host cores, on a bounded sample
+``--impl reference`` times the oracle instead (same metric, unit and config).
+
+Multi-GPU (torchrun): the path does not shard inside this build (replicas
+only) -- every rank simulates an independent replica (its own seeds); value = all ranks' events /
+max-over-ranks device time; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import db_inputs
+
+METRIC = "synaptic_events_per_s"
+UNIT = "events/s"
+
+# Algorithmic bytes.
+UPDATE_BYTES_PER_NEURON_STEP = 58      # read V 4 + g 16 + rt 2 + ring slot 16; write V 4 + g 16 (compulsory)
+UPDATE_BYTES_SURVEY = 76               # plus rt 2 and the zeroed slot 16 written back every step
+DELIVER_BYTES_PER_EVENT = {0: 17, 1: 15}   # tgt|rec 4 + w 4 (fp32) / 2 (fp16) + delay 1 + accumulator read 4 + write 4
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.device = device
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.device), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(rate_hz: int, scale: float, warm_steps: int, timed_steps: int, repeats: int = 1):
+    """Times the oracle as it stands (single thread) on configs[1] shrunk to `scale` (same in-degree,
+    weights, delays, background): returns a list of (seconds, events, neuron_updates) per repeat."""
+    import oracle
+    cfg = db_inputs.config(1, rate_hz=rate_hz, scale=scale)
+    net = oracle.generate(cfg["net"], db_inputs.GEN_SEED)
+    o = oracle.OracleSim(cfg["sim"], net, db_inputs.DYN_SEED)
+    o.step(warm_steps)
+    out = []
+    for _ in range(repeats):
+        e0 = o.counters()["events"]
+        t0 = time.perf_counter()
+        o.step(timed_steps)
+        dt = time.perf_counter() - t0
+        out.append((dt, o.counters()["events"] - e0, timed_steps * cfg["net"]["N"]))
+    o.close()
+    return out, cfg
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    scale = args.ref_scale
+    # the start-up transient runs at several times the steady rate: warm the oracle past part of it
+    warm = max(args.ref_sim_steps * args.warmup, args.ref_warm_steps)
+    res, cfg = oracle_sample(args.rate, scale, warm_steps=warm, timed_steps=args.ref_sim_steps, repeats=args.steps)
+    secs = sum(r[0] for r in res)
+    events = sum(r[1] for r in res)
+    updates = sum(r[2] for r in res)
+    value = events / secs
+    sample = (f"configs[1] shrunk to N={cfg['net']['N']} (in-degree 100, same distributions), "
+              f"{args.steps} x {args.ref_sim_steps} time steps after {warm} warm-up steps, "
+              f"single thread")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": dict(_config_dict(args, int(1_000_000 * args.scale), args.sim_steps),
+                       reference_sample={"n_neurons": cfg["net"]["N"], "sim_steps_per_bench_step": args.ref_sim_steps}),
+        "neuron_updates_per_s": updates / secs,
+        "rtf": secs / (args.steps * args.ref_sim_steps * cfg["sim"]["dt_ms"] * 1e-3),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def _config_dict(args, n_neurons, sim_steps):
+    return {"workload": f"configs[1]: {n_neurons} LIF neurons, in-degree 100, dt 0.1 ms, ~{args.rate} Hz",
+            "n_neurons": n_neurons, "in_degree": 100, "rate_hz_target": args.rate,
+            "sim_steps_per_bench_step": sim_steps, "dt_ms": 0.1,
+            "l2": "no flush: device footprint (state + ring + CSR ~1.4 GB) exceeds the 126 MB L2; the step loop "
+                  "runs back to back as in production"}
+
+
+# --------------------------------------------------------------------------------------------- CUDA arm
+def run_ours(args):
+    import torch
+    import paper_2211_15963_b200 as db
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU path); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    db.load()
+
+    cfg = db_inputs.config(1, rate_hz=args.rate, scale=args.scale)
+    N = cfg["net"]["N"]
+    n_sim = args.sim_steps
+    mode = {"auto": db.EXEC_AUTO, "kernels": db.EXEC_KERNELS, "persistent": db.EXEC_PERSISTENT}[args.exec_mode]
+    raster_cap = 1 << 25
+    sim = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED + rank, dyn_seed=db_inputs.DYN_SEED + rank,
+                           exec_mode=mode, raster_capacity=raster_cap, device=local)
+    fp16 = int(cfg["net"]["weight_fp16"])
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident throughput -------------------------------------------------
+    for _ in range(args.warmup):
+        sim.db_step(n_sim)
+    barrier()
+    c0 = sim.db_get_counters()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        sim.db_step(n_sim)
+    ev1.record()
+    barrier()
+    clk = clocks.stop() if rank == 0 else None
+    ms = ev0.elapsed_time(ev1)
+    c1 = sim.db_get_counters()
+    events = c1["events"] - c0["events"]
+    spikes = c1["spikes"] - c0["spikes"]
+    launches = c1["launches"] - c0["launches"]
+    t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
+    tot = torch.tensor([events, spikes, launches], dtype=torch.float64, device=f"cuda:{local}")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms_max = float(t.item())
+    events_all, spikes_all, launches_all = [float(x) for x in tot.tolist()]
+    secs = ms_max * 1e-3
+    bio_s = args.steps * n_sim * cfg["sim"]["dt_ms"] * 1e-3
+    value = events_all / secs
+    rate_hz = spikes_all / (world * N) / bio_s
+
+    # ---------------- per-kernel roofline (CUDA events around every kernel, on the library's stream) ----
+    prof = sim.db_step_profiled(args.profile_steps)
+    peak, peak_src = _peaks()
+    upd_s = prof["update_ms"] * 1e-3 / prof["steps"]
+    del_s = prof["deliver_ms"] * 1e-3 / prof["steps"]
+    upd_gbs = UPDATE_BYTES_PER_NEURON_STEP * N / upd_s / 1e9
+    del_bytes = DELIVER_BYTES_PER_EVENT[fp16] * prof["events"] / prof["steps"]
+    del_gbs = del_bytes / del_s / 1e9
+    roofline = {
+        "bound": "hbm", "kernel": "k_update", "achieved": upd_gbs, "peak": peak, "unit": "GB/s", "frac": upd_gbs / peak,
+        "traffic": None, "peak_source": peak_src,
+        "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
+        "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
+        "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
+        "deliver": {"kernel": "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
+                    "events_per_launch": prof["events"] / prof["steps"], "bytes_per_event": DELIVER_BYTES_PER_EVENT[fp16],
+                    "share_of_step": prof["deliver_ms"] / max(prof["total_ms"], 1e-12)},
+        "note": "per-step working set (state 22 MB + one ring slot 16 MB) is L2-resident at this size: achieved is "
+                "algorithmic bytes / time and may exceed the HBM copy peak",
+    }
+
+    # ---------------- end to end through the C ABI with host buffers --------------------------------
+    V_h = torch.empty(N, dtype=torch.float32).pin_memory()
+    g_h = [torch.empty(N, dtype=torch.float32).pin_memory() for _ in range(4)]
+    ref_h = torch.empty(N, dtype=torch.int32).pin_memory()
+    V_h.numpy()[:] = sim.db_read_state(db.FIELD_V)
+    for u in range(4):
+        g_h[u].numpy()[:] = sim.db_read_state(db.FIELD_G_AMPA + u)
+    ref_h.numpy()[:] = sim.db_read_state(db.FIELD_REF)
+    cap = int(3 * max(spikes / max(args.steps, 1), 1)) + 4096
+    st_h = torch.empty(cap, dtype=torch.int64).pin_memory()
+    id_h = torch.empty(cap, dtype=torch.int32).pin_memory()
+    st_np, id_np = st_h.numpy().view(np.uint64), id_h.numpy()
+    Vout_h = torch.empty(N, dtype=torch.float32).pin_memory()
+    C = db.binding.C
+
+    def e2e_step():
+        s0 = sim.db_get_counters()["steps"]
+        sim.db_write_state(db.FIELD_V, V_h.numpy())
+        for u in range(4):
+            sim.db_write_state(db.FIELD_G_AMPA + u, g_h[u].numpy())
+        sim.db_write_state(db.FIELD_REF, ref_h.numpy())
+        sim.db_step(n_sim)
+        st, ids = sim.db_read_spikes(s0, s0 + n_sim, st_np, id_np)
+        rates, _ = sim.db_region_rates()
+        sim.L.db_read_state(sim.h, db.FIELD_V, 0, N, C.c_void_p(Vout_h.data_ptr()))
+        return len(ids), rates.nbytes
+
+    e2e_step()                                   # warm
+    barrier()
+    ce0 = sim.db_get_counters()
+    t0 = time.perf_counter()
+    n_sp = 0
+    for _ in range(args.e2e_steps):
+        k, rate_bytes = e2e_step()
+        n_sp += k
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    ce1 = sim.db_get_counters()
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
+    ee = torch.tensor([float(ce1["events"] - ce0["events"])], dtype=torch.float64, device=f"cuda:{local}")
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ee, op=dist.ReduceOp.SUM)
+    e2e = {"value": float(ee.item()) / float(te.item()), "unit": UNIT,
+           "h2d_bytes_per_step": int(N * (4 + 16 + 4)),
+           "d2h_bytes_per_step": int(N * 4 + (n_sp // max(args.e2e_steps, 1)) * 12 + rate_bytes),
+           "steps": args.e2e_steps, "ms_per_step": 1e3 * float(te.item()) / args.e2e_steps,
+           "what": "db_write_state(V, g[4], ref) from pinned host + db_step + db_read_spikes + db_region_rates + "
+                   "db_read_state(V) to pinned host, wall clock"}
+
+    exec_used = sim.db_get_counters()["exec_mode"]
+    sim.db_destroy()
+
+    # ---------------- CPU baseline: the oracle on the host cores (rank 0, N = 1 only) ----------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        res, ocfg = oracle_sample(args.rate, args.ref_scale, warm_steps=args.ref_warm_steps, timed_steps=300)
+        dt_o, ev_o, up_o = res[0]
+        cpu = {"value": ev_o / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "neuron_updates_per_s": up_o / dt_o,
+               "sample": f"configs[1] shrunk to N={ocfg['net']['N']} (in-degree 100, same distributions), 300 time "
+                         f"steps after {args.ref_warm_steps} warm-up steps, single thread, {dt_o:.1f} s (+ network generation)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": dict(_config_dict(args, N, n_sim), replicas=world,
+                           exec_mode={1: "kernels+graph", 2: "persistent"}.get(exec_used, str(exec_used))),
+            "neuron_updates_per_s": world * N * args.steps * n_sim / secs,
+            "rtf": secs / bio_s, "mean_rate_hz": rate_hz, "us_per_sim_step": 1e6 * secs / (args.steps * n_sim),
+            "paper_context": "paper RTF 65 / 78.8 / 118.8 at 7 / 15 / 30 Hz for 86e9 neurons on 14,012 GPUs (dt 1 ms): "
+                             "another machine and workload, not a target",
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches_all),
+            "clocks": clk,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--rate", type=int, default=7, choices=[7, 15, 30])
+    ap.add_argument("--sim-steps", type=int, default=1000, help="simulation time steps per bench step")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink configs[1] (debugging only)")
+    ap.add_argument("--exec-mode", choices=["auto", "kernels", "persistent"], default="auto")
+    ap.add_argument("--profile-steps", type=int, default=512)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-scale", type=float, default=0.25, help="oracle sample: fraction of configs[1]'s neurons")
+    ap.add_argument("--ref-warm-steps", type=int, default=1000, help="oracle: untimed steps past the start-up transient")
+    ap.add_argument("--ref-sim-steps", type=int, default=50, help="oracle arm: time steps per bench step")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print(f"bench.py: warmup {args.warmup} < 3 is below the timing rules", file=sys.stderr)
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

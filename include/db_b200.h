@@ -145,6 +145,7 @@ typedef struct db_counters {
     uint64_t bg_events;    /* background Poisson events drawn */
     uint32_t ring_overflow;/* sticky: some consumed ring cell exceeded 2^30 in magnitude (R28) */
     uint32_t exec_mode;    /* DB_EXEC_* actually in use */
+    uint64_t launches;     /* kernels launched by db_step / db_step_profiled on this handle */
 } db_counters;
 
 /* Per-phase device time of the last db_step_profiled() call, in milliseconds. */

@@ -179,6 +179,8 @@ def generate(net: dict, seed: int) -> dict:
     L = lib()
     sp = _net_spec(net)
     h = L.orc_generate(C.byref(sp), int(seed))
+    if not h:
+        raise ValueError("oracle.generate: a region is too small for the requested in-degree (sampling without replacement)")
     n = h.contents
     N, E, R = n.N, n.E, n.n_regions
     out = dict(

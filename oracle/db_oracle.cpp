@@ -467,10 +467,25 @@ int64_t orc_gen_owner_edges(const orc_gen* g, int64_t i, int64_t cap, int32_t* s
     return (int64_t)e.size();
 }
 
+// 1 if the spec can be generated: every region must hold the K_intra distinct
+// non-self sources and the K_inter distinct excitatory sources a target draws
+// from it ("without replacement"); otherwise prp() has no answer.
+int32_t orc_gen_valid(const orc_gen* g) {
+    const orc_net_spec& sp = g->sp;
+    if (sp.N < 2 || sp.n_regions < 1) return 0;
+    for (int r = 0; r < sp.n_regions; ++r) {
+        int64_t size = g->region_start[(size_t)r + 1] - g->region_start[(size_t)r];
+        if (sp.mode == 0 && size - 1 < g->K_intra) return 0;
+        if (sp.mode == 0 && g->K_inter > 0 && g->region_nexc[(size_t)r] < g->K_inter) return 0;
+    }
+    return 1;
+}
+
 orc_network* orc_generate(const orc_net_spec* sp, uint64_t seed) {
     const int64_t N = sp->N;
     const int R = sp->n_regions;
     orc_gen* g = orc_gen_create(sp, seed);
+    if (!orc_gen_valid(g)) { orc_gen_destroy(g); return nullptr; }
     orc_network* net = (orc_network*)std::calloc(1, sizeof(orc_network));
     net->N = N; net->n_regions = R;
     net->region_start = (int64_t*)std::calloc((size_t)R + 1, sizeof(int64_t));

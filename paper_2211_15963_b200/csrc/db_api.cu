@@ -38,6 +38,7 @@ struct db_sim {
     int deliver_grid = 0, persistent_grid = 0;
     cudaGraphExec_t graph_exec = nullptr;
     int graph_steps = 0;
+    uint64_t launches = 0;
     std::vector<cudaEvent_t> prof_events;
     std::string err;
 };
@@ -377,6 +378,7 @@ int32_t db_step(db_sim* sim, uint32_t n_steps) {
     CK(cudaSetDevice(sim->device));
     if (sim->exec_mode == DB_EXEC_PERSISTENT) {
         CK(launch_persistent(sim->dev, n_steps, sim->persistent_grid, sim->stream));
+        sim->launches += 1;
         return DB_OK;
     }
     if (!sim->graph_exec && n_steps >= 32) { int32_t rc = build_graph(sim); if (rc) return rc; }
@@ -384,10 +386,12 @@ int32_t db_step(db_sim* sim, uint32_t n_steps) {
     while (sim->graph_exec && left >= (uint32_t)sim->graph_steps) {
         CK(cudaGraphLaunch(sim->graph_exec, sim->stream));
         left -= (uint32_t)sim->graph_steps;
+        sim->launches += 2ull * (uint64_t)sim->graph_steps;
     }
     for (; left; --left) {
         CK(launch_update(sim->dev, sim->stream));
         CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
+        sim->launches += 2;
     }
     return DB_OK;
 }
@@ -412,6 +416,7 @@ int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
             CK(cudaEventRecord(sim->prof_events[2 * s + 1], sim->stream));
             CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
             CK(cudaEventRecord(sim->prof_events[2 * s + 2], sim->stream));
+            sim->launches += 2;
         }
         CK(cudaStreamSynchronize(sim->stream));
         for (uint32_t s = 0; s < b; ++s) {
@@ -447,6 +452,7 @@ int32_t db_get_counters(db_sim* sim, db_counters* out) {
     for (auto v : parts) bg += v;
     out->steps = c.step; out->spikes = c.spike_begin; out->events = c.events; out->bg_events = bg;
     out->ring_overflow = c.overflow; out->exec_mode = (uint32_t)sim->exec_mode;
+    out->launches = sim->launches;
     return DB_OK;
 }
 

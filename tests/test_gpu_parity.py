@@ -218,7 +218,8 @@ def test_generator_matches_oracle_generator(db, oracle_mod, which):
     if which == "config0":
         cfg = db_inputs.config(0)
     elif which == "regions":
-        cfg = db_inputs.config(2, scale=0.01)             # 50,000 neurons, 200 regions
+        cfg = db_inputs.config(2, scale=0.01)             # 50,000 neurons, K = 160 + 40
+        cfg["net"].update(n_regions=20)                   # (200 regions of >= 161 neurons need N >= 3e5)
     elif which == "regions_fp16":
         cfg = db_inputs.config(3, scale=0.001)
         cfg["net"].update(N=20_000, n_regions=12, K=300)

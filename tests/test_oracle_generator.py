@@ -224,3 +224,10 @@ def test_owner_edges_match_full_generation(oracle_mod, net_regions):
         assert np.array_equal(net["w"][m], e["w"][order])
         assert np.array_equal(net["delay"][m], e["delay"][order])
         assert np.array_equal(net["rec"][m], e["rec"][order])
+
+
+def test_impossible_spec_is_rejected(oracle_mod):
+    # 200 regions of ~250 neurons cannot supply 160 distinct intra-region sources each
+    spec = dict(db_inputs.config(2)["net"], N=50_000)
+    with pytest.raises(ValueError):
+        oracle_mod.generate(spec, db_inputs.GEN_SEED)
