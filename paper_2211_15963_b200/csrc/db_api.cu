@@ -35,7 +35,8 @@ struct db_sim {
     std::vector<int64_t> region_start;
     uint8_t* ntype_dev = nullptr;
     int exec_mode = DB_EXEC_KERNELS;
-    int deliver_grid = 0, persistent_grid = 0;
+    int deliver_grid = 0;
+    bool heavy = false;             // some row is longer than kInlineMax
     cudaGraphExec_t graph_exec = nullptr;
     int graph_steps = 0;
     uint64_t launches = 0;
@@ -205,19 +206,24 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
 }
 
 // After the CSR is on the device: work list, execution mode, initial state.
-int32_t finish_setup(db_sim* sim, uint64_t work_cap) {
+int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     SimDev& d = sim->dev;
     int32_t rc;
     sim->work_cap = std::max<uint64_t>(work_cap, 1);
     if ((rc = alloc_zero(sim, &d.work, (size_t)sim->work_cap))) return rc;
+    sim->heavy = heavy_chunks > 0;
+    if (heavy_chunks > 0xFFFFFFFFull) return fail(sim, DB_EINVAL, "too many heavy-row chunks");
+    d.hq_cap = (uint32_t)std::max<uint64_t>(heavy_chunks, 1);
+    if ((rc = alloc_zero(sim, &d.hq, 2 * (size_t)d.hq_cap))) return rc;
     CK(launch_init_state(d, sim->ntype_dev, sim->stream));
     sim->deliver_grid = sim->n_sm * 4;
-    CK(persistent_max_grid(d, sim->n_sm, &sim->persistent_grid));
     int coop = 0;
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device));
+    bool fits = false;
+    CK(persistent_fits(d, sim->heavy, sim->n_sm, &fits));
     int mode = sim->params.exec_mode;
-    if (mode == DB_EXEC_AUTO) mode = DB_EXEC_KERNELS;
-    if (mode == DB_EXEC_PERSISTENT && (!coop || sim->persistent_grid < 1))
+    if (mode == DB_EXEC_AUTO) mode = (coop && fits) ? DB_EXEC_PERSISTENT : DB_EXEC_KERNELS;
+    if (mode == DB_EXEC_PERSISTENT && (!coop || !fits))
         return fail(sim, DB_ECUDA, "cooperative launch not available for the persistent mode");
     sim->exec_mode = mode;
     CK(cudaStreamSynchronize(sim->stream));
@@ -277,7 +283,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     std::vector<int64_t> row_begin((size_t)N);
     std::vector<int32_t> row_len((size_t)N);
     int64_t pos = 0;
-    uint64_t work_cap = 0;
+    uint64_t work_cap = 0, heavy_chunks = 0;
     for (int64_t j = 0; j < N; ++j) {
         const int64_t len = csr->row_ptr[j + 1] - csr->row_ptr[j];
         if (len < 0 || len > 0x7FFFFFFF) return bail(fail(sim, DB_EINVAL, "row_ptr must be non-decreasing"));
@@ -285,6 +291,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
         row_begin[(size_t)j] = pos; row_len[(size_t)j] = (int32_t)len;
         pos += (len + kRowAlign - 1) / kRowAlign * kRowAlign;
         work_cap += (uint64_t)((len + kChunk - 1) / kChunk);
+        if (len > kInlineMax) heavy_chunks += (uint64_t)((len + kChunk - 1) / kChunk);
     }
     const int64_t Epad = pos + kRowAlign;
     sim->E = E; sim->Epad = Epad;
@@ -323,7 +330,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
         return bail(fail(sim, DB_ECUDA, std::string("CSR upload: ") + cudaGetErrorString(cudaGetLastError())));
     d.row_begin = rb_dev; d.row_len = rl_dev; d.tgt_rec = tr_dev; d.delay = dl_dev; d.w = w_dev;
     d.w_fp16 = csr->weight_fp16 ? 1 : 0;
-    if ((rc = finish_setup(sim, work_cap))) return bail(rc);
+    if ((rc = finish_setup(sim, work_cap, heavy_chunks))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -356,7 +363,7 @@ int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
     d.w_fp16 = spec->weight_fp16 ? 1 : 0;
     sim->E = gr.E; sim->Epad = gr.Epad;
     if (gr.max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
-    if ((rc = finish_setup(sim, gr.work_cap))) return bail(rc);
+    if ((rc = finish_setup(sim, gr.work_cap, gr.heavy_chunks))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -377,8 +384,14 @@ int32_t db_step(db_sim* sim, uint32_t n_steps) {
     if (n_steps == 0) return DB_OK;
     CK(cudaSetDevice(sim->device));
     if (sim->exec_mode == DB_EXEC_PERSISTENT) {
-        CK(launch_persistent(sim->dev, n_steps, sim->persistent_grid, sim->stream));
-        sim->launches += 1;
+        // per launch: spikes (<= N per step) must fit the 32-bit half of the barrier word
+        const uint32_t cap = (uint32_t)std::min<uint64_t>(1u << 20, std::max<uint64_t>(1, 0xFFFFFFFFull / (uint64_t)sim->dev.N));
+        for (uint32_t left = n_steps; left;) {
+            const uint32_t b = std::min(left, cap);
+            CK(launch_persistent(sim->dev, sim->heavy, b, sim->n_sm, sim->stream));
+            sim->launches += 1;
+            left -= b;
+        }
         return DB_OK;
     }
     if (!sim->graph_exec && n_steps >= 32) { int32_t rc = build_graph(sim); if (rc) return rc; }

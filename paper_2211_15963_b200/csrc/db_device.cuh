@@ -11,6 +11,8 @@ constexpr int kPoissonMax = 32;
 constexpr int kNeuronPad = 1024;     // Npad is a multiple of this: whole warps, 128-bit accesses
 constexpr int kRowAlign = 4;         // CSR rows start on a multiple of 4 synapses (128-bit target loads)
 constexpr int kChunk = 512;          // synapses per delivery work item (one warp)
+constexpr int kInlineMax = 1024;     // persistent kernel: rows up to this length are delivered by the warp that found the spike
+constexpr int kRunThreads = 896;     // persistent kernel: most threads per block (one block per SM)
 constexpr int kRefMask = 0x0FFF;     // rt = type << 12 | refractory steps left
 
 // Philox streams
@@ -33,9 +35,12 @@ struct Ctl {                         // device-resident control block
     unsigned long long events;       // synaptic events delivered so far
     unsigned int overflow;           // sticky ring overflow flag
     unsigned int done_blocks;        // delivery kernel: finished-block ticket
-    unsigned int bar_count;          // persistent kernel: grid barrier arrivals
-    unsigned int pad;
-    unsigned long long t_update, t_deliver;   // persistent kernel: accumulated phase time (ns, block 0)
+    unsigned int hq_tail[2];         // persistent kernel: heavy-row chunks queued in step n, cell [n & 1]
+    // persistent kernel: grid barriers, one word per step parity.  Low 32 bits = arrivals since the
+    // launch, high 32 bits (bar1 only) = spikes of the arrived blocks since the launch.
+    unsigned long long bar1[2];      // end of update + inline delivery
+    unsigned long long bar2[2];      // end of the heavy-row phase (networks with heavy rows only)
+    unsigned long long spike_cursor; // persistent kernel: next free raster position (= spike_begin between steps)
 };
 
 constexpr int kBgParts = 1024;       // background-event counter is spread over this many cells
@@ -62,6 +67,8 @@ struct SimDev {                      // passed by value to every kernel
     int32_t* spike_ids;              // [spike_cap] circular
     unsigned long long spike_mask;
     int2* work;                      // [work_cap] (neuron, chunk) of this step
+    int2* hq;                        // [2][hq_cap] persistent kernel: heavy-row chunks queued in step n, half [n & 1]
+    uint32_t hq_cap;
     unsigned long long* step_end;    // [step_log_cap] circular: spikes emitted up to and including step n
     uint32_t step_log_mask;
     // regions

@@ -354,15 +354,16 @@ cudaError_t generate_network(const db_network_spec& sp, uint64_t seed, const Gen
     GCK(cudaStreamSynchronize(st));
     std::vector<int64_t> begin_h((size_t)N);
     int64_t pos = 0, E = 0;
-    uint64_t work_cap = 0;
+    uint64_t work_cap = 0, heavy_chunks = 0;
     for (int64_t j = 0; j < N; ++j) {
         const int64_t len = len_h[(size_t)j];
         begin_h[(size_t)j] = pos;
         pos += (len + kRowAlign - 1) / kRowAlign * kRowAlign;
         E += len;
         work_cap += (uint64_t)((len + kChunk - 1) / kChunk);
+        if (len > kInlineMax) heavy_chunks += (uint64_t)((len + kChunk - 1) / kChunk);
     }
-    out->E = E; out->Epad = pos + kRowAlign; out->work_cap = work_cap;
+    out->E = E; out->Epad = pos + kRowAlign; out->work_cap = work_cap; out->heavy_chunks = heavy_chunks;
     GCK(cudaMemcpyAsync(row_begin, begin_h.data(), (size_t)N * 8, cudaMemcpyHostToDevice, st));
 
     uint32_t* tgt_rec = (uint32_t*)A((size_t)out->Epad * 4); if (!tgt_rec) return cudaSuccess;

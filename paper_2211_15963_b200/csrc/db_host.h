@@ -13,8 +13,8 @@ namespace dbk {
 cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
 cudaError_t launch_update(const SimDev& p, cudaStream_t st);
 cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);
-cudaError_t persistent_max_grid(const SimDev& p, int n_sm, int* grid);
-cudaError_t launch_persistent(const SimDev& p, unsigned n_steps, int grid, cudaStream_t st);
+cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
+cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 
 // ---- db_gen.cu -------------------------------------------------------------
 struct GenHostTables {                 // distribution tables formed on the host in double
@@ -35,6 +35,7 @@ struct GenResult {
     uint32_t* tgt_rec = nullptr; void* w = nullptr; uint8_t* delay = nullptr;
     int64_t E = 0, Epad = 0;
     uint64_t work_cap = 0;
+    uint64_t heavy_chunks = 0;      // chunks of the rows longer than kInlineMax
     int32_t max_delay = 0;
     bool oom = false;
 };

@@ -262,6 +262,7 @@ __device__ __forceinline__ void finalize_step(const SimDev& p, const unsigned lo
     Ctl* c = p.ctl;
     const unsigned long long end = c->spike_begin + (counts >> 32);
     c->spike_begin = end;
+    c->spike_cursor = end;
     p.step_end[n & p.step_log_mask] = end;
     c->step_counts[n & 1ull] = 0ull;
     if ((n + 1) % (unsigned long long)p.window_steps == 0) {
@@ -303,44 +304,437 @@ __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev 
 }
 
 // ===========================================================================
-// Mode DB_EXEC_PERSISTENT: one cooperative kernel runs all the steps; two grid
-// barriers per step replace two kernel launches.
+// Mode DB_EXEC_PERSISTENT: one cooperative kernel runs all the steps, one block
+// per SM.  Every block owns a fixed, contiguous range of 128-neuron tasks, so a
+// thread meets the same neurons in every step.  All global->SM traffic of the
+// update is staged through shared memory with cp.async (16 bytes per thread and
+// plane: ring x4, V, g x4, rt), which keeps the loaded data out of the register
+// file and lets the copies of the next task run while this one is computed:
+//   - while plane u of task k is consumed, plane u of task k + 1 is requested
+//     into the same shared-memory cells;
+//   - at the end of a step the state planes (V, g, rt -- the thread's own data)
+//     of the first task of the next step are requested BEFORE the grid barrier,
+//     the ring planes right after it.
+// Per step: wait for the barrier that closes the previous step (all deliveries
+// into this step's ring slot have landed), then per task consume the slot,
+// update, compact, and push the rows of the spikes this warp found (rows longer
+// than kInlineMax are queued and shared by the whole grid after a second
+// barrier), then arrive.  Delays are >= 1, so step n's deliveries never touch
+// slot n: one barrier per step suffices.  The barrier words alternate with the
+// step parity, so a word is frozen from the moment its target is reached until
+// every block has seen it; the high half of bar1 carries the spike count for
+// the raster log.
 // ===========================================================================
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
+struct alignas(16) TypeSmem {        // TypeConst regrouped into 128-bit words for broadcast LDS.128
+    float4 rec[4];                   // per receptor u: G_u, E_u, alpha_u, -
+    float4 m0;                       // neg_gL, VL, kappa, Iext
+    float4 m1;                       // Vth, Vreset, R (int bits), wq_bg (int bits)
+    uint4 m2;                        // M, T[0], -, -
+};
+
+constexpr int kStageBytesPerThread = 9 * 16 + 8;   // ring x4, V, g x4 (16 B each), rt (8 B)
+
+__device__ __forceinline__ unsigned ld_cg_u32(const unsigned* p) {
+    unsigned r;
+    asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long r;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_cg_f4(float* p, float4 v) {
+    asm volatile("st.global.cg.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void st_cg_i4(int32_t* p, int4 v) {
+    asm volatile("st.global.cg.v4.s32 [%0], {%1,%2,%3,%4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void cp_async16(const uint32_t smem, const void* g) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(smem), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async8(const uint32_t smem, const void* g) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(smem), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ uint4 lds128(const uint32_t smem) {
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(smem) : "memory");
+    return r;
+}
+__device__ __forceinline__ uint2 lds64(const uint32_t smem) {
+    uint2 r;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(smem) : "memory");
+    return r;
 }
 
+// Spin until the low half of *word reaches `target`; returns the word.
+__device__ __forceinline__ unsigned long long bar_wait(const unsigned long long* word, const unsigned target) {
+    unsigned long long v = ld_acquire_u64(word);
+    while ((unsigned)v < target) { __nanosleep(20); v = ld_acquire_u64(word); }
+    return v;
+}
+
+// Push one row (or one chunk of a row): 4 synapses per lane and 128-bit load,
+// two batches of loads in flight before the first reduction is issued.
 template <bool kHalf>
-__global__ void __launch_bounds__(256) k_persistent(const __grid_constant__ SimDev p, const unsigned n_steps) {
-    cg::grid_group grid = cg::this_grid();
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
-    const unsigned n_thr = gridDim.x * blockDim.x;
-    const unsigned n_grp = (unsigned)(p.Npad / 4);
-    unsigned long long n = p.ctl->step;
-    unsigned long long sb = p.ctl->spike_begin;
-    const bool timer = (tid == 0);
-    unsigned long long t0 = timer ? globaltimer_ns() : 0ull, t_upd = 0, t_del = 0;
-    unsigned long long prev_counts = 0ull;
-    for (unsigned s = 0; s < n_steps; ++s, ++n) {
-        if (tid == 0 && s > 0) finalize_step(p, n - 1, prev_counts);   // overlaps this step's update
-        for (unsigned grp = tid; grp < n_grp; grp += n_thr) update_group(p, n, sb, (int)grp);
-        grid.sync();
-        if (timer) { const unsigned long long t1 = globaltimer_ns(); t_upd += t1 - t0; t0 = t1; }
-        const unsigned long long counts = *(volatile unsigned long long*)&p.ctl->step_counts[n & 1ull];
-        const unsigned n_work = (unsigned)counts;
-        for (unsigned q = tid >> 5; q < n_work; q += n_thr >> 5) deliver_item<kHalf>(p, n, p.work[q], lane);
-        sb += counts >> 32;
-        prev_counts = counts;
-        grid.sync();
-        if (timer) { const unsigned long long t1 = globaltimer_ns(); t_del += t1 - t0; t0 = t1; }
+__device__ __forceinline__ void deliver_span(const SimDev& p, const unsigned nlo, const int64_t rb, const int len,
+                                             const unsigned lane) {
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    for (int base = 0; base < len; base += 256) {
+        uint4 tr[2];
+        float4 wv[2];
+        uchar4 dl[2];
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = base + it * 128 + (int)lane * 4;
+            if (e < len) {
+                tr[it] = __ldg(reinterpret_cast<const uint4*>(p.tgt_rec + rb + e));
+                dl[it] = __ldg(reinterpret_cast<const uchar4*>(p.delay + rb + e));
+                if (kHalf) {
+                    const uint2 h = __ldg(reinterpret_cast<const uint2*>(static_cast<const __half*>(p.w) + rb + e));
+                    const __half2 h0 = *reinterpret_cast<const __half2*>(&h.x);
+                    const __half2 h1 = *reinterpret_cast<const __half2*>(&h.y);
+                    wv[it] = make_float4(__low2float(h0), __high2float(h0), __low2float(h1), __high2float(h1));
+                } else {
+                    wv[it] = __ldg(reinterpret_cast<const float4*>(static_cast<const float*>(p.w) + rb + e));
+                }
+            }
+        }
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = base + it * 128 + (int)lane * 4;
+            if (e < len) {
+                const unsigned t4[4] = {tr[it].x, tr[it].y, tr[it].z, tr[it].w};
+                const float w4[4] = {wv[it].x, wv[it].y, wv[it].z, wv[it].w};
+                const unsigned d4[4] = {dl[it].x, dl[it].y, dl[it].z, dl[it].w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (e + k < len) {
+                        const int wq = __float2int_rn(__fmul_rn(w4[k], p.wscale));
+                        const unsigned sl = (nlo + d4[k]) & Dm;
+                        const unsigned rec = t4[k] >> 30, tg = t4[k] & 0x3FFFFFFFu;
+                        red_add_s32(p.ring + ((size_t)sl * 4 + rec) * Np + tg, wq);
+                    }
+            }
+        }
     }
-    if (tid == 0) {
-        if (n_steps) finalize_step(p, n - 1, prev_counts);
-        p.ctl->t_update += t_upd; p.ctl->t_deliver += t_del;
+}
+
+struct RunCfg { unsigned n_steps; int n_tasks; int tasks_per_block; int iters; };
+
+// Shared-memory staging cells of one thread: plane k at sbase + k * pstride (k = 0..3 ring,
+// 4 V, 5..8 g), rt at srt.
+struct Stage { uint32_t sbase, pstride, srt; };
+
+__device__ __forceinline__ void request_state(const SimDev& p, const Stage& sg, const int i0) {
+    const size_t Np = (size_t)p.Npad;
+    cp_async16(sg.sbase + 4u * sg.pstride, p.V + i0);
+    cp_async8(sg.srt, p.rt + i0);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)(5 + u) * sg.pstride, p.g + u * Np + i0);
+}
+__device__ __forceinline__ void request_ring(const SimDev& p, const Stage& sg, const int32_t* slot_i0) {
+    const size_t Np = (size_t)p.Npad;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)u * sg.pstride, slot_i0 + u * Np);
+}
+
+// a1 for the four neurons of one thread, receptor by receptor, out of the staging cells.  While
+// plane u is consumed the same plane of the next task (i0 + next_off, if next_off != 0) is
+// requested.  tp0..tp3 are the neuron types; the caller passes the same variable four times when
+// they agree, which lets the constant loads (broadcast LDS.128) be shared.  Operation order:
+// DESIGN.md "Arithmetic contract".
+__device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem* s_tc,
+                                                 const uint32_t (*s_T)[kPoissonMax], const Stage& sg,
+                                                 const int tp0, const int tp1, const int tp2, const int tp3,
+                                                 const int i0, int32_t* slot, const int next_off,
+                                                 const uint4 v_bits, const uint2 rt_bits, const uint4 rnd,
+                                                 unsigned& bg_acc) {
+    const size_t Np = (size_t)p.Npad;
+    const int tp[4] = {tp0, tp1, tp2, tp3};
+    const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
+    const float v[4] = {__uint_as_float(v_bits.x), __uint_as_float(v_bits.y), __uint_as_float(v_bits.z),
+                        __uint_as_float(v_bits.w)};
+    float I[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const uint4 ab = lds128(sg.sbase + (unsigned)u * sg.pstride);
+        const uint4 gb = lds128(sg.sbase + (unsigned)(5 + u) * sg.pstride);
+        if (next_off) {
+            cp_async16(sg.sbase + (unsigned)u * sg.pstride, slot + u * Np + next_off);
+            cp_async16(sg.sbase + (unsigned)(5 + u) * sg.pstride, p.g + u * Np + i0 + next_off);
+        }
+        int a[4] = {(int)ab.x, (int)ab.y, (int)ab.z, (int)ab.w};
+        const bool nz = (a[0] | a[1] | a[2] | a[3]) != 0;
+        if (nz) {                       // consumed: zero the cells again, check the overflow bound
+            st_cg_i4(slot + u * Np, make_int4(0, 0, 0, 0));
+            const int lim = 1 << 30;
+            if (a[0] > lim || a[0] < -lim || a[1] > lim || a[1] < -lim ||
+                a[2] > lim || a[2] < -lim || a[3] > lim || a[3] < -lim) p.ctl->overflow = 1u;
+        }
+        const float gu[4] = {__uint_as_float(gb.x), __uint_as_float(gb.y), __uint_as_float(gb.z), __uint_as_float(gb.w)};
+        float gn[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float4 r = s_tc[tp[q]].rec[u];
+            float x;
+            if (u == 0) {               // Poisson background joins the AMPA arrivals (R14)
+                const uint4 m2 = s_tc[tp[q]].m2;
+                if ((i0 + q) < p.N && m2.x > 0u && rw[q] >= m2.y) {      // thresholds increase: count all u >= T_m
+                    int k = 1;
+                    while (k < (int)m2.x && rw[q] >= s_T[tp[q]][k]) ++k;
+                    bg_acc += (unsigned)k;
+                    a[q] = (int)((unsigned)a[q] + (unsigned)k * (unsigned)__float_as_int(s_tc[tp[q]].m1.w));
+                }
+                x = __fmul_rn(__int2float_rn(a[q]), p.scale);
+            } else {
+                x = nz ? __fmul_rn(__int2float_rn(a[q]), p.scale) : 0.0f;
+            }
+            const float t = __fmul_rn(__fmul_rn(r.x, gu[q]), __fsub_rn(r.y, v[q]));
+            I[q] = (u == 0) ? t : __fadd_rn(I[q], t);
+            gn[q] = __fadd_rn(__fmul_rn(gu[q], r.z), x);
+        }
+        st_cg_f4(p.g + u * Np + i0, make_float4(gn[0], gn[1], gn[2], gn[3]));
     }
+    unsigned rt[4] = {rt_bits.x & 0xFFFFu, rt_bits.x >> 16, rt_bits.y & 0xFFFFu, rt_bits.y >> 16};
+    float vn[4];
+    unsigned spike_bits = 0, rt_changed = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 m0 = s_tc[tp[q]].m0, m1 = s_tc[tp[q]].m1;
+        const float Iq = __fadd_rn(I[q], m0.w);
+        const float leak = __fmul_rn(m0.x, __fsub_rn(v[q], m0.y));
+        float w = __fadd_rn(v[q], __fmul_rn(m0.z, __fadd_rn(leak, Iq)));
+        if ((rt[q] & (unsigned)kRefMask) > 0u) { w = m1.y; rt[q] -= 1u; rt_changed = 1u; }
+        else if (w >= m1.x) {
+            const unsigned R = (unsigned)__float_as_int(m1.z);
+            w = m1.y; rt[q] |= R; rt_changed |= (unsigned)(R != 0u);
+            if ((i0 + q) < p.N) spike_bits |= 1u << q;
+        }
+        vn[q] = w;
+    }
+    st_cg_f4(p.V + i0, make_float4(vn[0], vn[1], vn[2], vn[3]));
+    if (rt_changed) *reinterpret_cast<uint2*>(p.rt + i0) = make_uint2(rt[0] | (rt[1] << 16), rt[2] | (rt[3] << 16));
+    return spike_bits;
+}
+
+// a1 + a2 + a3 + a4 for one 128-neuron task of one warp.  next_off != 0: distance (in neurons) to
+// the warp's next task of this step, whose planes are requested while this one is consumed.
+template <bool kHalf, bool kHeavy>
+__device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, const uint32_t (*s_T)[kPoissonMax],
+                                         const Stage& sg, const unsigned long long n, const int task,
+                                         const unsigned lane, const int next_off, unsigned* s_blk_spk,
+                                         unsigned& bg_acc) {
+    const int grp = task * 32 + (int)lane;
+    const int i0 = grp * 4;
+    const size_t Np = (size_t)p.Npad;
+    int32_t* slot = p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
+    // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
+    const uint4 rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)),
+                                    p.seed_lo, p.seed_hi);
+    cp_async_wait_all();
+    const uint4 v_bits = lds128(sg.sbase + 4u * sg.pstride);
+    const uint2 rt_bits = lds64(sg.srt);
+    if (next_off) {
+        cp_async16(sg.sbase + 4u * sg.pstride, p.V + i0 + next_off);
+        cp_async8(sg.srt, p.rt + i0 + next_off);
+    }
+    const int tp0 = (int)((rt_bits.x >> 12) & 0xFu), tp1 = (int)(rt_bits.x >> 28);
+    const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
+    unsigned spike_bits;
+    if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
+        spike_bits = neuron_group(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+    else                                // a type boundary inside the group (rare)
+        spike_bits = neuron_group(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+    cp_async_commit();
+
+    // ---- a2 + a4 + a3: spikes are rare (rate * dt per neuron-step); whole warps skip this
+    unsigned any = __ballot_sync(0xffffffffu, spike_bits != 0);
+    if (any == 0) return;
+    int len[4] = {0, 0, 0, 0};
+    int64_t rb[4] = {0, 0, 0, 0};
+    unsigned my_events = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (spike_bits & (1u << q)) {
+            len[q] = __ldg(p.row_len + i0 + q);
+            rb[q] = __ldg(p.row_begin + i0 + q);
+            my_events += (unsigned)len[q];
+        }
+    const unsigned my_spk = (unsigned)__popc(spike_bits);
+    unsigned inc = my_spk;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= (unsigned)d) inc += o;
+    }
+    const unsigned tot = __shfl_sync(0xffffffffu, inc, 31);
+    const unsigned ev_warp = __reduce_add_sync(0xffffffffu, my_events);
+    unsigned long long base = 0;
+    if (lane == 0) {
+        base = atomicAdd(&p.ctl->spike_cursor, (unsigned long long)tot);
+        atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
+        atomicAdd(s_blk_spk, tot);
+    }
+    base = __shfl_sync(0xffffffffu, base, 0);
+    unsigned long long pos = base + (inc - my_spk);
+    const unsigned win = (unsigned)((n / (unsigned long long)p.window_steps) % p.max_windows);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (spike_bits & (1u << q)) {
+            const int i = i0 + q;
+            p.spike_ids[pos & p.spike_mask] = i;
+            ++pos;
+            const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
+            atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
+        }
+    // a3: the warp pushes the rows of its own spikes, one row at a time
+    const unsigned nlo = (unsigned)n;
+    while (any) {
+        const int src = __ffs(any) - 1;
+        any &= any - 1u;
+        const unsigned bits = __shfl_sync(0xffffffffu, spike_bits, src);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int l = __shfl_sync(0xffffffffu, len[q], src);
+            const long long b = __shfl_sync(0xffffffffu, (long long)rb[q], src);
+            if (!(bits & (1u << q))) continue;
+            if (kHeavy && l > kInlineMax) {                      // queue the chunks for the whole grid
+                const int nch = (l + kChunk - 1) / kChunk;
+                unsigned at = 0;
+                if (lane == 0) at = atomicAdd(&p.ctl->hq_tail[n & 1ull], (unsigned)nch);
+                at = __shfl_sync(0xffffffffu, at, 0);
+                int2* q_out = p.hq + (size_t)(n & 1ull) * p.hq_cap + at;
+                const int j = (task * 32 + src) * 4 + q;
+                for (int ch = (int)lane; ch < nch; ch += 32) q_out[ch] = make_int2(j, ch);
+            } else {
+                deliver_span<kHalf>(p, nlo, (int64_t)b, l, lane);
+            }
+        }
+    }
+}
+
+template <bool kHalf, bool kHeavy>
+__global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ SimDev p, const RunCfg cfg) {
+    extern __shared__ uint4 s_stage[];                 // blockDim.x * kStageBytesPerThread bytes
+    __shared__ TypeSmem s_tc[kMaxTypes];
+    __shared__ uint32_t s_T[kMaxTypes][kPoissonMax];
+    __shared__ unsigned s_blk_spk, s_hq_n;
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+    for (int t = (int)threadIdx.x; t < kMaxTypes; t += (int)blockDim.x) {
+        const TypeConst& c = p.tc[t];
+        TypeSmem r;
+        for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(c.G[u], c.E[u], c.alpha[u], 0.0f);
+        r.m0 = make_float4(c.neg_gL, c.VL, c.kappa, c.Iext);
+        r.m1 = make_float4(c.Vth, c.Vreset, __int_as_float(c.R), __int_as_float(c.wq_bg));
+        r.m2 = make_uint4((unsigned)c.M, c.M > 0 ? c.T[0] : 0xFFFFFFFFu, 0u, 0u);
+        s_tc[t] = r;
+    }
+    for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
+        s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
+    if (threadIdx.x == 0) { s_blk_spk = 0u; s_hq_n = 0u; }
+    __syncthreads();
+
+    Stage sg;
+    sg.pstride = blockDim.x * 16u;
+    sg.sbase = (uint32_t)__cvta_generic_to_shared(s_stage) + threadIdx.x * 16u;
+    sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * sg.pstride + threadIdx.x * 8u;
+
+    Ctl* const ctl = p.ctl;
+    const unsigned long long n0 = ctl->step;          // nobody writes it before the end of the launch
+    unsigned long long sb = ctl->spike_begin;         // raster bookkeeping: block 0, thread 0
+    unsigned hi_even = 0u, hi_odd = 0u;
+    const bool keeper = (blockIdx.x == 0 && threadIdx.x == 0);
+    const int first = (int)blockIdx.x * cfg.tasks_per_block;
+    const int last = min(first + cfg.tasks_per_block, cfg.n_tasks);
+    const int task0 = first + (int)warp;              // the warp's first task of every step
+    const int i00 = (task0 * 32 + (int)lane) * 4;
+    const int task_stride = (int)n_warps * 128;       // neurons between consecutive tasks of a warp
+    const unsigned G = gridDim.x;
+    const size_t Np = (size_t)p.Npad;
+    unsigned bg_acc = 0u;
+
+    // closes step sp: the keeper logs the raster position and clears the region window two ahead
+    auto close_step = [&](const unsigned sp, const unsigned long long word) {
+        const unsigned hi = (unsigned)(word >> 32);
+        if (sp & 1u) { sb += (unsigned long long)(hi - hi_odd); hi_odd = hi; }
+        else         { sb += (unsigned long long)(hi - hi_even); hi_even = hi; }
+        const unsigned long long np = n0 + sp;
+        p.step_end[np & p.step_log_mask] = sb;
+        if ((np + 1) % (unsigned long long)p.window_steps == 0) {
+            const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + 1) % p.max_windows);
+            for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
+        }
+    };
+
+    if (task0 < last && cfg.n_steps > 0) { request_state(p, sg, i00); cp_async_commit(); }
+    for (unsigned s = 0; s < cfg.n_steps; ++s) {
+        const unsigned long long n = n0 + s;
+        if (s > 0) {                                   // every delivery of step n - 1 must have landed
+            const unsigned sp = s - 1;
+            if (threadIdx.x == 0) {
+                const unsigned target = (sp / 2u + 1u) * G;
+                if (kHeavy) {
+                    bar_wait(&ctl->bar2[sp & 1u], target);
+                    if (keeper) ctl->hq_tail[sp & 1u] = 0u;
+                } else {
+                    const unsigned long long w = bar_wait(&ctl->bar1[sp & 1u], target);
+                    if (keeper) close_step(sp, w);
+                }
+            }
+            __syncthreads();
+        }
+        if (task0 < last) {
+            request_ring(p, sg, p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np + i00);
+            cp_async_commit();
+            for (int task = task0; task < last; task += (int)n_warps) {
+                const int next_off = (task + (int)n_warps < last) ? task_stride : 0;
+                run_task<kHalf, kHeavy>(p, s_tc, s_T, sg, n, task, lane, next_off, &s_blk_spk, bg_acc);
+            }
+            if (s + 1 < cfg.n_steps) { request_state(p, sg, i00); cp_async_commit(); }   // own data: no need to wait for the grid
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned k = s_blk_spk;
+            s_blk_spk = 0u;
+            __threadfence();
+            atomicAdd(&ctl->bar1[s & 1u], ((unsigned long long)k << 32) | 1ull);
+        }
+        if (kHeavy) {                                  // rows too long for one warp: the whole grid shares them
+            if (threadIdx.x == 0) {
+                const unsigned long long w = bar_wait(&ctl->bar1[s & 1u], (s / 2u + 1u) * G);
+                if (keeper) close_step(s, w);
+                s_hq_n = ld_cg_u32(&ctl->hq_tail[n & 1ull]);
+            }
+            __syncthreads();
+            const unsigned cnt = s_hq_n;
+            const int2* qv = p.hq + (size_t)(n & 1ull) * p.hq_cap;
+            for (unsigned q = blockIdx.x * n_warps + warp; q < cnt; q += G * n_warps) {
+                const int2 wk = qv[q];
+                const int64_t rb = __ldg(p.row_begin + wk.x) + (int64_t)wk.y * kChunk;
+                int len = __ldg(p.row_len + wk.x) - wk.y * kChunk;
+                len = len < kChunk ? len : kChunk;
+                deliver_span<kHalf>(p, (unsigned)n, rb, len, lane);
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) { __threadfence(); atomicAdd(&ctl->bar2[s & 1u], 1ull); }
+        }
+    }
+    // close the last step and publish the position
+    if (cfg.n_steps > 0 && keeper) {
+        const unsigned sp = cfg.n_steps - 1;
+        const unsigned target = (sp / 2u + 1u) * G;
+        if (kHeavy) { bar_wait(&ctl->bar2[sp & 1u], target); ctl->hq_tail[sp & 1u] = 0u; }
+        else close_step(sp, bar_wait(&ctl->bar1[sp & 1u], target));
+        ctl->spike_begin = sb;
+        ctl->step = n0 + cfg.n_steps;
+    }
+    const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
+    if (lane == 0 && bg_warp)
+        atomicAdd(p.bg_parts + ((blockIdx.x * n_warps + warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
 }
 
 // ---------------------------------------------------------------------------
@@ -380,19 +774,46 @@ cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-cudaError_t persistent_max_grid(const SimDev& p, int n_sm, int* grid) {
-    int per_sm = 0;
-    cudaError_t e = p.w_fp16
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<true>, 256, 0)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_persistent<false>, 256, 0);
-    *grid = per_sm * n_sm;
+// One block per SM; tasks (128 neurons) are dealt out in contiguous ranges, and the block size is
+// chosen so that the warps of a block take the same number of tasks (no ragged last iteration).
+void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg) {
+    const int n_tasks = p.Npad / 128;
+    const int max_warps = kRunThreads / 32;
+    const int tpb = (n_tasks + n_sm - 1) / n_sm;
+    const int iters = (tpb + max_warps - 1) / max_warps;
+    const int warps = (tpb + iters - 1) / iters;
+    cfg->n_tasks = n_tasks; cfg->tasks_per_block = tpb; cfg->iters = iters;
+    *grid = (n_tasks + tpb - 1) / tpb;
+    *threads = warps * 32;
+}
+
+static const void* run_fn(const SimDev& p, bool heavy) {
+    if (p.w_fp16) return heavy ? (const void*)k_run<true, true> : (const void*)k_run<true, false>;
+    return heavy ? (const void*)k_run<false, true> : (const void*)k_run<false, false>;
+}
+
+cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok) {
+    int grid = 0, threads = 0, per_sm = 0;
+    RunCfg cfg{};
+    run_shape(p, n_sm, &grid, &threads, &cfg);
+    const size_t smem = (size_t)threads * kStageBytesPerThread;
+    cudaError_t e = cudaFuncSetAttribute(run_fn(p, heavy), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, run_fn(p, heavy), threads, smem);
+    *ok = (e == cudaSuccess) && (per_sm * n_sm >= grid);
     return e;
 }
 
-cudaError_t launch_persistent(const SimDev& p, unsigned n_steps, int grid, cudaStream_t st) {
-    void* args[] = {(void*)&p, (void*)&n_steps};
-    const void* fn = p.w_fp16 ? (const void*)k_persistent<true> : (const void*)k_persistent<false>;
-    return cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, 0, st);
+cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st) {
+    int grid = 0, threads = 0;
+    RunCfg cfg{};
+    run_shape(p, n_sm, &grid, &threads, &cfg);
+    cfg.n_steps = n_steps;
+    cudaError_t e = cudaMemsetAsync(p.ctl->bar1, 0, sizeof(p.ctl->bar1) + sizeof(p.ctl->bar2), st);   // bar1, bar2 are adjacent
+    if (e != cudaSuccess) return e;
+    void* args[] = {(void*)&p, (void*)&cfg};
+    return cudaLaunchCooperativeKernel(run_fn(p, heavy), dim3(grid), dim3(threads), args,
+                                       (size_t)threads * kStageBytesPerThread, st);
 }
 
 }  // namespace dbk
