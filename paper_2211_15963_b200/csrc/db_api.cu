@@ -154,20 +154,23 @@ int32_t open_device(db_sim* sim, const db_runtime* rt) {
 
 // Everything except the CSR arrays: state, ring, lists, counters.
 int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_regions,
-                     const int64_t* region_start) {
+                     const int64_t* region_start, int32_t max_delay) {
     SimDev& d = sim->dev;
     sim->params = *sp;
     if (N < 1 || N >= (1ll << 30)) return fail(sim, DB_EINVAL, "N must be within 1..2^30-1");
     if (n_regions < 1 || n_regions > 65536) return fail(sim, DB_EINVAL, "n_regions must be 1..65536");
     d.N = (int32_t)N;
     d.Npad = (int32_t)(((N + kNeuronPad - 1) / kNeuronPad) * kNeuronPad);
-    d.D = sp->D; d.S = sp->S;
+    // internal ring depth: the persistent kernel lets blocks run up to two steps apart and needs
+    // depth >= largest delay + 3 (db_step.cu); the API's D (slot = step mod D) is mapped on read / write
+    d.D = (max_delay + 3 > sp->D) ? 2 * sp->D : sp->D;
+    d.S = sp->S;
     d.scale = (float)std::ldexp(1.0, -sp->S);
     d.wscale = (float)std::ldexp(1.0, sp->S);
     d.seed_lo = (uint32_t)sp->dyn_seed; d.seed_hi = (uint32_t)(sp->dyn_seed >> 32);
     d.window_steps = sp->window_steps;
     d.max_windows = sp->max_windows ? sp->max_windows : 4096u;
-    if (d.max_windows < 4) return fail(sim, DB_EINVAL, "max_windows must be >= 4");
+    if (d.max_windows < 8) return fail(sim, DB_EINVAL, "max_windows must be >= 8");
     d.n_regions = n_regions;
     int32_t rc = make_type_consts(sim, *sp, d.tc);
     if (rc) return rc;
@@ -192,6 +195,7 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     sim->spike_cap = cap;
     d.spike_mask = cap - 1;
     if ((rc = alloc_zero(sim, &d.spike_ids, (size_t)cap))) return rc;
+    if ((rc = alloc_zero(sim, &d.spike_tag, (size_t)cap))) return rc;
     d.step_log_mask = (1u << 16) - 1u;
     if ((rc = alloc_zero(sim, &d.step_end, (size_t)d.step_log_mask + 1))) return rc;
     int32_t* rs_dev = nullptr;
@@ -212,9 +216,6 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     sim->work_cap = std::max<uint64_t>(work_cap, 1);
     if ((rc = alloc_zero(sim, &d.work, (size_t)sim->work_cap))) return rc;
     sim->heavy = heavy_chunks > 0;
-    if (heavy_chunks > 0xFFFFFFFFull) return fail(sim, DB_EINVAL, "too many heavy-row chunks");
-    d.hq_cap = (uint32_t)std::max<uint64_t>(heavy_chunks, 1);
-    if ((rc = alloc_zero(sim, &d.hq, 2 * (size_t)d.hq_cap))) return rc;
     CK(launch_init_state(d, sim->ntype_dev, sim->stream));
     sim->deliver_grid = sim->n_sm * 4;
     int coop = 0;
@@ -276,7 +277,10 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     const int64_t N = csr->N, E = csr->E;
     if (E < 0 || csr->row_ptr[0] != 0 || csr->row_ptr[N] != E) return bail(fail(sim, DB_EINVAL, "row_ptr must run from 0 to E"));
     if (E > 0 && (!csr->tgt || !csr->w || !csr->delay || !csr->rec)) return bail(fail(sim, DB_EINVAL, "csr arrays missing"));
-    if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start))) return bail(rc);
+    int32_t max_delay = 0;
+    for (int64_t e = 0; e < E; ++e) max_delay = std::max<int32_t>(max_delay, csr->delay[e]);
+    if (max_delay >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
+    if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start, max_delay))) return bail(rc);
     SimDev& d = sim->dev;
 
     // padded row layout + validation
@@ -349,7 +353,10 @@ int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
     GenHostTables tabs;
     std::string gerr;
     if (!gen_host_tables(*spec, seed, &tabs, &gerr)) return bail(fail(sim, DB_EINVAL, gerr));
-    if ((rc = setup_common(sim, &spec->sim, spec->N, spec->n_regions, tabs.region_start.data()))) return bail(rc);
+    int32_t max_delay = spec->delay_intra_max;
+    if (tabs.K_inter > 0) max_delay = std::max(max_delay, spec->delay_inter_max);
+    if (max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
+    if ((rc = setup_common(sim, &spec->sim, spec->N, spec->n_regions, tabs.region_start.data(), max_delay))) return bail(rc);
 
     GenAlloc ga;
     ga.user = sim;
@@ -384,8 +391,7 @@ int32_t db_step(db_sim* sim, uint32_t n_steps) {
     if (n_steps == 0) return DB_OK;
     CK(cudaSetDevice(sim->device));
     if (sim->exec_mode == DB_EXEC_PERSISTENT) {
-        // per launch: spikes (<= N per step) must fit the 32-bit half of the barrier word
-        const uint32_t cap = (uint32_t)std::min<uint64_t>(1u << 20, std::max<uint64_t>(1, 0xFFFFFFFFull / (uint64_t)sim->dev.N));
+        const uint32_t cap = 1u << 20;     // keeps the arrival counter of one launch far below 2^32
         for (uint32_t left = n_steps; left;) {
             const uint32_t b = std::min(left, cap);
             CK(launch_persistent(sim->dev, sim->heavy, b, sim->n_sm, sim->stream));
@@ -479,39 +485,51 @@ int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint
     if (step_begin > step_end) return fail(sim, DB_EINVAL, "step_begin > step_end");
     if (step_end > c.step) return fail(sim, DB_ERANGE, "steps not simulated yet");
     if (step_begin == step_end) return DB_OK;
+    // step_end[u] = S(u), the number of spikes of the steps <= u.  The raster is written through one
+    // cursor by blocks that may be one step apart, so the entries of step u lie somewhere in the
+    // positions [S(u-2), S(u+1)) and carry the low 32 bits of their step as a tag.
+    if (step_end - step_begin > 0xFFFFFFFFull) return fail(sim, DB_EINVAL, "step range too long");
     const uint64_t log_cap = (uint64_t)sim->dev.step_log_mask + 1;
-    const uint64_t first_log = step_begin ? step_begin - 1 : 0;      // first log entry needed
+    const uint64_t first_log = step_begin >= 2 ? step_begin - 2 : 0;            // first log entry needed
+    const uint64_t last_log = std::min<uint64_t>(step_end, c.step - 1);          // last one
     if (c.step - first_log > log_cap) return fail(sim, DB_ERANGE, "steps older than the step log");
-    const uint64_t n_log = step_end - first_log;                     // entries first_log .. step_end-1
-    std::vector<unsigned long long> ends((size_t)n_log);
+    const uint64_t n_log = last_log - first_log + 1;
+    std::vector<unsigned long long> S((size_t)n_log);
     for (uint64_t k = 0; k < n_log;) {                               // circular copy
         const uint64_t idx = (first_log + k) & sim->dev.step_log_mask;
         const uint64_t run = std::min<uint64_t>(n_log - k, log_cap - idx);
-        CK(cudaMemcpy(ends.data() + k, sim->dev.step_end + idx, (size_t)run * 8, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(S.data() + k, sim->dev.step_end + idx, (size_t)run * 8, cudaMemcpyDeviceToHost));
         k += run;
     }
-    const uint64_t seg_begin = step_begin ? ends[0] : 0ull;
-    const uint64_t seg_end = ends.back();
-    if (c.spike_begin - seg_begin > sim->spike_cap) return fail(sim, DB_ERANGE, "spikes already overwritten in the raster ring");
-    const uint64_t n = seg_end - seg_begin;
+    auto S_of = [&](uint64_t u) { return (uint64_t)S[(size_t)(u - first_log)]; };
+    const uint64_t scan_begin = step_begin >= 2 ? S_of(step_begin - 2) : 0ull;
+    const uint64_t scan_end = S_of(last_log);
+    const uint64_t n = S_of(step_end - 1) - (step_begin ? S_of(step_begin - 1) : 0ull);
+    if (c.spike_begin - scan_begin > sim->spike_cap) return fail(sim, DB_ERANGE, "spikes already overwritten in the raster ring");
     *n_out = n;
     if (n == 0 || cap == 0) return DB_OK;
-    std::vector<int32_t> tmp((size_t)n);
-    for (uint64_t k = 0; k < n;) {
-        const uint64_t idx = (seg_begin + k) & sim->dev.spike_mask;
-        const uint64_t run = std::min<uint64_t>(n - k, sim->spike_cap - idx);
-        CK(cudaMemcpy(tmp.data() + k, sim->dev.spike_ids + idx, (size_t)run * 4, cudaMemcpyDeviceToHost));
+    const uint64_t m = scan_end - scan_begin;
+    std::vector<int32_t> id_raw((size_t)m);
+    std::vector<uint32_t> tag_raw((size_t)m);
+    for (uint64_t k = 0; k < m;) {
+        const uint64_t idx = (scan_begin + k) & sim->dev.spike_mask;
+        const uint64_t run = std::min<uint64_t>(m - k, sim->spike_cap - idx);
+        CK(cudaMemcpy(id_raw.data() + k, sim->dev.spike_ids + idx, (size_t)run * 4, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(tag_raw.data() + k, sim->dev.spike_tag + idx, (size_t)run * 4, cudaMemcpyDeviceToHost));
         k += run;
     }
-    uint64_t o = 0, prev = seg_begin;
-    for (uint64_t s = step_begin; s < step_end && o < cap; ++s) {
-        const uint64_t e = ends[(size_t)(s - first_log)];
-        std::sort(tmp.begin() + (size_t)(prev - seg_begin), tmp.begin() + (size_t)(e - seg_begin));
-        for (uint64_t k = prev; k < e && o < cap; ++k, ++o) {
-            if (steps) steps[o] = s;
-            if (ids) ids[o] = tmp[(size_t)(k - seg_begin)];
-        }
-        prev = e;
+    std::vector<std::pair<uint64_t, int32_t>> sel;
+    sel.reserve((size_t)n);
+    const uint32_t span = (uint32_t)(step_end - step_begin), lo = (uint32_t)step_begin;
+    for (uint64_t k = 0; k < m; ++k) {
+        const uint32_t rel = tag_raw[(size_t)k] - lo;
+        if (rel < span) sel.emplace_back(step_begin + rel, id_raw[(size_t)k]);
+    }
+    if (sel.size() != n) return fail(sim, DB_ESTATE, "raster log is inconsistent");
+    std::sort(sel.begin(), sel.end());
+    for (uint64_t o = 0; o < n && o < cap; ++o) {
+        if (steps) steps[o] = sel[(size_t)o].first;
+        if (ids) ids[o] = sel[(size_t)o].second;
     }
     return DB_OK;
 }
@@ -538,13 +556,21 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
         break;
     }
     case DB_FIELD_RING: {
+        // API slot j holds the arrivals of the step t in [n, n + D) with t mod D == j; device slot = t mod d.D
+        Ctl c;
+        int32_t rc = read_ctl(sim, &c);
+        if (rc) return rc;
+        const int D = sim->params.D;
         std::vector<int32_t> t((size_t)count);
         int32_t* o = static_cast<int32_t*>(dst);
-        for (int s = 0; s < d.D; ++s)
+        for (int k = 0; k < D; ++k) {
+            const uint64_t step = c.step + (uint64_t)k;
+            const size_t s = (size_t)(step % (uint64_t)D), sd = (size_t)(step & (uint64_t)(d.D - 1));
             for (int u = 0; u < 4; ++u) {
-                CK(cudaMemcpy(t.data(), d.ring + ((size_t)s * 4 + u) * Np + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
-                for (int64_t i = 0; i < count; ++i) o[((size_t)s * (size_t)count + (size_t)i) * 4 + u] = t[(size_t)i];
+                CK(cudaMemcpy(t.data(), d.ring + (sd * 4 + u) * Np + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
+                for (int64_t i = 0; i < count; ++i) o[(s * (size_t)count + (size_t)i) * 4 + u] = t[(size_t)i];
             }
+        }
         break;
     }
     default: return fail(sim, DB_EINVAL, "unknown field");
@@ -576,13 +602,20 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
         break;
     }
     case DB_FIELD_RING: {
+        Ctl c;
+        int32_t rc = read_ctl(sim, &c);
+        if (rc) return rc;
+        const int D = sim->params.D;
         std::vector<int32_t> t((size_t)count);
         const int32_t* in = static_cast<const int32_t*>(src);
-        for (int s = 0; s < d.D; ++s)
+        for (int k = 0; k < D; ++k) {
+            const uint64_t step = c.step + (uint64_t)k;
+            const size_t s = (size_t)(step % (uint64_t)D), sd = (size_t)(step & (uint64_t)(d.D - 1));
             for (int u = 0; u < 4; ++u) {
-                for (int64_t i = 0; i < count; ++i) t[(size_t)i] = in[((size_t)s * (size_t)count + (size_t)i) * 4 + u];
-                CK(cudaMemcpy(d.ring + ((size_t)s * 4 + u) * Np + first, t.data(), (size_t)count * 4, cudaMemcpyHostToDevice));
+                for (int64_t i = 0; i < count; ++i) t[(size_t)i] = in[(s * (size_t)count + (size_t)i) * 4 + u];
+                CK(cudaMemcpy(d.ring + (sd * 4 + u) * Np + first, t.data(), (size_t)count * 4, cudaMemcpyHostToDevice));
             }
+        }
         break;
     }
     default: return fail(sim, DB_EINVAL, "field is not writable");
@@ -597,7 +630,8 @@ static int32_t region_windows(db_sim* sim, std::vector<uint32_t>* counts, uint64
     if (rc) return rc;
     const SimDev& d = sim->dev;
     const uint64_t done = c.step / (uint64_t)d.window_steps;           // completed windows
-    const uint64_t keep = (uint64_t)d.max_windows - 2;                  // the two newest slots may be in flux
+    const uint64_t ahead = 2u / (uint64_t)d.window_steps + 1u;         // windows cleared ahead of time (db_step.cu)
+    const uint64_t keep = (uint64_t)d.max_windows - 1 - ahead;         // the open window and the cleared ones are not history
     const uint64_t first = done > keep ? done - keep : 0;
     uint64_t n = done - first;
     if (first_window) *first_window = first;
@@ -699,6 +733,15 @@ int32_t db_export_csr(db_sim* sim, db_csr_host* out) {
     }
     return DB_OK;
 }
+
+#ifdef DB_TRACE
+// Debugging builds only (not part of the ABI): per-block phase timestamps of the persistent kernel.
+int32_t db_debug_set_trace(db_sim* sim, void* dev_buf) {
+    if (!sim) return DB_EINVAL;
+    sim->dev.trace = static_cast<unsigned long long*>(dev_buf);
+    return DB_OK;
+}
+#endif
 
 int32_t db_free_csr(db_csr_host* c) {
     if (!c) return DB_EINVAL;

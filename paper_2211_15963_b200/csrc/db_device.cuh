@@ -35,11 +35,13 @@ struct Ctl {                         // device-resident control block
     unsigned long long events;       // synaptic events delivered so far
     unsigned int overflow;           // sticky ring overflow flag
     unsigned int done_blocks;        // delivery kernel: finished-block ticket
-    unsigned int hq_tail[2];         // persistent kernel: heavy-row chunks queued in step n, cell [n & 1]
-    // persistent kernel: grid barriers, one word per step parity.  Low 32 bits = arrivals since the
-    // launch, high 32 bits (bar1 only) = spikes of the arrived blocks since the launch.
-    unsigned long long bar1[2];      // end of update + inline delivery
-    unsigned long long bar2[2];      // end of the heavy-row phase (networks with heavy rows only)
+    unsigned int pad0[2];
+    // persistent kernel (see db_step.cu): arrivals of the blocks that finished unit j go to the
+    // monotonic counter [j & 3] (blocks are at most two units apart), the spike count of the step
+    // produced by unit j to unit_spikes[j & 3]
+    unsigned int bar[4];
+    unsigned int unit_spikes[4];
+    unsigned int pad1[2];
     unsigned long long spike_cursor; // persistent kernel: next free raster position (= spike_begin between steps)
 };
 
@@ -65,10 +67,9 @@ struct SimDev {                      // passed by value to every kernel
     int32_t w_fp16;
     // spike list = raster ring; per-step work list
     int32_t* spike_ids;              // [spike_cap] circular
+    uint32_t* spike_tag;             // [spike_cap] low 32 bits of the step of each entry (steps may interleave by one)
     unsigned long long spike_mask;
     int2* work;                      // [work_cap] (neuron, chunk) of this step
-    int2* hq;                        // [2][hq_cap] persistent kernel: heavy-row chunks queued in step n, half [n & 1]
-    uint32_t hq_cap;
     unsigned long long* step_end;    // [step_log_cap] circular: spikes emitted up to and including step n
     uint32_t step_log_mask;
     // regions
@@ -79,6 +80,7 @@ struct SimDev {                      // passed by value to every kernel
     uint32_t max_windows;
     unsigned long long* bg_parts;    // [kBgParts]
     Ctl* ctl;
+    unsigned long long* trace;       // debugging builds (-DDB_TRACE) only: per-block phase timestamps
     TypeConst tc[kMaxTypes];
 };
 

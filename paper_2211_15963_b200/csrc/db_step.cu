@@ -44,6 +44,10 @@ __device__ __forceinline__ void red_add_s32(int32_t* p, int32_t v) {
     asm volatile("red.global.add.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
+// Region-count windows are cleared this many windows ahead of the one that is being closed: far
+// enough that no block (up to three steps ahead of the step being logged) writes into it yet.
+__device__ __forceinline__ unsigned window_clear_ahead(const int window_steps) { return 2u / (unsigned)window_steps + 1u; }
+
 __device__ __forceinline__ int region_of(const SimDev& p, int i) {
     int lo = 0, hi = p.n_regions;                 // region_start[lo] <= i < region_start[hi]
     while (hi - lo > 1) {
@@ -192,6 +196,7 @@ __device__ __forceinline__ void update_group(const SimDev& p, const unsigned lon
         if (spike_bits & (1u << q)) {
             const int i = i0 + q;
             p.spike_ids[spk_pos & p.spike_mask] = i;
+            p.spike_tag[spk_pos & p.spike_mask] = (uint32_t)n;
             ++spk_pos;
             const int nch = (len[q] + kChunk - 1) / kChunk;
             for (int c = 0; c < nch; ++c) p.work[work_pos++] = make_int2(i, c);
@@ -266,7 +271,7 @@ __device__ __forceinline__ void finalize_step(const SimDev& p, const unsigned lo
     p.step_end[n & p.step_log_mask] = end;
     c->step_counts[n & 1ull] = 0ull;
     if ((n + 1) % (unsigned long long)p.window_steps == 0) {
-        const unsigned w = (unsigned)(((n + 1) / (unsigned long long)p.window_steps + 1) % p.max_windows);
+        const unsigned w = (unsigned)(((n + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
         for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
     }
     c->step = n + 1;
@@ -306,33 +311,47 @@ __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev 
 // ===========================================================================
 // Mode DB_EXEC_PERSISTENT: one cooperative kernel runs all the steps, one block
 // per SM.  Every block owns a fixed, contiguous range of 128-neuron tasks, so a
-// thread meets the same neurons in every step.  All global->SM traffic of the
-// update is staged through shared memory with cp.async (16 bytes per thread and
-// plane: ring x4, V, g x4, rt), which keeps the loaded data out of the register
-// file and lets the copies of the next task run while this one is computed:
-//   - while plane u of task k is consumed, plane u of task k + 1 is requested
-//     into the same shared-memory cells;
-//   - at the end of a step the state planes (V, g, rt -- the thread's own data)
-//     of the first task of the next step are requested BEFORE the grid barrier,
-//     the ring planes right after it.
-// Per step: wait for the barrier that closes the previous step (all deliveries
-// into this step's ring slot have landed), then per task consume the slot,
-// update, compact, and push the rows of the spikes this warp found (rows longer
-// than kInlineMax are queued and shared by the whole grid after a second
-// barrier), then arrive.  Delays are >= 1, so step n's deliveries never touch
-// slot n: one barrier per step suffices.  The barrier words alternate with the
-// step parity, so a word is frozen from the moment its target is reached until
-// every block has seen it; the high half of bar1 carries the spike count for
-// the raster log.
+// thread meets the same neurons in every step.
+//
+// Software pipeline across the step boundary.  The membrane step is fully
+// explicit (SI Eq.(5) takes J at time t, R8): V(n+1) and the spike decision of
+// step n depend on the state after step n-1 only, NOT on the arrivals consumed
+// in step n; only g(n+1) = alpha g(n) + x(n) needs ring slot n.  A step is
+// therefore split into
+//   A_n: V(n) -> V(n+1), refractory / threshold / reset, spike list L_n, and the
+//        push of L_n along its rows into slots n + d          (needs g(n))
+//   B_n: consume slot n, g(n) -> g(n+1)                       (needs L_m, m < n)
+// and the kernel runs "units": unit 0 = A_n0, unit j = B_(n0+j-1) then A_(n0+j)
+// in ONE pass over the data (same bytes as an unfused step), unit n_steps =
+// B_(n0+n_steps-1).  The result is the oracle's, operation for operation.
+// Unit j+1 needs only the deliveries of units <= j-1, so a block waits on a
+// monotonic arrival counter for "everyone has finished unit j-1" while it may
+// itself run a whole unit ahead: the barrier latency and the tail of the
+// deliveries are off the critical path.  Slots written by the fastest block
+// (up to n+1+d_max) must not meet the slot the slowest still consumes (n-1):
+// the ring depth is kept >= d_max + 3.
+//
+// All global->SM traffic of the update is staged through shared memory with
+// cp.async (16 bytes per thread and plane: ring x4, V, g x4, rt), which keeps
+// the loaded data out of the register file; while plane u of a task is
+// consumed, plane u of the warp's next task is requested into the same cells,
+// and the state planes of the first task of the next unit are requested before
+// the wait.  Spikes are pushed by the warp that found them; rows longer than
+// kInlineMax are shared by the warps of the block at the end of the unit.
+// The raster is written through one global cursor with a step tag per entry
+// (entries of adjacent steps may interleave); per-step counts go to
+// Ctl::unit_spikes and are folded into the step log by block 0.
 // ===========================================================================
 struct alignas(16) TypeSmem {        // TypeConst regrouped into 128-bit words for broadcast LDS.128
     float4 rec[4];                   // per receptor u: G_u, E_u, alpha_u, -
     float4 m0;                       // neg_gL, VL, kappa, Iext
     float4 m1;                       // Vth, Vreset, R (int bits), wq_bg (int bits)
-    uint4 m2;                        // M, T[0], -, -
+    uint4 m2;                        // M, T[0], T[1], T[2] (0xFFFFFFFF where m >= M)
 };
 
 constexpr int kStageBytesPerThread = 9 * 16 + 8;   // ring x4, V, g x4 (16 B each), rt (8 B)
+constexpr uint32_t kPlaneStride = kRunThreads * 16;   // bytes between staging planes (fixed: immediate offsets)
+constexpr int kStageBytes = kRunThreads * kStageBytesPerThread;
 
 __device__ __forceinline__ unsigned ld_cg_u32(const unsigned* p) {
     unsigned r;
@@ -369,11 +388,17 @@ __device__ __forceinline__ uint2 lds64(const uint32_t smem) {
     return r;
 }
 
-// Spin until the low half of *word reaches `target`; returns the word.
-__device__ __forceinline__ unsigned long long bar_wait(const unsigned long long* word, const unsigned target) {
-    unsigned long long v = ld_acquire_u64(word);
-    while ((unsigned)v < target) { __nanosleep(20); v = ld_acquire_u64(word); }
-    return v;
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned r;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
+    return r;
+}
+// Spin until every block has finished unit u of this launch: counter [u & 3] collects the arrivals
+// of the units u, u + 4, ... and only grows, so "all G blocks finished unit u" is count >= (u/4 + 1) G.
+__device__ __forceinline__ void bar_wait(const unsigned* bar, const unsigned u, const unsigned G) {
+    const unsigned* word = bar + (u & 3u);
+    const unsigned target = (u / 4u + 1u) * G;
+    while (ld_acquire_u32(word) < target) __nanosleep(20);
 }
 
 // Push one row (or one chunk of a row): 4 synapses per lane and 128-bit load,
@@ -425,28 +450,31 @@ __device__ __forceinline__ void deliver_span(const SimDev& p, const unsigned nlo
 
 struct RunCfg { unsigned n_steps; int n_tasks; int tasks_per_block; int iters; };
 
-// Shared-memory staging cells of one thread: plane k at sbase + k * pstride (k = 0..3 ring,
+// Shared-memory staging cells of one thread: plane k at sbase + k * kPlaneStride (k = 0..3 ring,
 // 4 V, 5..8 g), rt at srt.
-struct Stage { uint32_t sbase, pstride, srt; };
+struct Stage { uint32_t sbase, srt; };
 
 __device__ __forceinline__ void request_state(const SimDev& p, const Stage& sg, const int i0) {
     const size_t Np = (size_t)p.Npad;
-    cp_async16(sg.sbase + 4u * sg.pstride, p.V + i0);
+    cp_async16(sg.sbase + 4u * kPlaneStride, p.V + i0);
     cp_async8(sg.srt, p.rt + i0);
 #pragma unroll
-    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)(5 + u) * sg.pstride, p.g + u * Np + i0);
+    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)(5 + u) * kPlaneStride, p.g + u * Np + i0);
 }
 __device__ __forceinline__ void request_ring(const SimDev& p, const Stage& sg, const int32_t* slot_i0) {
     const size_t Np = (size_t)p.Npad;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)u * sg.pstride, slot_i0 + u * Np);
+    for (int u = 0; u < 4; ++u) cp_async16(sg.sbase + (unsigned)u * kPlaneStride, slot_i0 + u * Np);
 }
 
-// a1 for the four neurons of one thread, receptor by receptor, out of the staging cells.  While
-// plane u is consumed the same plane of the next task (i0 + next_off, if next_off != 0) is
-// requested.  tp0..tp3 are the neuron types; the caller passes the same variable four times when
-// they agree, which lets the constant loads (broadcast LDS.128) be shared.  Operation order:
-// DESIGN.md "Arithmetic contract".
+// The four neurons of one thread, receptor by receptor, out of the staging cells.
+//   kB: consume the ring planes of step nB (slot), add the Poisson background, g <- g alpha + x, store g
+//   kA: membrane step with the (new) g, refractory / threshold / reset, store V and rt; returns spike bits
+// While plane u is consumed the same plane of the next task (next_off neurons further, if != 0)
+// is requested (ring planes only if kB).  tp0..tp3 are the neuron types; the caller passes the
+// same variable four times when they agree, which lets the constant loads (broadcast LDS.128)
+// be shared.  Operation order: DESIGN.md "Arithmetic contract".
+template <bool kB, bool kA>
 __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem* s_tc,
                                                  const uint32_t (*s_T)[kPoissonMax], const Stage& sg,
                                                  const int tp0, const int tp1, const int tp2, const int tp3,
@@ -458,98 +486,119 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
     const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
     const float v[4] = {__uint_as_float(v_bits.x), __uint_as_float(v_bits.y), __uint_as_float(v_bits.z),
                         __uint_as_float(v_bits.w)};
-    float I[4];
+    const bool tail = (i0 + 3) >= p.N;              // only the last group can hold padding neurons
+    float I[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        const uint4 ab = lds128(sg.sbase + (unsigned)u * sg.pstride);
-        const uint4 gb = lds128(sg.sbase + (unsigned)(5 + u) * sg.pstride);
+        uint4 ab = make_uint4(0u, 0u, 0u, 0u);
+        if (kB) ab = lds128(sg.sbase + (unsigned)u * kPlaneStride);
+        const uint4 gb = lds128(sg.sbase + (unsigned)(5 + u) * kPlaneStride);
         if (next_off) {
-            cp_async16(sg.sbase + (unsigned)u * sg.pstride, slot + u * Np + next_off);
-            cp_async16(sg.sbase + (unsigned)(5 + u) * sg.pstride, p.g + u * Np + i0 + next_off);
+            if (kB) cp_async16(sg.sbase + (unsigned)u * kPlaneStride, slot + u * Np + next_off);
+            cp_async16(sg.sbase + (unsigned)(5 + u) * kPlaneStride, p.g + u * Np + i0 + next_off);
         }
-        int a[4] = {(int)ab.x, (int)ab.y, (int)ab.z, (int)ab.w};
-        const bool nz = (a[0] | a[1] | a[2] | a[3]) != 0;
-        if (nz) {                       // consumed: zero the cells again, check the overflow bound
-            st_cg_i4(slot + u * Np, make_int4(0, 0, 0, 0));
-            const int lim = 1 << 30;
-            if (a[0] > lim || a[0] < -lim || a[1] > lim || a[1] < -lim ||
-                a[2] > lim || a[2] < -lim || a[3] > lim || a[3] < -lim) p.ctl->overflow = 1u;
+        float gn[4] = {__uint_as_float(gb.x), __uint_as_float(gb.y), __uint_as_float(gb.z), __uint_as_float(gb.w)};
+        if (kB) {
+            int a[4] = {(int)ab.x, (int)ab.y, (int)ab.z, (int)ab.w};
+            if ((a[0] | a[1] | a[2] | a[3]) != 0) {  // consumed: zero the cells again, check the overflow bound
+                st_cg_i4(slot + u * Np, make_int4(0, 0, 0, 0));
+                const int lim = 1 << 30;
+                if (a[0] > lim || a[0] < -lim || a[1] > lim || a[1] < -lim ||
+                    a[2] > lim || a[2] < -lim || a[3] > lim || a[3] < -lim) p.ctl->overflow = 1u;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (u == 0) {           // Poisson background joins the AMPA arrivals (R14)
+                    // k = #{m < M : u >= T_m}; thresholds increase, so the first three decide almost always
+                    const uint4 m2 = s_tc[tp[q]].m2;
+                    unsigned k = (unsigned)(rw[q] >= m2.y) + (unsigned)(rw[q] >= m2.z) + (unsigned)(rw[q] >= m2.w);
+                    if (k == 3u) {
+                        if (m2.x > 3u) { while (k < m2.x && rw[q] >= s_T[tp[q]][k]) ++k; }
+                        else k = m2.x;  // padded thresholds (u = 0xFFFFFFFF) do not count
+                    }
+                    if (tail && (i0 + q) >= p.N) k = 0u;
+                    bg_acc += k;
+                    a[q] = (int)((unsigned)a[q] + k * (unsigned)__float_as_int(s_tc[tp[q]].m1.w));
+                }
+                const float x = __fmul_rn(__int2float_rn(a[q]), p.scale);
+                gn[q] = __fadd_rn(__fmul_rn(gn[q], s_tc[tp[q]].rec[u].z), x);
+            }
+            st_cg_f4(p.g + u * Np + i0, make_float4(gn[0], gn[1], gn[2], gn[3]));
         }
-        const float gu[4] = {__uint_as_float(gb.x), __uint_as_float(gb.y), __uint_as_float(gb.z), __uint_as_float(gb.w)};
-        float gn[4];
+        if (kA) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 r = s_tc[tp[q]].rec[u];
+                const float t = __fmul_rn(__fmul_rn(r.x, gn[q]), __fsub_rn(r.y, v[q]));
+                I[q] = (u == 0) ? t : __fadd_rn(I[q], t);
+            }
+        }
+    }
+    unsigned spike_bits = 0;
+    if (kA) {
+        unsigned rt[4] = {rt_bits.x & 0xFFFFu, rt_bits.x >> 16, rt_bits.y & 0xFFFFu, rt_bits.y >> 16};
+        float vn[4];
+        unsigned rt_changed = 0;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const float4 r = s_tc[tp[q]].rec[u];
-            float x;
-            if (u == 0) {               // Poisson background joins the AMPA arrivals (R14)
-                const uint4 m2 = s_tc[tp[q]].m2;
-                if ((i0 + q) < p.N && m2.x > 0u && rw[q] >= m2.y) {      // thresholds increase: count all u >= T_m
-                    int k = 1;
-                    while (k < (int)m2.x && rw[q] >= s_T[tp[q]][k]) ++k;
-                    bg_acc += (unsigned)k;
-                    a[q] = (int)((unsigned)a[q] + (unsigned)k * (unsigned)__float_as_int(s_tc[tp[q]].m1.w));
-                }
-                x = __fmul_rn(__int2float_rn(a[q]), p.scale);
-            } else {
-                x = nz ? __fmul_rn(__int2float_rn(a[q]), p.scale) : 0.0f;
+            const float4 m0 = s_tc[tp[q]].m0, m1 = s_tc[tp[q]].m1;
+            const float Iq = __fadd_rn(I[q], m0.w);
+            const float leak = __fmul_rn(m0.x, __fsub_rn(v[q], m0.y));
+            float w = __fadd_rn(v[q], __fmul_rn(m0.z, __fadd_rn(leak, Iq)));
+            if ((rt[q] & (unsigned)kRefMask) > 0u) { w = m1.y; rt[q] -= 1u; rt_changed = 1u; }
+            else if (w >= m1.x) {
+                const unsigned R = (unsigned)__float_as_int(m1.z);
+                w = m1.y; rt[q] |= R; rt_changed |= (unsigned)(R != 0u);
+                if (!tail || (i0 + q) < p.N) spike_bits |= 1u << q;
             }
-            const float t = __fmul_rn(__fmul_rn(r.x, gu[q]), __fsub_rn(r.y, v[q]));
-            I[q] = (u == 0) ? t : __fadd_rn(I[q], t);
-            gn[q] = __fadd_rn(__fmul_rn(gu[q], r.z), x);
+            vn[q] = w;
         }
-        st_cg_f4(p.g + u * Np + i0, make_float4(gn[0], gn[1], gn[2], gn[3]));
+        st_cg_f4(p.V + i0, make_float4(vn[0], vn[1], vn[2], vn[3]));
+        if (rt_changed) *reinterpret_cast<uint2*>(p.rt + i0) = make_uint2(rt[0] | (rt[1] << 16), rt[2] | (rt[3] << 16));
     }
-    unsigned rt[4] = {rt_bits.x & 0xFFFFu, rt_bits.x >> 16, rt_bits.y & 0xFFFFu, rt_bits.y >> 16};
-    float vn[4];
-    unsigned spike_bits = 0, rt_changed = 0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const float4 m0 = s_tc[tp[q]].m0, m1 = s_tc[tp[q]].m1;
-        const float Iq = __fadd_rn(I[q], m0.w);
-        const float leak = __fmul_rn(m0.x, __fsub_rn(v[q], m0.y));
-        float w = __fadd_rn(v[q], __fmul_rn(m0.z, __fadd_rn(leak, Iq)));
-        if ((rt[q] & (unsigned)kRefMask) > 0u) { w = m1.y; rt[q] -= 1u; rt_changed = 1u; }
-        else if (w >= m1.x) {
-            const unsigned R = (unsigned)__float_as_int(m1.z);
-            w = m1.y; rt[q] |= R; rt_changed |= (unsigned)(R != 0u);
-            if ((i0 + q) < p.N) spike_bits |= 1u << q;
-        }
-        vn[q] = w;
-    }
-    st_cg_f4(p.V + i0, make_float4(vn[0], vn[1], vn[2], vn[3]));
-    if (rt_changed) *reinterpret_cast<uint2*>(p.rt + i0) = make_uint2(rt[0] | (rt[1] << 16), rt[2] | (rt[3] << 16));
     return spike_bits;
 }
 
-// a1 + a2 + a3 + a4 for one 128-neuron task of one warp.  next_off != 0: distance (in neurons) to
-// the warp's next task of this step, whose planes are requested while this one is consumed.
-template <bool kHalf, bool kHeavy>
+constexpr int kHeavyListCap = 512;   // heavy rows one block can defer per unit; beyond that the finder pushes them itself
+
+struct BlockShared {                 // small per-block scratch of the persistent kernel
+    unsigned unit_spikes;            // spikes found by this block in the current unit
+    unsigned heavy_n;                // deferred heavy rows of the current unit
+    int heavy_row[kHeavyListCap];
+};
+
+// One 128-neuron task of one warp in unit (kB: B of step nB, kA: A of step nA).  next_off != 0:
+// distance (in neurons) to the warp's next task of this unit, whose planes are requested while
+// this one is consumed.
+template <bool kHalf, bool kHeavy, bool kB, bool kA>
 __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, const uint32_t (*s_T)[kPoissonMax],
-                                         const Stage& sg, const unsigned long long n, const int task,
-                                         const unsigned lane, const int next_off, unsigned* s_blk_spk,
-                                         unsigned& bg_acc) {
+                                         BlockShared* bs, const Stage& sg, const unsigned long long nB,
+                                         const unsigned long long nA, const int task, const unsigned lane,
+                                         const int next_off, unsigned& bg_acc) {
     const int grp = task * 32 + (int)lane;
     const int i0 = grp * 4;
     const size_t Np = (size_t)p.Npad;
-    int32_t* slot = p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
+    int32_t* slot = p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
     // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
-    const uint4 rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)),
-                                    p.seed_lo, p.seed_hi);
+    uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
+    if (kB) rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)),
+                                p.seed_lo, p.seed_hi);
     cp_async_wait_all();
-    const uint4 v_bits = lds128(sg.sbase + 4u * sg.pstride);
+    const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
     const uint2 rt_bits = lds64(sg.srt);
     if (next_off) {
-        cp_async16(sg.sbase + 4u * sg.pstride, p.V + i0 + next_off);
+        cp_async16(sg.sbase + 4u * kPlaneStride, p.V + i0 + next_off);
         cp_async8(sg.srt, p.rt + i0 + next_off);
     }
     const int tp0 = (int)((rt_bits.x >> 12) & 0xFu), tp1 = (int)(rt_bits.x >> 28);
     const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
     unsigned spike_bits;
     if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-        spike_bits = neuron_group(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+        spike_bits = neuron_group<kB, kA>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
     else                                // a type boundary inside the group (rare)
-        spike_bits = neuron_group(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+        spike_bits = neuron_group<kB, kA>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
     cp_async_commit();
+    if (!kA) return;
 
     // ---- a2 + a4 + a3: spikes are rare (rate * dt per neuron-step); whole warps skip this
     unsigned any = __ballot_sync(0xffffffffu, spike_bits != 0);
@@ -577,22 +626,23 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     if (lane == 0) {
         base = atomicAdd(&p.ctl->spike_cursor, (unsigned long long)tot);
         atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
-        atomicAdd(s_blk_spk, tot);
+        atomicAdd(&bs->unit_spikes, tot);
     }
     base = __shfl_sync(0xffffffffu, base, 0);
     unsigned long long pos = base + (inc - my_spk);
-    const unsigned win = (unsigned)((n / (unsigned long long)p.window_steps) % p.max_windows);
+    const unsigned win = (unsigned)((nA / (unsigned long long)p.window_steps) % p.max_windows);
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
             const int i = i0 + q;
             p.spike_ids[pos & p.spike_mask] = i;
+            p.spike_tag[pos & p.spike_mask] = (uint32_t)nA;
             ++pos;
             const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
             atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
         }
     // a3: the warp pushes the rows of its own spikes, one row at a time
-    const unsigned nlo = (unsigned)n;
+    const unsigned nlo = (unsigned)nA;
     while (any) {
         const int src = __ffs(any) - 1;
         any &= any - 1u;
@@ -602,139 +652,168 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
             const int l = __shfl_sync(0xffffffffu, len[q], src);
             const long long b = __shfl_sync(0xffffffffu, (long long)rb[q], src);
             if (!(bits & (1u << q))) continue;
-            if (kHeavy && l > kInlineMax) {                      // queue the chunks for the whole grid
-                const int nch = (l + kChunk - 1) / kChunk;
+            if (kHeavy && l > kInlineMax) {                      // leave it to the whole block (end of the unit)
                 unsigned at = 0;
-                if (lane == 0) at = atomicAdd(&p.ctl->hq_tail[n & 1ull], (unsigned)nch);
+                if (lane == 0) at = atomicAdd(&bs->heavy_n, 1u);
                 at = __shfl_sync(0xffffffffu, at, 0);
-                int2* q_out = p.hq + (size_t)(n & 1ull) * p.hq_cap + at;
-                const int j = (task * 32 + src) * 4 + q;
-                for (int ch = (int)lane; ch < nch; ch += 32) q_out[ch] = make_int2(j, ch);
-            } else {
-                deliver_span<kHalf>(p, nlo, (int64_t)b, l, lane);
+                if (at < (unsigned)kHeavyListCap) {
+                    if (lane == 0) bs->heavy_row[at] = (task * 32 + src) * 4 + q;
+                    continue;
+                }
             }
+            deliver_span<kHalf>(p, nlo, (int64_t)b, l, lane);
         }
     }
 }
 
+#ifdef DB_TRACE
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define DB_TRACE_MARK(s, k) do { if (p.trace && threadIdx.x == 0 && (s) < 64u) \
+    p.trace[((size_t)blockIdx.x * 64u + (s)) * 4u + (k)] = globaltimer_ns(); } while (0)
+#else
+#define DB_TRACE_MARK(s, k) do { } while (0)
+#endif
+
+struct RunCtx {                      // per-thread constants of the persistent kernel
+    unsigned long long n0;           // step at launch
+    int task0, last, i00, task_stride;
+    unsigned lane, warp, n_warps, G;
+    bool keeper;
+};
+
+// Unit j of the launch (see the header comment): B of step n0 + j - 1 (if kB), A of step n0 + j (if kA).
+template <bool kHalf, bool kHeavy, bool kB, bool kA>
+__device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, const RunCtx& c, const TypeSmem* s_tc,
+                                         const uint32_t (*s_T)[kPoissonMax], BlockShared* bs, const Stage& sg,
+                                         const unsigned j, unsigned long long& sb, unsigned& fin, unsigned& bg_acc) {
+    Ctl* const ctl = p.ctl;
+    const unsigned long long nA = c.n0 + j, nB = c.n0 + j - 1ull;
+    if (j >= 2u) {                     // every delivery of the units <= j - 2 must have landed
+        if (threadIdx.x == 0) {
+            bar_wait(ctl->bar, j - 2u, c.G);
+            if (c.keeper) {            // fold the spike count of unit j - 2 into the step log
+                const unsigned u = j - 2u;
+                sb += (unsigned long long)ld_cg_u32(&ctl->unit_spikes[u & 3u]);
+                ctl->unit_spikes[u & 3u] = 0u;
+                const unsigned long long np = c.n0 + u;
+                p.step_end[np & p.step_log_mask] = sb;
+                if ((np + 1) % (unsigned long long)p.window_steps == 0) {
+                    const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
+                    for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
+                }
+                fin = u + 1u;
+            }
+        }
+        __syncthreads();
+    }
+    DB_TRACE_MARK(j, 0);
+    if (c.task0 < c.last) {
+        if (kB) request_ring(p, sg, p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * (size_t)p.Npad + c.i00);
+        cp_async_commit();
+        for (int task = c.task0; task < c.last; task += (int)c.n_warps) {
+            const int next_off = (task + (int)c.n_warps < c.last) ? c.task_stride : 0;
+            run_task<kHalf, kHeavy, kB, kA>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
+        }
+        if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
+    }
+    DB_TRACE_MARK(j, 1);
+    __syncthreads();
+    if (kHeavy && kA) {                // rows too long for one warp: shared by the warps of the block
+        const unsigned nh = min(bs->heavy_n, (unsigned)kHeavyListCap);
+        if (nh) {
+            unsigned idx = 0;
+            for (unsigned r = 0; r < nh; ++r) {
+                const int row = bs->heavy_row[r];
+                const int64_t rb = __ldg(p.row_begin + row);
+                const int len = __ldg(p.row_len + row);
+                for (int off = 0; off < len; off += kChunk, ++idx)
+                    if (idx % c.n_warps == c.warp)
+                        deliver_span<kHalf>(p, (unsigned)nA, rb + off, min(kChunk, len - off), c.lane);
+            }
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) bs->heavy_n = 0u;
+    }
+    DB_TRACE_MARK(j, 2);
+    if (threadIdx.x == 0) {
+        const unsigned k = bs->unit_spikes;
+        bs->unit_spikes = 0u;
+        if (k) atomicAdd(&ctl->unit_spikes[j & 3u], k);
+        __threadfence();
+        atomicAdd(&ctl->bar[j & 3u], 1u);
+    }
+    DB_TRACE_MARK(j, 3);
+}
+
 template <bool kHalf, bool kHeavy>
 __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ SimDev p, const RunCfg cfg) {
-    extern __shared__ uint4 s_stage[];                 // blockDim.x * kStageBytesPerThread bytes
+    extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
     __shared__ uint32_t s_T[kMaxTypes][kPoissonMax];
-    __shared__ unsigned s_blk_spk, s_hq_n;
-    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5;
+    __shared__ BlockShared bs;
+    RunCtx c;
+    c.lane = threadIdx.x & 31u; c.warp = threadIdx.x >> 5; c.n_warps = blockDim.x >> 5; c.G = gridDim.x;
     for (int t = (int)threadIdx.x; t < kMaxTypes; t += (int)blockDim.x) {
-        const TypeConst& c = p.tc[t];
+        const TypeConst& tc = p.tc[t];
         TypeSmem r;
-        for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(c.G[u], c.E[u], c.alpha[u], 0.0f);
-        r.m0 = make_float4(c.neg_gL, c.VL, c.kappa, c.Iext);
-        r.m1 = make_float4(c.Vth, c.Vreset, __int_as_float(c.R), __int_as_float(c.wq_bg));
-        r.m2 = make_uint4((unsigned)c.M, c.M > 0 ? c.T[0] : 0xFFFFFFFFu, 0u, 0u);
+        for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(tc.G[u], tc.E[u], tc.alpha[u], 0.0f);
+        r.m0 = make_float4(tc.neg_gL, tc.VL, tc.kappa, tc.Iext);
+        r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
+        r.m2 = make_uint4((unsigned)tc.M, tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu, tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu,
+                          tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu);
         s_tc[t] = r;
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
         s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
-    if (threadIdx.x == 0) { s_blk_spk = 0u; s_hq_n = 0u; }
+    if (threadIdx.x == 0) { bs.unit_spikes = 0u; bs.heavy_n = 0u; }
     __syncthreads();
 
     Stage sg;
-    sg.pstride = blockDim.x * 16u;
     sg.sbase = (uint32_t)__cvta_generic_to_shared(s_stage) + threadIdx.x * 16u;
-    sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * sg.pstride + threadIdx.x * 8u;
+    sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * kPlaneStride + threadIdx.x * 8u;
 
-    Ctl* const ctl = p.ctl;
-    const unsigned long long n0 = ctl->step;          // nobody writes it before the end of the launch
-    unsigned long long sb = ctl->spike_begin;         // raster bookkeeping: block 0, thread 0
-    unsigned hi_even = 0u, hi_odd = 0u;
-    const bool keeper = (blockIdx.x == 0 && threadIdx.x == 0);
+    c.n0 = p.ctl->step;                               // nobody writes it before the end of the launch
+    unsigned long long sb = p.ctl->spike_begin;       // raster bookkeeping: block 0, thread 0
+    unsigned fin = 0u;                                // units whose step the keeper has logged
+    c.keeper = (blockIdx.x == 0 && threadIdx.x == 0);
     const int first = (int)blockIdx.x * cfg.tasks_per_block;
-    const int last = min(first + cfg.tasks_per_block, cfg.n_tasks);
-    const int task0 = first + (int)warp;              // the warp's first task of every step
-    const int i00 = (task0 * 32 + (int)lane) * 4;
-    const int task_stride = (int)n_warps * 128;       // neurons between consecutive tasks of a warp
-    const unsigned G = gridDim.x;
-    const size_t Np = (size_t)p.Npad;
+    c.last = min(first + cfg.tasks_per_block, cfg.n_tasks);
+    c.task0 = first + (int)c.warp;                    // the warp's first task of every unit
+    c.i00 = (c.task0 * 32 + (int)c.lane) * 4;
+    c.task_stride = (int)c.n_warps * 128;             // neurons between consecutive tasks of a warp
     unsigned bg_acc = 0u;
+    if (cfg.n_steps == 0) return;
 
-    // closes step sp: the keeper logs the raster position and clears the region window two ahead
-    auto close_step = [&](const unsigned sp, const unsigned long long word) {
-        const unsigned hi = (unsigned)(word >> 32);
-        if (sp & 1u) { sb += (unsigned long long)(hi - hi_odd); hi_odd = hi; }
-        else         { sb += (unsigned long long)(hi - hi_even); hi_even = hi; }
-        const unsigned long long np = n0 + sp;
-        p.step_end[np & p.step_log_mask] = sb;
-        if ((np + 1) % (unsigned long long)p.window_steps == 0) {
-            const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + 1) % p.max_windows);
-            for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
-        }
-    };
+    if (c.task0 < c.last) { request_state(p, sg, c.i00); cp_async_commit(); }
+    run_unit<kHalf, kHeavy, false, true>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, sb, fin, bg_acc);
+    for (unsigned j = 1; j < cfg.n_steps; ++j)
+        run_unit<kHalf, kHeavy, true, true>(p, cfg, c, s_tc, s_T, &bs, sg, j, sb, fin, bg_acc);
+    run_unit<kHalf, kHeavy, true, false>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, sb, fin, bg_acc);
 
-    if (task0 < last && cfg.n_steps > 0) { request_state(p, sg, i00); cp_async_commit(); }
-    for (unsigned s = 0; s < cfg.n_steps; ++s) {
-        const unsigned long long n = n0 + s;
-        if (s > 0) {                                   // every delivery of step n - 1 must have landed
-            const unsigned sp = s - 1;
-            if (threadIdx.x == 0) {
-                const unsigned target = (sp / 2u + 1u) * G;
-                if (kHeavy) {
-                    bar_wait(&ctl->bar2[sp & 1u], target);
-                    if (keeper) ctl->hq_tail[sp & 1u] = 0u;
-                } else {
-                    const unsigned long long w = bar_wait(&ctl->bar1[sp & 1u], target);
-                    if (keeper) close_step(sp, w);
-                }
+    // close the launch: log the remaining steps and publish the position
+    if (c.keeper) {
+        if (cfg.n_steps >= 1u) bar_wait(p.ctl->bar, cfg.n_steps - 1u, c.G);   // the last unit that produces spikes
+        bar_wait(p.ctl->bar, cfg.n_steps, c.G);
+        for (unsigned u = fin; u < cfg.n_steps; ++u) {
+            sb += (unsigned long long)ld_cg_u32(&p.ctl->unit_spikes[u & 3u]);
+            p.ctl->unit_spikes[u & 3u] = 0u;
+            const unsigned long long np = c.n0 + u;
+            p.step_end[np & p.step_log_mask] = sb;
+            if ((np + 1) % (unsigned long long)p.window_steps == 0) {
+                const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
+                for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
             }
-            __syncthreads();
         }
-        if (task0 < last) {
-            request_ring(p, sg, p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np + i00);
-            cp_async_commit();
-            for (int task = task0; task < last; task += (int)n_warps) {
-                const int next_off = (task + (int)n_warps < last) ? task_stride : 0;
-                run_task<kHalf, kHeavy>(p, s_tc, s_T, sg, n, task, lane, next_off, &s_blk_spk, bg_acc);
-            }
-            if (s + 1 < cfg.n_steps) { request_state(p, sg, i00); cp_async_commit(); }   // own data: no need to wait for the grid
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            const unsigned k = s_blk_spk;
-            s_blk_spk = 0u;
-            __threadfence();
-            atomicAdd(&ctl->bar1[s & 1u], ((unsigned long long)k << 32) | 1ull);
-        }
-        if (kHeavy) {                                  // rows too long for one warp: the whole grid shares them
-            if (threadIdx.x == 0) {
-                const unsigned long long w = bar_wait(&ctl->bar1[s & 1u], (s / 2u + 1u) * G);
-                if (keeper) close_step(s, w);
-                s_hq_n = ld_cg_u32(&ctl->hq_tail[n & 1ull]);
-            }
-            __syncthreads();
-            const unsigned cnt = s_hq_n;
-            const int2* qv = p.hq + (size_t)(n & 1ull) * p.hq_cap;
-            for (unsigned q = blockIdx.x * n_warps + warp; q < cnt; q += G * n_warps) {
-                const int2 wk = qv[q];
-                const int64_t rb = __ldg(p.row_begin + wk.x) + (int64_t)wk.y * kChunk;
-                int len = __ldg(p.row_len + wk.x) - wk.y * kChunk;
-                len = len < kChunk ? len : kChunk;
-                deliver_span<kHalf>(p, (unsigned)n, rb, len, lane);
-            }
-            __syncthreads();
-            if (threadIdx.x == 0) { __threadfence(); atomicAdd(&ctl->bar2[s & 1u], 1ull); }
-        }
-    }
-    // close the last step and publish the position
-    if (cfg.n_steps > 0 && keeper) {
-        const unsigned sp = cfg.n_steps - 1;
-        const unsigned target = (sp / 2u + 1u) * G;
-        if (kHeavy) { bar_wait(&ctl->bar2[sp & 1u], target); ctl->hq_tail[sp & 1u] = 0u; }
-        else close_step(sp, bar_wait(&ctl->bar1[sp & 1u], target));
-        ctl->spike_begin = sb;
-        ctl->step = n0 + cfg.n_steps;
+        p.ctl->spike_begin = sb;
+        p.ctl->step = c.n0 + cfg.n_steps;
     }
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
-    if (lane == 0 && bg_warp)
-        atomicAdd(p.bg_parts + ((blockIdx.x * n_warps + warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
+    if (c.lane == 0 && bg_warp)
+        atomicAdd(p.bg_parts + ((blockIdx.x * c.n_warps + c.warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
 }
 
 // ---------------------------------------------------------------------------
@@ -796,7 +875,7 @@ cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok) {
     int grid = 0, threads = 0, per_sm = 0;
     RunCfg cfg{};
     run_shape(p, n_sm, &grid, &threads, &cfg);
-    const size_t smem = (size_t)threads * kStageBytesPerThread;
+    const size_t smem = (size_t)kStageBytes;
     cudaError_t e = cudaFuncSetAttribute(run_fn(p, heavy), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, run_fn(p, heavy), threads, smem);
@@ -809,11 +888,11 @@ cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int
     RunCfg cfg{};
     run_shape(p, n_sm, &grid, &threads, &cfg);
     cfg.n_steps = n_steps;
-    cudaError_t e = cudaMemsetAsync(p.ctl->bar1, 0, sizeof(p.ctl->bar1) + sizeof(p.ctl->bar2), st);   // bar1, bar2 are adjacent
+    cudaError_t e = cudaMemsetAsync(p.ctl->bar, 0, sizeof(p.ctl->bar) + sizeof(p.ctl->unit_spikes), st);   // adjacent
     if (e != cudaSuccess) return e;
     void* args[] = {(void*)&p, (void*)&cfg};
     return cudaLaunchCooperativeKernel(run_fn(p, heavy), dim3(grid), dim3(threads), args,
-                                       (size_t)threads * kStageBytesPerThread, st);
+                                       (size_t)kStageBytes, st);
 }
 
 }  // namespace dbk
