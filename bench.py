@@ -13,7 +13,8 @@ Prints ONE JSON line (rank 0):
   e2e           same metric through the C ABI with HOST buffers: every bench step restores the neuron
                 state from pinned host memory (db_write_state), steps, and reads the raster, the
                 region rates and V back to the host (db_read_spikes / db_region_rates / db_read_state)
-  roofline      the dominant kernel (k_update) against the measured HBM copy peak
+  roofline      the dominant kernel of the timed region (k_run in persistent mode: one launch = all the time
+                steps of a db_step call; k_update in two-kernel mode) against the measured HBM copy peak
   cpu_baseline  the oracle (oracle/, as it stands) on the host cores, on a bounded sample
 ``--impl reference`` times the oracle instead (same metric, unit and config).
 
@@ -46,6 +47,10 @@ UNIT = "events/s"
 UPDATE_BYTES_PER_NEURON_STEP = 58      # read V 4 + g 16 + rt 2 + ring slot 16; write V 4 + g 16 (compulsory)
 UPDATE_BYTES_SURVEY = 76               # plus rt 2 and the zeroed slot 16 written back every step
 DELIVER_BYTES_PER_EVENT = {0: 17, 1: 15}   # tgt|rec 4 + w 4 (fp32) / 2 (fp16) + delay 1 + accumulator read 4 + write 4
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full`
+# captures under profiles/ (bytes per launch in that capture's configuration; see the .md beside each)
+NCU_TRAFFIC = {"k_update": 38.1e6,          # profiles/r1a_two_kernel_baseline.md (one time step)
+               "k_run_per_sim_step": 24.7e6}  # profiles/r1b_persistent_kernel.md (4.93 GB per 200-step launch)
 
 
 def _peaks():
@@ -209,19 +214,23 @@ def run_ours(args):
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # one CUDA event before every db_step call and one after the last, on the stream the library launches on
+    # (torch's current stream, handed to db_create by the binding): per-launch durations of the timed region
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    ev0.record()
-    for _ in range(args.steps):
+    evs[0].record()
+    for k in range(args.steps):
         sim.db_step(n_sim)
-    ev1.record()
+        evs[k + 1].record()
     barrier()
     clk = clocks.stop() if rank == 0 else None
-    ms = ev0.elapsed_time(ev1)
+    ms = evs[0].elapsed_time(evs[-1])
+    launch_ms = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
     c1 = sim.db_get_counters()
     events = c1["events"] - c0["events"]
     spikes = c1["spikes"] - c0["spikes"]
     launches = c1["launches"] - c0["launches"]
+    exec_used = c1["exec_mode"]
     t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
     tot = torch.tensor([events, spikes, launches], dtype=torch.float64, device=f"cuda:{local}")
     if dist is not None:
@@ -234,26 +243,52 @@ def run_ours(args):
     value = events_all / secs
     rate_hz = spikes_all / (world * N) / bio_s
 
-    # ---------------- per-kernel roofline (CUDA events around every kernel, on the library's stream) ----
-    prof = sim.db_step_profiled(args.profile_steps)
+    # ---------------- roofline of the dominant kernel of the timed region ---------------------------
     peak, peak_src = _peaks()
-    upd_s = prof["update_ms"] * 1e-3 / prof["steps"]
-    del_s = prof["deliver_ms"] * 1e-3 / prof["steps"]
-    upd_gbs = UPDATE_BYTES_PER_NEURON_STEP * N / upd_s / 1e9
-    del_bytes = DELIVER_BYTES_PER_EVENT[fp16] * prof["events"] / prof["steps"]
-    del_gbs = del_bytes / del_s / 1e9
-    roofline = {
-        "bound": "hbm", "kernel": "k_update", "achieved": upd_gbs, "peak": peak, "unit": "GB/s", "frac": upd_gbs / peak,
-        "traffic": None, "peak_source": peak_src,
-        "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
-        "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
-        "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
-        "deliver": {"kernel": "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
-                    "events_per_launch": prof["events"] / prof["steps"], "bytes_per_event": DELIVER_BYTES_PER_EVENT[fp16],
-                    "share_of_step": prof["deliver_ms"] / max(prof["total_ms"], 1e-12)},
-        "note": "per-step working set (state 22 MB + one ring slot 16 MB) is L2-resident at this size: achieved is "
-                "algorithmic bytes / time and may exceed the HBM copy peak",
-    }
+    ev_bytes = DELIVER_BYTES_PER_EVENT[fp16]
+    note = ("per-step working set (state 22 MB + one ring slot 16 MB) fits the 126 MB L2 at this size: achieved is "
+            "algorithmic bytes / time; `traffic` is the DRAM traffic ncu saw (profiles/)")
+    if exec_used == db.EXEC_PERSISTENT:
+        # k_run: ONE launch = n_sim fused steps (a1 + a2 + a3 + a4); algorithmic bytes per launch =
+        # n_sim * 58 B * N (update) + 17 B (15 B fp16) * events of the launch (delivery)
+        upd_bytes = float(UPDATE_BYTES_PER_NEURON_STEP) * N * n_sim
+        del_bytes = float(ev_bytes) * events / max(args.steps, 1)
+        dur_s = float(np.mean(launch_ms)) * 1e-3
+        gbs = (upd_bytes + del_bytes) / dur_s / 1e9
+        roofline = {
+            "bound": "hbm", "kernel": "k_run (persistent: update + compaction + delivery + region counts, fused)",
+            "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": NCU_TRAFFIC["k_run_per_sim_step"] * n_sim,
+            "peak_source": peak_src, "bytes_per_launch": upd_bytes + del_bytes,
+            "bytes_per_launch_update": upd_bytes, "bytes_per_launch_delivery": del_bytes,
+            "sim_steps_per_launch": n_sim, "us_per_launch": dur_s * 1e6, "us_per_sim_step": dur_s * 1e6 / n_sim,
+            "launch_ms": launch_ms, "frac_of_nominal_8000": gbs / 8000.0,
+            "achieved_survey_76B": (float(UPDATE_BYTES_SURVEY) * N * n_sim + del_bytes) / dur_s / 1e9,
+            "share_of_step": 1.0, "note": note,
+        }
+    else:
+        roofline = None
+    # two-kernel mode, CUDA events around every kernel (db_step_profiled): the roofline of that mode, and
+    # context for the fused kernel
+    if args.profile_steps > 0:
+        prof = sim.db_step_profiled(args.profile_steps)
+        upd_s = prof["update_ms"] * 1e-3 / prof["steps"]
+        del_s = prof["deliver_ms"] * 1e-3 / prof["steps"]
+        upd_gbs = UPDATE_BYTES_PER_NEURON_STEP * N / upd_s / 1e9
+        del_gbs = ev_bytes * prof["events"] / prof["steps"] / del_s / 1e9
+        two = {
+            "bound": "hbm", "kernel": "k_update", "achieved": upd_gbs, "peak": peak, "unit": "GB/s",
+            "frac": upd_gbs / peak, "traffic": NCU_TRAFFIC.get("k_update"), "peak_source": peak_src,
+            "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
+            "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
+            "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
+            "deliver": {"kernel": "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
+                        "events_per_launch": prof["events"] / prof["steps"], "bytes_per_event": ev_bytes,
+                        "share_of_step": prof["deliver_ms"] / max(prof["total_ms"], 1e-12)},
+        }
+        if roofline is None:
+            roofline = dict(two, note=note)
+        else:
+            roofline["two_kernel_mode"] = two
 
     # ---------------- end to end through the C ABI with host buffers --------------------------------
     V_h = torch.empty(N, dtype=torch.float32).pin_memory()
@@ -305,7 +340,6 @@ def run_ours(args):
            "what": "db_write_state(V, g[4], ref) from pinned host + db_step + db_read_spikes + db_region_rates + "
                    "db_read_state(V) to pinned host, wall clock"}
 
-    exec_used = sim.db_get_counters()["exec_mode"]
     sim.db_destroy()
 
     # ---------------- CPU baseline: the oracle on the host cores (rank 0, N = 1 only) ----------------
