@@ -164,6 +164,7 @@ typedef struct db_phase_times {
 #define DB_FIELD_REF    5  /* int32  [count], refractory steps left */
 #define DB_FIELD_TYPE   6  /* uint8  [count] */
 #define DB_FIELD_RING   7  /* int32  [D][count][4] fixed-point arrivals, slot = step mod D */
+#define DB_FIELD_OUTDEG 8  /* int32  [count], out-degree = length of the neuron's destination list (read only) */
 
 /* a0: generate the network on the device from `spec` (seed keys every draw of
  * the generator), build the CSR and initialise the state (V0 keyed by

@@ -65,6 +65,8 @@ def lib():
         L.orc_gen_create.restype = C.c_void_p
         L.orc_gen_create.argtypes = [C.POINTER(NetSpec), C.c_uint64]
         L.orc_gen_destroy.argtypes = [C.c_void_p]
+        L.orc_gen_ntype.restype = C.c_int32
+        L.orc_gen_ntype.argtypes = [C.c_void_p, C.c_int64]
         L.orc_gen_owner_edges.restype = C.c_int64
         L.orc_gen_owner_edges.argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 5
         L.orc_sim_create.restype = C.c_void_p
@@ -214,6 +216,9 @@ class OwnerEdges:
         n = lib().orc_gen_owner_edges(self.h, int(i), cap, _p(src), _p(tgt), _p(w), _p(d), _p(r))
         assert n <= cap
         return dict(src=src[:n], tgt=tgt[:n], w=w[:n], delay=d[:n], rec=r[:n])
+
+    def ntype(self, first: int, count: int) -> np.ndarray:
+        return np.array([lib().orc_gen_ntype(self.h, int(i)) for i in range(first, first + count)], np.uint8)
 
     def close(self):
         if self.h:

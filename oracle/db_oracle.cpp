@@ -454,6 +454,9 @@ orc_gen* orc_gen_create(const orc_net_spec* sp, uint64_t seed) {
 }
 void orc_gen_destroy(orc_gen* g) { delete g; }
 
+// neuron type of neuron i (0 excitatory, 1 inhibitory): excitatory neurons come first in each region
+int32_t orc_gen_ntype(const orc_gen* g, int64_t i) { return g->is_inh(i) ? 1 : 0; }
+
 // The synapses owned by neuron i, in slot order (sampled parity at full size).
 // Returns the count; writes at most cap entries.
 int64_t orc_gen_owner_edges(const orc_gen* g, int64_t i, int64_t cap, int32_t* src, int32_t* tgt,

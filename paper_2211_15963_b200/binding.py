@@ -16,7 +16,8 @@ from . import build as _build
 
 DB_OK, DB_EINVAL, DB_ENOMEM, DB_ECUDA, DB_ERANGE, DB_ESTATE = 0, -1, -2, -3, -4, -5
 EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT = 0, 1, 2
-FIELD_V, FIELD_G_AMPA, FIELD_G_NMDA, FIELD_G_GABAA, FIELD_G_GABAB, FIELD_REF, FIELD_TYPE, FIELD_RING = range(8)
+(FIELD_V, FIELD_G_AMPA, FIELD_G_NMDA, FIELD_G_GABAA, FIELD_G_GABAB, FIELD_REF, FIELD_TYPE, FIELD_RING,
+ FIELD_OUTDEG) = range(9)
 
 EXPORTS = [
     "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_step_profiled", "db_read_spikes",
@@ -282,7 +283,7 @@ class Sim:
         count = self.N - first if count is None else count
         if field == FIELD_RING:
             out = np.empty((self.D, count, 4), np.int32)
-        elif field == FIELD_REF:
+        elif field in (FIELD_REF, FIELD_OUTDEG):
             out = np.empty(count, np.int32)
         elif field == FIELD_TYPE:
             out = np.empty(count, np.uint8)

@@ -555,6 +555,8 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
         }
         break;
     }
+    case DB_FIELD_OUTDEG:
+        CK(cudaMemcpy(dst, d.row_len + first, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;
     case DB_FIELD_RING: {
         // API slot j holds the arrivals of the step t in [n, n + D) with t mod D == j; device slot = t mod d.D
         Ctl c;
