@@ -28,22 +28,23 @@ struct TypeConst {                   // per neuron type, rounded once on the hos
     uint32_t T[kPoissonMax];
 };
 
-struct Ctl {                         // device-resident control block
+struct alignas(128) Ctl {            // device-resident control block
     unsigned long long step;         // current time step n
     unsigned long long spike_begin;  // spikes emitted before step n
     unsigned long long step_counts[2];  // [n & 1] of step n: high 32 = spikes, low 32 = work items (one atomic)
     unsigned long long events;       // synaptic events delivered so far
+    unsigned long long spike_cursor; // persistent kernel: next free raster position (= spike_begin between steps)
     unsigned int overflow;           // sticky ring overflow flag
     unsigned int done_blocks;        // delivery kernel: finished-block ticket
-    unsigned int pad0[2];
-    // persistent kernel (see db_step.cu): arrivals of the blocks that finished unit j go to the
-    // monotonic counter [j & 3] (blocks are at most two units apart), the spike count of the step
-    // produced by unit j to unit_spikes[j & 3]
+    unsigned int pad0[18];
+    // persistent kernel (see db_step.cu), on a 128-byte line of their own (every block polls it):
+    // arrivals of the blocks that closed unit j go to the monotonic counter [j & 3] (blocks are at most
+    // two units apart), the spike count of the step produced by unit j to unit_spikes[j & 3]
     unsigned int bar[4];
     unsigned int unit_spikes[4];
-    unsigned int pad1[2];
-    unsigned long long spike_cursor; // persistent kernel: next free raster position (= spike_begin between steps)
+    unsigned int pad1[24];
 };
+static_assert(sizeof(Ctl) == 256, "Ctl layout");
 
 constexpr int kBgParts = 1024;       // background-event counter is spread over this many cells
 

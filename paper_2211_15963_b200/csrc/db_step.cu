@@ -563,6 +563,7 @@ constexpr int kHeavyListCap = 512;   // heavy rows one block can defer per unit;
 
 struct BlockShared {                 // small per-block scratch of the persistent kernel
     unsigned unit_spikes;            // spikes found by this block in the current unit
+    unsigned long long events;       // synaptic events of this block's spikes (whole launch)
     unsigned heavy_n;                // deferred heavy rows of the current unit
     int heavy_row[kHeavyListCap];
 };
@@ -625,7 +626,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     unsigned long long base = 0;
     if (lane == 0) {
         base = atomicAdd(&p.ctl->spike_cursor, (unsigned long long)tot);
-        atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
+        atomicAdd(&bs->events, (unsigned long long)ev_warp);   // flushed once per block at the end of the launch
         atomicAdd(&bs->unit_spikes, tot);
     }
     base = __shfl_sync(0xffffffffu, base, 0);
@@ -638,9 +639,8 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
             p.spike_ids[pos & p.spike_mask] = i;
             p.spike_tag[pos & p.spike_mask] = (uint32_t)nA;
             ++pos;
-            const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
-            atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
-        }
+            if (p.n_regions > 1) atomicAdd(p.region_counts + (size_t)win * p.n_regions + region_of(p, i), 1u);
+        }                                                      // one region: added per block and unit (run_unit)
     // a3: the warp pushes the rows of its own spikes, one row at a time
     const unsigned nlo = (unsigned)nA;
     while (any) {
@@ -742,7 +742,11 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
     if (threadIdx.x == 0) {
         const unsigned k = bs->unit_spikes;
         bs->unit_spikes = 0u;
-        if (k) atomicAdd(&ctl->unit_spikes[j & 3u], k);
+        if (k) {
+            atomicAdd(&ctl->unit_spikes[j & 3u], k);
+            if (p.n_regions == 1)
+                atomicAdd(p.region_counts + (size_t)((nA / (unsigned long long)p.window_steps) % p.max_windows), k);
+        }
         __threadfence();
         atomicAdd(&ctl->bar[j & 3u], 1u);
     }
@@ -769,7 +773,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
         s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
-    if (threadIdx.x == 0) { bs.unit_spikes = 0u; bs.heavy_n = 0u; }
+    if (threadIdx.x == 0) { bs.unit_spikes = 0u; bs.heavy_n = 0u; bs.events = 0ull; }
     __syncthreads();
 
     Stage sg;
@@ -811,6 +815,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
         p.ctl->spike_begin = sb;
         p.ctl->step = c.n0 + cfg.n_steps;
     }
+    if (threadIdx.x == 0 && bs.events) atomicAdd(&p.ctl->events, bs.events);   // every emit of the block lies before the last barrier
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (c.lane == 0 && bg_warp)
         atomicAdd(p.bg_parts + ((blockIdx.x * c.n_warps + c.warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
