@@ -559,11 +559,14 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
     return spike_bits;
 }
 
+constexpr int kSpkCap = 1024;        // spikes one block can stage per unit; beyond that the finder reserves raster positions itself
 constexpr int kHeavyListCap = 512;   // heavy rows one block can defer per unit; beyond that the finder pushes them itself
 
 struct BlockShared {                 // small per-block scratch of the persistent kernel
-    unsigned unit_spikes;            // spikes found by this block in the current unit
+    unsigned unit_spikes[2];         // [unit & 1] spikes found by this block in the unit
+    unsigned staged[2];              // [unit & 1] how many of them wait in spk[] for their raster position
     unsigned long long events;       // synaptic events of this block's spikes (whole launch)
+    int spk[2][kSpkCap];             // [unit & 1] spikes of the unit, copied to the raster after the unit's barrier
     unsigned heavy_n;                // deferred heavy rows of the current unit
     int heavy_row[kHeavyListCap];
 };
@@ -623,22 +626,35 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     }
     const unsigned tot = __shfl_sync(0xffffffffu, inc, 31);
     const unsigned ev_warp = __reduce_add_sync(0xffffffffu, my_events);
-    unsigned long long base = 0;
+    // a2: the ids go to the block's list of the unit (shared memory); one warp copies the list to the
+    // raster after the unit's barrier, with ONE reservation on the global cursor per block and unit
+    const unsigned par = (unsigned)nA & 1u;
+    unsigned lbase = 0;
     if (lane == 0) {
-        base = atomicAdd(&p.ctl->spike_cursor, (unsigned long long)tot);
+        lbase = atomicAdd(&bs->unit_spikes[par], tot);
         atomicAdd(&bs->events, (unsigned long long)ev_warp);   // flushed once per block at the end of the launch
-        atomicAdd(&bs->unit_spikes, tot);
+        if (lbase + tot <= (unsigned)kSpkCap) atomicMax(&bs->staged[par], lbase + tot);
     }
-    base = __shfl_sync(0xffffffffu, base, 0);
+    lbase = __shfl_sync(0xffffffffu, lbase, 0);
+    const bool staged = (lbase + tot <= (unsigned)kSpkCap);   // else (list full): positions straight from the cursor
+    unsigned long long base = 0;
+    if (!staged) {
+        if (lane == 0) base = atomicAdd(&p.ctl->spike_cursor, (unsigned long long)tot);
+        base = __shfl_sync(0xffffffffu, base, 0);
+    }
+    unsigned at = lbase + (inc - my_spk);
     unsigned long long pos = base + (inc - my_spk);
     const unsigned win = (unsigned)((nA / (unsigned long long)p.window_steps) % p.max_windows);
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
             const int i = i0 + q;
-            p.spike_ids[pos & p.spike_mask] = i;
-            p.spike_tag[pos & p.spike_mask] = (uint32_t)nA;
-            ++pos;
+            if (staged) bs->spk[par][at++] = i;
+            else {
+                p.spike_ids[pos & p.spike_mask] = i;
+                p.spike_tag[pos & p.spike_mask] = (uint32_t)nA;
+                ++pos;
+            }
             if (p.n_regions > 1) atomicAdd(p.region_counts + (size_t)win * p.n_regions + region_of(p, i), 1u);
         }                                                      // one region: added per block and unit (run_unit)
     // a3: the warp pushes the rows of its own spikes, one row at a time
@@ -739,16 +755,39 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         if (threadIdx.x == 0) bs->heavy_n = 0u;
     }
     DB_TRACE_MARK(j, 2);
-    if (threadIdx.x == 0) {
-        const unsigned k = bs->unit_spikes;
-        bs->unit_spikes = 0u;
-        if (k) {
-            atomicAdd(&ctl->unit_spikes[j & 3u], k);
-            if (p.n_regions == 1)
-                atomicAdd(p.region_counts + (size_t)((nA / (unsigned long long)p.window_steps) % p.max_windows), k);
+    // The last warp of the block closes the unit: it reserves the raster positions of the block's
+    // spikes (before the arrival, so that the entries of step n lie between the cumulative counts of
+    // the steps n - 2 and n + 1, as db_read_spikes assumes), arrives, then copies the list out.  The
+    // other warps are already on their way to the next unit; the list is reused two units later,
+    // behind the next unit's barrier.
+    if (c.warp == c.n_warps - 1u) {
+        const unsigned par = (unsigned)nA & 1u;
+        unsigned k = 0, st = 0;
+        unsigned long long base = 0;
+        if (c.lane == 0) {
+            k = bs->unit_spikes[par];
+            st = bs->staged[par];
+            bs->unit_spikes[par] = 0u;
+            bs->staged[par] = 0u;
+            if (k) {
+                if (st) base = atomicAdd(&ctl->spike_cursor, (unsigned long long)st);
+                atomicAdd(&ctl->unit_spikes[j & 3u], k);
+                if (p.n_regions == 1)
+                    atomicAdd(p.region_counts + (size_t)((nA / (unsigned long long)p.window_steps) % p.max_windows), k);
+            }
+            __threadfence();
+            atomicAdd(&ctl->bar[j & 3u], 1u);
         }
-        __threadfence();
-        atomicAdd(&ctl->bar[j & 3u], 1u);
+        if (kA) {
+            st = __shfl_sync(0xffffffffu, st, 0);
+            if (st) {
+                base = __shfl_sync(0xffffffffu, base, 0);
+                for (unsigned k2 = c.lane; k2 < st; k2 += 32u) {
+                    p.spike_ids[(base + k2) & p.spike_mask] = bs->spk[par][k2];
+                    p.spike_tag[(base + k2) & p.spike_mask] = (uint32_t)nA;
+                }
+            }
+        }
     }
     DB_TRACE_MARK(j, 3);
 }
@@ -773,7 +812,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
         s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
-    if (threadIdx.x == 0) { bs.unit_spikes = 0u; bs.heavy_n = 0u; bs.events = 0ull; }
+    if (threadIdx.x == 0) { bs.unit_spikes[0] = bs.unit_spikes[1] = 0u; bs.staged[0] = bs.staged[1] = 0u; bs.heavy_n = 0u; bs.events = 0ull; }
     __syncthreads();
 
     Stage sg;
