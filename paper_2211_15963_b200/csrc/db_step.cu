@@ -567,8 +567,10 @@ struct BlockShared {                 // small per-block scratch of the persisten
     unsigned staged[2];              // [unit & 1] how many of them wait in spk[] for their raster position
     unsigned long long events;       // synaptic events of this block's spikes (whole launch)
     int spk[2][kSpkCap];             // [unit & 1] spikes of the unit, copied to the raster after the unit's barrier
-    unsigned heavy_n;                // deferred heavy rows of the current unit
-    int heavy_row[kHeavyListCap];
+    unsigned done[2];                // [unit & 1] update warps that have finished the unit (networks without heavy rows)
+    unsigned grid_ok;                // units up to this one may start: the grid has closed everything they depend on
+    unsigned heavy_n[2];             // [unit & 1] deferred heavy rows of the unit
+    int heavy_row[2][kHeavyListCap];
 };
 
 // One 128-neuron task of one warp in unit (kB: B of step nB, kA: A of step nA).  next_off != 0:
@@ -670,10 +672,10 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
             if (!(bits & (1u << q))) continue;
             if (kHeavy && l > kInlineMax) {                      // leave it to the whole block (end of the unit)
                 unsigned at = 0;
-                if (lane == 0) at = atomicAdd(&bs->heavy_n, 1u);
+                if (lane == 0) at = atomicAdd(&bs->heavy_n[nlo & 1u], 1u);
                 at = __shfl_sync(0xffffffffu, at, 0);
                 if (at < (unsigned)kHeavyListCap) {
-                    if (lane == 0) bs->heavy_row[at] = (task * 32 + src) * 4 + q;
+                    if (lane == 0) bs->heavy_row[nlo & 1u][at] = (task * 32 + src) * 4 + q;
                     continue;
                 }
             }
@@ -705,26 +707,13 @@ struct RunCtx {                      // per-thread constants of the persistent k
 template <bool kHalf, bool kHeavy, bool kB, bool kA>
 __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, const RunCtx& c, const TypeSmem* s_tc,
                                          const uint32_t (*s_T)[kPoissonMax], BlockShared* bs, const Stage& sg,
-                                         const unsigned j, unsigned long long& sb, unsigned& fin, unsigned& bg_acc) {
-    Ctl* const ctl = p.ctl;
+                                         const unsigned j, unsigned& bg_acc) {
     const unsigned long long nA = c.n0 + j, nB = c.n0 + j - 1ull;
-    if (j >= 2u) {                     // every delivery of the units <= j - 2 must have landed
-        if (threadIdx.x == 0) {
-            bar_wait(ctl->bar, j - 2u, c.G);
-            if (c.keeper) {            // fold the spike count of unit j - 2 into the step log
-                const unsigned u = j - 2u;
-                sb += (unsigned long long)ld_cg_u32(&ctl->unit_spikes[u & 3u]);
-                ctl->unit_spikes[u & 3u] = 0u;
-                const unsigned long long np = c.n0 + u;
-                p.step_end[np & p.step_log_mask] = sb;
-                if ((np + 1) % (unsigned long long)p.window_steps == 0) {
-                    const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
-                    for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
-                }
-                fin = u + 1u;
-            }
-        }
-        __syncthreads();
+    if (j >= 2u) {                     // every delivery of the units <= j - 2 must have landed: the service warp
+        if (c.lane == 0)               // of the block polls the grid ahead of time and raises the flag
+            while (*reinterpret_cast<volatile unsigned*>(&bs->grid_ok) < j) __nanosleep(20);
+        __syncwarp();
+        __threadfence_block();
     }
     DB_TRACE_MARK(j, 0);
     if (c.task0 < c.last) {
@@ -737,13 +726,22 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
     }
     DB_TRACE_MARK(j, 1);
+    if (!kHeavy) {                     // no block barrier: the warp reports to the service warp and moves on
+        __syncwarp();
+        if (c.lane == 0) {
+            __threadfence_block();     // cta-scope release of this warp's pushes; the closer's gpu-scope fence is cumulative
+            atomicAdd(&bs->done[(unsigned)nA & 1u], 1u);
+        }
+        return;
+    }
     __syncthreads();
     if (kHeavy && kA) {                // rows too long for one warp: shared by the warps of the block
-        const unsigned nh = min(bs->heavy_n, (unsigned)kHeavyListCap);
+        const unsigned hp = (unsigned)nA & 1u;
+        const unsigned nh = min(bs->heavy_n[hp], (unsigned)kHeavyListCap);
         if (nh) {
             unsigned idx = 0;
             for (unsigned r = 0; r < nh; ++r) {
-                const int row = bs->heavy_row[r];
+                const int row = bs->heavy_row[hp][r];
                 const int64_t rb = __ldg(p.row_begin + row);
                 const int len = __ldg(p.row_len + row);
                 for (int off = 0; off < len; off += kChunk, ++idx)
@@ -752,20 +750,67 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
             }
             __syncthreads();
         }
-        if (threadIdx.x == 0) bs->heavy_n = 0u;
     }
     DB_TRACE_MARK(j, 2);
-    // The last warp of the block closes the unit: it reserves the raster positions of the block's
-    // spikes (before the arrival, so that the entries of step n lie between the cumulative counts of
-    // the steps n - 2 and n + 1, as db_read_spikes assumes), arrives, then copies the list out.  The
-    // other warps are already on their way to the next unit; the list is reused two units later,
-    // behind the next unit's barrier.
-    if (c.warp == c.n_warps - 1u) {
+    DB_TRACE_MARK(j, 3);
+}
+
+// The service warp of a block (its last warp; it owns no neurons).  Per unit j:
+//   1. ahead of time, while the update warps work on unit j: wait until the whole grid has closed unit
+//      j - 1 (acquire polls of the arrival counter), in block 0 fold that unit's spike count into the
+//      step log, and raise grid_ok to j + 1 -- the update warps find the flag up when they get there;
+//   2. join the end-of-unit barrier (and the second one of a unit with shared heavy rows);
+//   3. close the unit: reserve the raster positions of the block's spikes (before the arrival, so
+//      that the entries of step n lie between the cumulative counts of the steps n - 2 and n + 1, as
+//      db_read_spikes assumes), add the counters, fence, arrive, then copy the spike list out.  The
+//      list and the counters of a unit are reused two units later, behind the next unit's barrier.
+template <bool kHeavy>
+__device__ __noinline__ void service_warp(const SimDev& p, const RunCfg& cfg, const RunCtx& c, BlockShared* bs) {
+    Ctl* const ctl = p.ctl;
+    const bool keeper = (blockIdx.x == 0);
+    unsigned long long sb = ctl->spike_begin;       // raster bookkeeping (block 0)
+    unsigned fin = 0u;                              // units whose step the keeper has logged
+    auto log_unit = [&](const unsigned u) {
+        sb += (unsigned long long)ld_cg_u32(&ctl->unit_spikes[u & 3u]);
+        ctl->unit_spikes[u & 3u] = 0u;
+        const unsigned long long np = c.n0 + u;
+        p.step_end[np & p.step_log_mask] = sb;
+        if ((np + 1) % (unsigned long long)p.window_steps == 0) {
+            const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
+            for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
+        }
+    };
+    for (unsigned j = 0; j <= cfg.n_steps; ++j) {
+        const unsigned long long nA = c.n0 + j;
+        const bool kA = j < cfg.n_steps;
+        if (j >= 1u && kA) {                        // unit j + 1 needs the grid to have closed unit j - 1
+            if (c.lane == 0) {
+                bar_wait(ctl->bar, j - 1u, c.G);
+                if (keeper) { log_unit(j - 1u); fin = j; }
+                __threadfence_block();
+                *reinterpret_cast<volatile unsigned*>(&bs->grid_ok) = j + 1u;
+            }
+            __syncwarp();
+        }
         const unsigned par = (unsigned)nA & 1u;
-        unsigned k = 0, st = 0;
+        if (kHeavy) __syncthreads();                // every update warp has finished unit j
+        else {
+            if (c.lane == 0) {
+                while (*reinterpret_cast<volatile unsigned*>(&bs->done[par]) < c.n_warps) __nanosleep(20);
+                __threadfence_block();
+                bs->done[par] = 0u;                 // next used two units later, after this unit has been closed grid-wide
+            }
+            __syncwarp();
+        }
+        if (kHeavy && kA) {
+            const unsigned nh = min(bs->heavy_n[par], (unsigned)kHeavyListCap);
+            if (nh) __syncthreads();                // the update warps share the heavy rows, then meet again
+            if (c.lane == 0) bs->heavy_n[par] = 0u;
+        }
+        unsigned st = 0;
         unsigned long long base = 0;
         if (c.lane == 0) {
-            k = bs->unit_spikes[par];
+            const unsigned k = bs->unit_spikes[par];
             st = bs->staged[par];
             bs->unit_spikes[par] = 0u;
             bs->staged[par] = 0u;
@@ -778,18 +823,25 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
             __threadfence();
             atomicAdd(&ctl->bar[j & 3u], 1u);
         }
-        if (kA) {
-            st = __shfl_sync(0xffffffffu, st, 0);
-            if (st) {
-                base = __shfl_sync(0xffffffffu, base, 0);
-                for (unsigned k2 = c.lane; k2 < st; k2 += 32u) {
-                    p.spike_ids[(base + k2) & p.spike_mask] = bs->spk[par][k2];
-                    p.spike_tag[(base + k2) & p.spike_mask] = (uint32_t)nA;
-                }
+        st = __shfl_sync(0xffffffffu, st, 0);
+        if (st) {
+            base = __shfl_sync(0xffffffffu, base, 0);
+            for (unsigned k2 = c.lane; k2 < st; k2 += 32u) {
+                p.spike_ids[(base + k2) & p.spike_mask] = bs->spk[par][k2];
+                p.spike_tag[(base + k2) & p.spike_mask] = (uint32_t)nA;
             }
         }
     }
-    DB_TRACE_MARK(j, 3);
+    if (c.lane == 0) {
+        if (bs->events) atomicAdd(&ctl->events, bs->events);     // every emit of the block lies before the last barrier
+        if (keeper) {                               // close the launch: log the remaining steps, publish the position
+            if (cfg.n_steps >= 1u) bar_wait(ctl->bar, cfg.n_steps - 1u, c.G);   // the last unit that produces spikes
+            bar_wait(ctl->bar, cfg.n_steps, c.G);
+            for (unsigned u = fin; u < cfg.n_steps; ++u) log_unit(u);
+            ctl->spike_begin = sb;
+            ctl->step = c.n0 + cfg.n_steps;
+        }
+    }
 }
 
 template <bool kHalf, bool kHeavy>
@@ -799,7 +851,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     __shared__ uint32_t s_T[kMaxTypes][kPoissonMax];
     __shared__ BlockShared bs;
     RunCtx c;
-    c.lane = threadIdx.x & 31u; c.warp = threadIdx.x >> 5; c.n_warps = blockDim.x >> 5; c.G = gridDim.x;
+    c.lane = threadIdx.x & 31u; c.warp = threadIdx.x >> 5; c.n_warps = (blockDim.x >> 5) - 1u; c.G = gridDim.x;   // update warps; the last warp is the service warp
     for (int t = (int)threadIdx.x; t < kMaxTypes; t += (int)blockDim.x) {
         const TypeConst& tc = p.tc[t];
         TypeSmem r;
@@ -812,7 +864,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
         s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
-    if (threadIdx.x == 0) { bs.unit_spikes[0] = bs.unit_spikes[1] = 0u; bs.staged[0] = bs.staged[1] = 0u; bs.heavy_n = 0u; bs.events = 0ull; }
+    if (threadIdx.x == 0) { bs.unit_spikes[0] = bs.unit_spikes[1] = 0u; bs.staged[0] = bs.staged[1] = 0u; bs.heavy_n[0] = bs.heavy_n[1] = 0u; bs.grid_ok = 0u; bs.done[0] = bs.done[1] = 0u; bs.events = 0ull; }
     __syncthreads();
 
     Stage sg;
@@ -820,9 +872,6 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * kPlaneStride + threadIdx.x * 8u;
 
     c.n0 = p.ctl->step;                               // nobody writes it before the end of the launch
-    unsigned long long sb = p.ctl->spike_begin;       // raster bookkeeping: block 0, thread 0
-    unsigned fin = 0u;                                // units whose step the keeper has logged
-    c.keeper = (blockIdx.x == 0 && threadIdx.x == 0);
     const int first = (int)blockIdx.x * cfg.tasks_per_block;
     c.last = min(first + cfg.tasks_per_block, cfg.n_tasks);
     c.task0 = first + (int)c.warp;                    // the warp's first task of every unit
@@ -830,31 +879,14 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     c.task_stride = (int)c.n_warps * 128;             // neurons between consecutive tasks of a warp
     unsigned bg_acc = 0u;
     if (cfg.n_steps == 0) return;
+    if (c.warp == c.n_warps) { service_warp<kHeavy>(p, cfg, c, &bs); return; }
 
     if (c.task0 < c.last) { request_state(p, sg, c.i00); cp_async_commit(); }
-    run_unit<kHalf, kHeavy, false, true>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, sb, fin, bg_acc);
+    run_unit<kHalf, kHeavy, false, true>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
     for (unsigned j = 1; j < cfg.n_steps; ++j)
-        run_unit<kHalf, kHeavy, true, true>(p, cfg, c, s_tc, s_T, &bs, sg, j, sb, fin, bg_acc);
-    run_unit<kHalf, kHeavy, true, false>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, sb, fin, bg_acc);
+        run_unit<kHalf, kHeavy, true, true>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
+    run_unit<kHalf, kHeavy, true, false>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
 
-    // close the launch: log the remaining steps and publish the position
-    if (c.keeper) {
-        if (cfg.n_steps >= 1u) bar_wait(p.ctl->bar, cfg.n_steps - 1u, c.G);   // the last unit that produces spikes
-        bar_wait(p.ctl->bar, cfg.n_steps, c.G);
-        for (unsigned u = fin; u < cfg.n_steps; ++u) {
-            sb += (unsigned long long)ld_cg_u32(&p.ctl->unit_spikes[u & 3u]);
-            p.ctl->unit_spikes[u & 3u] = 0u;
-            const unsigned long long np = c.n0 + u;
-            p.step_end[np & p.step_log_mask] = sb;
-            if ((np + 1) % (unsigned long long)p.window_steps == 0) {
-                const unsigned w = (unsigned)(((np + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
-                for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
-            }
-        }
-        p.ctl->spike_begin = sb;
-        p.ctl->step = c.n0 + cfg.n_steps;
-    }
-    if (threadIdx.x == 0 && bs.events) atomicAdd(&p.ctl->events, bs.events);   // every emit of the block lies before the last barrier
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (c.lane == 0 && bg_warp)
         atomicAdd(p.bg_parts + ((blockIdx.x * c.n_warps + c.warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
@@ -901,13 +933,13 @@ cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
 // chosen so that the warps of a block take the same number of tasks (no ragged last iteration).
 void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg) {
     const int n_tasks = p.Npad / 128;
-    const int max_warps = kRunThreads / 32;
+    const int max_warps = kRunThreads / 32 - 1;        // update warps; one more warp per block is the service warp
     const int tpb = (n_tasks + n_sm - 1) / n_sm;
     const int iters = (tpb + max_warps - 1) / max_warps;
     const int warps = (tpb + iters - 1) / iters;
     cfg->n_tasks = n_tasks; cfg->tasks_per_block = tpb; cfg->iters = iters;
     *grid = (n_tasks + tpb - 1) / tpb;
-    *threads = warps * 32;
+    *threads = (warps + 1) * 32;
 }
 
 static const void* run_fn(const SimDev& p, bool heavy) {
