@@ -168,6 +168,10 @@ def run_reference(args):
 
 
 def _config_dict(args, n_neurons, sim_steps):
+    if args.config != 1:           # configs 2-4 are parity-test cases; `--config` times them for profiles/ only
+        return {"workload": f"configs[{args.config}] (DESIGN.md section 5): {n_neurons} LIF neurons, dt 0.1 ms",
+                "n_neurons": n_neurons, "sim_steps_per_bench_step": sim_steps, "dt_ms": 0.1,
+                "l2": "no flush: device footprint far exceeds the 126 MB L2"}
     return {"workload": f"configs[1]: {n_neurons} LIF neurons, in-degree 100, dt 0.1 ms, ~{args.rate} Hz",
             "n_neurons": n_neurons, "in_degree": 100, "rate_hz_target": args.rate,
             "sim_steps_per_bench_step": sim_steps, "dt_ms": 0.1,
@@ -192,7 +196,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     db.load()
 
-    cfg = db_inputs.config(1, rate_hz=args.rate, scale=args.scale)
+    cfg = db_inputs.config(args.config, rate_hz=(args.rate if args.config == 1 else None), scale=args.scale)
     N = cfg["net"]["N"]
     n_sim = args.sim_steps
     mode = {"auto": db.EXEC_AUTO, "kernels": db.EXEC_KERNELS, "persistent": db.EXEC_PERSISTENT}[args.exec_mode]
@@ -257,7 +261,9 @@ def run_ours(args):
         gbs = (upd_bytes + del_bytes) / dur_s / 1e9
         roofline = {
             "bound": "hbm", "kernel": "k_run (persistent: update + compaction + delivery + region counts, fused)",
-            "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": NCU_TRAFFIC["k_run_per_sim_step"] * n_sim,
+            "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+            "traffic": (NCU_TRAFFIC["k_run_per_sim_step"] * n_sim
+                        if (args.config == 1 and args.rate == 7 and args.scale == 1.0) else None),
             "peak_source": peak_src, "bytes_per_launch": upd_bytes + del_bytes,
             "bytes_per_launch_update": upd_bytes, "bytes_per_launch_delivery": del_bytes,
             "sim_steps_per_launch": n_sim, "us_per_launch": dur_s * 1e6, "us_per_sim_step": dur_s * 1e6 / n_sim,
@@ -287,8 +293,19 @@ def run_ours(args):
         }
         if roofline is None:
             roofline = dict(two, note=note)
+            if two["deliver"]["share_of_step"] > two["share_of_step"]:      # delivery-bound workloads (configs 3, 4)
+                dlv = two["deliver"]
+                roofline = {"bound": "hbm", "kernel": "k_deliver", "achieved": dlv["achieved"], "peak": peak,
+                            "unit": "GB/s", "frac": dlv["frac"], "traffic": None, "peak_source": peak_src,
+                            "bytes_per_launch": ev_bytes * dlv["events_per_launch"], "us_per_launch": dlv["us_per_launch"],
+                            "share_of_step": dlv["share_of_step"], "update": {k: v for k, v in two.items() if k != "deliver"},
+                            "note": "random 4-byte reductions into a ring far larger than L2: the hardware moves whole "
+                                    "sectors, DRAM traffic per event is several times the 17 (15) algorithmic bytes"}
         else:
             roofline["two_kernel_mode"] = two
+    if roofline is None:
+        roofline = {"bound": "hbm", "kernel": "k_update + k_deliver", "achieved": None, "peak": peak, "unit": "GB/s",
+                    "frac": None, "traffic": None, "note": "run with --profile-steps > 0 for per-kernel times"}
 
     # ---------------- end to end through the C ABI with host buffers --------------------------------
     V_h = torch.empty(N, dtype=torch.float32).pin_memory()
@@ -380,6 +397,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--rate", type=int, default=7, choices=[7, 15, 30])
+    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4],
+                    help="BASELINE.json configs[i]; 1 is the bench workload, the others are timed for profiles/ only")
     ap.add_argument("--sim-steps", type=int, default=1000, help="simulation time steps per bench step")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink configs[1] (debugging only)")
     ap.add_argument("--exec-mode", choices=["auto", "kernels", "persistent"], default="auto")

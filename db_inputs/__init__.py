@@ -23,6 +23,10 @@ RECEPTORS = ("AMPA", "NMDA", "GABA_A", "GABA_B")
 # config 0; mean-field is size independent at
 # fixed in-degree, so the same values serve configs 1, 2, 4.
 BG_WEIGHT_FOR_RATE = {7: 0.0072, 15: 0.0110, 30: 0.0240}
+# The larger in-degrees of configs 2-4 (G scaled by 100/K, R20) shrink the input variance, so the
+# same drive gives a lower rate there: effective drive G_AMPA * w_bg tuned per config by bisection
+# on full-size runs (rate over 0.1-0.2 s after a 0.15-0.3 s warm-up).
+BG_DRIVE_FOR_CONFIG = {(2, 7): 0.00773, (3, 15): 0.0171, (4, 30): 0.0378}
 
 
 def type_params(bg_weight: float = BG_WEIGHT_FOR_RATE[7], bg_rate_hz: float = 1000.0,
@@ -38,11 +42,13 @@ def type_params(bg_weight: float = BG_WEIGHT_FOR_RATE[7], bg_rate_hz: float = 10
 
 
 def sim_params(dt_ms: float = 0.1, S: int = 22, D: int = 32, window_steps: int = 10,
-               rate_hz: int = 7, g_scale: float = 1.0, types: list | None = None) -> dict:
+               rate_hz: int = 7, g_scale: float = 1.0, types: list | None = None,
+               bg_drive: float | None = None) -> dict:
     if types is None:
         # G scales with 100/K (R20); the background enters through G_AMPA too, so its
         # weight is divided by the same factor to keep the drive fixed.
-        t = type_params(BG_WEIGHT_FOR_RATE[rate_hz] / g_scale, g_scale=g_scale)
+        drive = BG_WEIGHT_FOR_RATE[rate_hz] if bg_drive is None else bg_drive
+        t = type_params(drive / g_scale, g_scale=g_scale)
         types = [t, copy.deepcopy(t)]            # exc and inh share constants (R13)
     return dict(dt_ms=dt_ms, S=S, D=D, window_steps=window_steps, types=types)
 
@@ -77,16 +83,19 @@ def config(idx: int, rate_hz: int | None = None, scale: float = 1.0) -> dict:
                    intra_frac=0.8)
         # 200 inputs per neuron: hold the mean input of K=100 fixed (R20)
         return dict(name="config2", net=net,
-                    sim=sim_params(rate_hz=rate_hz or 7, D=256, g_scale=0.5), steps=10_000)
+                    sim=sim_params(rate_hz=rate_hz or 7, D=256, g_scale=0.5,
+                                   bg_drive=BG_DRIVE_FOR_CONFIG.get((2, rate_hz or 7))), steps=10_000)
     if idx == 3:
         net = _net(N=int(10_000_000 * scale), n_regions=200, region_size_sigma=0.7, K=1000,
                    intra_frac=0.8, weight_fp16=1)
         return dict(name="config3", net=net,
-                    sim=sim_params(rate_hz=rate_hz or 15, D=256, g_scale=0.1), steps=1000)
+                    sim=sim_params(rate_hz=rate_hz or 15, D=256, g_scale=0.1,
+                                   bg_drive=BG_DRIVE_FOR_CONFIG.get((3, rate_hz or 15))), steps=1000)
     if idx == 4:
         net = _net(N=int(2_000_000 * scale), mode=1, K=0)
         return dict(name="config4", net=net,
-                    sim=sim_params(rate_hz=rate_hz or 30, g_scale=0.2), steps=10_000)
+                    sim=sim_params(rate_hz=rate_hz or 30, g_scale=0.2,
+                                   bg_drive=BG_DRIVE_FOR_CONFIG.get((4, rate_hz or 30))), steps=10_000)
     raise ValueError(idx)
 
 

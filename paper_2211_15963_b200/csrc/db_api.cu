@@ -223,7 +223,11 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     bool fits = false;
     CK(persistent_fits(d, sim->heavy, sim->n_sm, &fits));
     int mode = sim->params.exec_mode;
-    if (mode == DB_EXEC_AUTO) mode = (coop && fits) ? DB_EXEC_PERSISTENT : DB_EXEC_KERNELS;
+    // AUTO: the persistent kernel wins while the update dominates the step; with long rows (mean
+    // out-degree >= 400: configs 3 and 4) the step is delivery-bound and the two-kernel mode, where every
+    // warp of the grid pushes rows, is faster (measured: profiles/)
+    const bool delivery_bound = sim->heavy || (sim->E >= 400 * (int64_t)d.N);
+    if (mode == DB_EXEC_AUTO) mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : DB_EXEC_KERNELS;
     if (mode == DB_EXEC_PERSISTENT && (!coop || !fits))
         return fail(sim, DB_ECUDA, "cooperative launch not available for the persistent mode");
     sim->exec_mode = mode;

@@ -63,7 +63,7 @@ def test_config1_full_size_closed_loop(db, oracle_mod):
     steps = 60
     s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, dyn_seed=db_inputs.DYN_SEED,
                          raster_capacity=1 << 25)
-    assert s.db_get_counters()["exec_mode"] == db.EXEC_PERSISTENT          # what bench.py times
+    assert s.db_get_counters()["exec_mode"] == db.EXEC_PERSISTENT          # what AUTO picks here and bench.py times
     net = oracle_mod.generate(cfg["net"], db_inputs.GEN_SEED)        # the oracle's own network (about 45 s of CPU)
     got = s.db_export_csr()
     for key in ("N", "E", "n_regions"):
@@ -159,7 +159,9 @@ def test_region_configs_full_size_replay_and_properties(db, oracle_mod, idx, ste
     cfg = db_inputs.config(idx)
     region_start = None
     keep = {}
-    for mode in (db.EXEC_AUTO, db.EXEC_KERNELS):
+    for mode in (db.EXEC_AUTO, "other"):
+        if mode == "other":                     # the execution mode AUTO did not pick: an independent schedule
+            mode = db.EXEC_KERNELS if keep["mode"] == db.EXEC_PERSISTENT else db.EXEC_PERSISTENT
         s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, dyn_seed=db_inputs.DYN_SEED,
                              exec_mode=mode, raster_capacity=1 << 26)
         if region_start is None:
@@ -185,7 +187,9 @@ def test_config4_full_size_rows_and_properties(db, oracle_mod):
     steps = 150
     N = cfg["net"]["N"]
     keep = {}
-    for mode in (db.EXEC_AUTO, db.EXEC_KERNELS):
+    for mode in (db.EXEC_AUTO, "other"):
+        if mode == "other":
+            mode = db.EXEC_KERNELS if keep["mode"] == db.EXEC_PERSISTENT else db.EXEC_PERSISTENT
         s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, dyn_seed=db_inputs.DYN_SEED,
                              exec_mode=mode, raster_capacity=1 << 26)
         if mode == db.EXEC_AUTO:
@@ -200,7 +204,8 @@ def test_config4_full_size_rows_and_properties(db, oracle_mod):
         st, ids = _raster_props(s, db, steps, 1, np.array([0, N]), cfg["sim"]["window_steps"])
         assert len(ids) > 10 * steps
         if mode == db.EXEC_AUTO:
-            keep = dict(st=st, ids=ids, V=s.db_read_state(db.FIELD_V), ring0=s.db_read_state(db.FIELD_RING, 0, 4096))
+            keep = dict(st=st, ids=ids, V=s.db_read_state(db.FIELD_V), ring0=s.db_read_state(db.FIELD_RING, 0, 4096),
+                        mode=s.db_get_counters()["exec_mode"])
         else:
             assert np.array_equal(st, keep["st"]) and np.array_equal(ids, keep["ids"])
             assert np.array_equal(s.db_read_state(db.FIELD_V), keep["V"])
