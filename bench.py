@@ -179,6 +179,18 @@ def _config_dict(args, n_neurons, sim_steps):
                   "runs back to back as in production"}
 
 
+def reduce_over_ranks(dist, device, ms: float, sums: list):
+    """Whole-job figures from per-rank ones: MAX of the device time over the ranks, SUM of the counters
+    (replicas only).  `dist` is torch.distributed or None (single process)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    tot = torch.tensor([float(x) for x in sums], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(x) for x in tot.tolist()]
+
+
 # --------------------------------------------------------------------------------------------- CUDA arm
 def run_ours(args):
     import torch
@@ -235,13 +247,7 @@ def run_ours(args):
     spikes = c1["spikes"] - c0["spikes"]
     launches = c1["launches"] - c0["launches"]
     exec_used = c1["exec_mode"]
-    t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
-    tot = torch.tensor([events, spikes, launches], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_max = float(t.item())
-    events_all, spikes_all, launches_all = [float(x) for x in tot.tolist()]
+    ms_max, (events_all, spikes_all, launches_all) = reduce_over_ranks(dist, f"cuda:{local}", ms, [events, spikes, launches])
     secs = ms_max * 1e-3
     bio_s = args.steps * n_sim * cfg["sim"]["dt_ms"] * 1e-3
     value = events_all / secs
@@ -345,15 +351,11 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     ce1 = sim.db_get_counters()
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local}")
-    ee = torch.tensor([float(ce1["events"] - ce0["events"])], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        dist.all_reduce(ee, op=dist.ReduceOp.SUM)
-    e2e = {"value": float(ee.item()) / float(te.item()), "unit": UNIT,
+    e2e_max, (e2e_events,) = reduce_over_ranks(dist, f"cuda:{local}", e2e_s, [ce1["events"] - ce0["events"]])
+    e2e = {"value": e2e_events / e2e_max, "unit": UNIT,
            "h2d_bytes_per_step": int(N * (4 + 16 + 4)),
            "d2h_bytes_per_step": int(N * 4 + (n_sp // max(args.e2e_steps, 1)) * 12 + rate_bytes),
-           "steps": args.e2e_steps, "ms_per_step": 1e3 * float(te.item()) / args.e2e_steps,
+           "steps": args.e2e_steps, "ms_per_step": 1e3 * e2e_max / args.e2e_steps,
            "what": "db_write_state(V, g[4], ref) from pinned host + db_step + db_read_spikes + db_region_rates + "
                    "db_read_state(V) to pinned host, wall clock"}
 

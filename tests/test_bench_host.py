@@ -1,0 +1,73 @@
+"""Host-side logic of bench.py that needs no GPU: the reference arm (the oracle timed on the host
+cores), its behaviour under torchrun (rank 0 alone works and prints), and the whole-job reduction
+over ranks (MAX of the device time, SUM of the counters) on a world_size-2 gloo group."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(args, env=None, timeout=300):
+    e = dict(os.environ)
+    e.update(env or {})
+    return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], cwd=ROOT, env=e,
+                          capture_output=True, text=True, timeout=timeout)
+
+
+def test_reference_arm_prints_the_contract_line():
+    r = _run(["--impl", "reference", "--steps", "1", "--warmup", "0", "--ref-scale", "0.01",
+              "--ref-warm-steps", "50", "--ref-sim-steps", "20"])
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["metric"] == "synaptic_events_per_s" and line["unit"] == "events/s"
+    assert line["higher_is_better"] is True and line["value"] > 0 and line["vs_baseline"] is None
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] == 1
+    assert line["cpu_baseline"]["value"] == line["value"]
+    assert line["e2e"] == {"value": line["value"], "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert line["config"]["workload"].startswith("configs[1]")
+
+
+def test_reference_arm_other_ranks_exit_silently():
+    r = _run(["--impl", "reference", "--gpus", "2"], env={"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"})
+    assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%%s" %% os.environ["PORT"],
+                        rank=int(os.environ["RANK"]), world_size=2)
+rank = dist.get_rank()
+ms, sums = bench.reduce_over_ranks(dist, "cpu", 10.0 + 5.0 * rank, [100 * (rank + 1), 7, rank])
+print(json.dumps({"rank": rank, "ms": ms, "sums": sums}))
+dist.barrier()
+dist.destroy_process_group()
+""" % ROOT
+
+
+def test_whole_job_reduction_over_two_ranks_gloo():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    procs = [subprocess.Popen([sys.executable, "-c", _WORKER], cwd=ROOT, text=True, stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, env=dict(os.environ, RANK=str(r), PORT=str(port)))
+             for r in range(2)]
+    outs = [p.communicate(timeout=300) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e
+    for o, _ in outs:
+        d = json.loads(o.strip().splitlines()[-1])
+        assert d["ms"] == 15.0                       # MAX over ranks
+        assert d["sums"] == [300.0, 14.0, 1.0]       # SUM over ranks
+
+
+def test_single_process_reduction_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    ms, sums = bench.reduce_over_ranks(None, "cpu", 3.5, [1, 2])
+    assert ms == 3.5 and sums == [1.0, 2.0]
