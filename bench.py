@@ -14,7 +14,7 @@ Prints ONE JSON line (rank 0):
                 state from pinned host memory (db_write_state), steps, and reads the raster, the
                 region rates and V back to the host (db_read_spikes / db_region_rates / db_read_state)
   roofline      the dominant kernel of the timed region (k_run in persistent mode: one launch = all the time
-                steps of a db_step call; k_update in two-kernel mode) against the measured HBM copy peak
+                steps of a db_step call; k_update_stream or k_deliver in two-kernel mode) against the measured HBM copy peak
   cpu_baseline  the oracle (oracle/, as it stands) on the host cores, on a bounded sample
 ``--impl reference`` times the oracle instead (same metric, unit and config).
 
@@ -288,8 +288,8 @@ def run_ours(args):
         upd_gbs = UPDATE_BYTES_PER_NEURON_STEP * N / upd_s / 1e9
         del_gbs = ev_bytes * prof["events"] / prof["steps"] / del_s / 1e9
         two = {
-            "bound": "hbm", "kernel": "k_update", "achieved": upd_gbs, "peak": peak, "unit": "GB/s",
-            "frac": upd_gbs / peak, "traffic": NCU_TRAFFIC.get("k_update"), "peak_source": peak_src,
+            "bound": "hbm", "kernel": "k_update_stream", "achieved": upd_gbs, "peak": peak, "unit": "GB/s",
+            "frac": upd_gbs / peak, "traffic": None, "peak_source": peak_src,
             "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
             "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
             "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
@@ -310,7 +310,7 @@ def run_ours(args):
         else:
             roofline["two_kernel_mode"] = two
     if roofline is None:
-        roofline = {"bound": "hbm", "kernel": "k_update + k_deliver", "achieved": None, "peak": peak, "unit": "GB/s",
+        roofline = {"bound": "hbm", "kernel": "k_update_stream + k_deliver", "achieved": None, "peak": peak, "unit": "GB/s",
                     "frac": None, "traffic": None, "note": "run with --profile-steps > 0 for per-kernel times"}
 
     # ---------------- end to end through the C ABI with host buffers --------------------------------

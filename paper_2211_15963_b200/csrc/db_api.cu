@@ -37,6 +37,7 @@ struct db_sim {
     int exec_mode = DB_EXEC_KERNELS;
     int deliver_grid = 0;
     bool heavy = false;             // some row is longer than kInlineMax
+    int update_sm = 0;              // two-kernel mode: SM count the update kernel is shaped for
     cudaGraphExec_t graph_exec = nullptr;
     int graph_steps = 0;
     uint64_t launches = 0;
@@ -218,6 +219,7 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     sim->heavy = heavy_chunks > 0;
     CK(launch_init_state(d, sim->ntype_dev, sim->stream));
     sim->deliver_grid = sim->n_sm * 4;
+    sim->update_sm = sim->n_sm;
     int coop = 0;
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device));
     bool fits = false;
@@ -242,7 +244,7 @@ int32_t build_graph(db_sim* sim) {
     CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
     CK(cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
     for (int s = 0; s < steps; ++s) {
-        launch_update(sim->dev, cap);
+        launch_update(sim->dev, sim->update_sm, cap);
         launch_deliver(sim->dev, sim->deliver_grid, cap);
     }
     cudaError_t e = cudaStreamEndCapture(cap, &graph);
@@ -412,7 +414,7 @@ int32_t db_step(db_sim* sim, uint32_t n_steps) {
         sim->launches += 2ull * (uint64_t)sim->graph_steps;
     }
     for (; left; --left) {
-        CK(launch_update(sim->dev, sim->stream));
+        CK(launch_update(sim->dev, sim->update_sm, sim->stream));
         CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
         sim->launches += 2;
     }
@@ -435,7 +437,7 @@ int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
         const uint32_t b = std::min(left, batch);
         CK(cudaEventRecord(sim->prof_events[0], sim->stream));
         for (uint32_t s = 0; s < b; ++s) {
-            CK(launch_update(sim->dev, sim->stream));
+            CK(launch_update(sim->dev, sim->update_sm, sim->stream));
             CK(cudaEventRecord(sim->prof_events[2 * s + 1], sim->stream));
             CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
             CK(cudaEventRecord(sim->prof_events[2 * s + 2], sim->stream));

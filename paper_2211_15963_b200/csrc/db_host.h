@@ -11,7 +11,7 @@ namespace dbk {
 
 // ---- db_step.cu ------------------------------------------------------------
 cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
-cudaError_t launch_update(const SimDev& p, cudaStream_t st);
+cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st);
 cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);

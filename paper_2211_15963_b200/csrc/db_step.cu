@@ -58,154 +58,6 @@ __device__ __forceinline__ int region_of(const SimDev& p, int i) {
 }
 
 // ---------------------------------------------------------------------------
-// One neuron, one step.  Returns 1 if it spikes.  `a` holds the four consumed
-// ring cells (AMPA already including the background), v / g / ref are updated
-// in place.
-// ---------------------------------------------------------------------------
-__device__ __forceinline__ int neuron_step(const TypeConst& c, float scale, const int a[4],
-                                           float& v, float g[4], int& ref) {
-    float x[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) x[u] = __fmul_rn(__int2float_rn(a[u]), scale);
-    const float t0 = __fmul_rn(__fmul_rn(c.G[0], g[0]), __fsub_rn(c.E[0], v));
-    const float t1 = __fmul_rn(__fmul_rn(c.G[1], g[1]), __fsub_rn(c.E[1], v));
-    const float t2 = __fmul_rn(__fmul_rn(c.G[2], g[2]), __fsub_rn(c.E[2], v));
-    const float t3 = __fmul_rn(__fmul_rn(c.G[3], g[3]), __fsub_rn(c.E[3], v));
-    const float I = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(t0, t1), t2), t3), c.Iext);
-    const float leak = __fmul_rn(c.neg_gL, __fsub_rn(v, c.VL));
-    float vn = __fadd_rn(v, __fmul_rn(c.kappa, __fadd_rn(leak, I)));
-#pragma unroll
-    for (int u = 0; u < 4; ++u) g[u] = __fadd_rn(__fmul_rn(g[u], c.alpha[u]), x[u]);
-    int spike = 0;
-    if (ref > 0) { vn = c.Vreset; ref -= 1; }
-    else if (vn >= c.Vth) { spike = 1; vn = c.Vreset; ref = c.R; }
-    v = vn;
-    return spike;
-}
-
-__device__ __forceinline__ int poisson_count(const TypeConst& c, uint32_t u) {
-    int k = 0;
-    while (k < c.M && u >= c.T[k]) ++k;           // thresholds increase: same as counting all u >= T_m
-    return k;
-}
-
-// ---------------------------------------------------------------------------
-// a1 + a2 + a4 for the four neurons i0..i0+3 owned by this thread.  Called by
-// whole warps (Npad is a multiple of 128).
-// ---------------------------------------------------------------------------
-__device__ __forceinline__ void update_group(const SimDev& p, const unsigned long long n,
-                                             const unsigned long long spike_begin, const int grp) {
-    const int i0 = grp * 4;
-    const size_t Np = (size_t)p.Npad;
-    int32_t* slot = p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
-
-    // all loads first: ten independent 128-bit (and one 64-bit) requests in flight
-    int4 ar[4];
-    float4 gr[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) ar[u] = ld_stream_i4(slot + u * Np);
-    const float4 v4 = ld_stream_f4(p.V + i0);
-#pragma unroll
-    for (int u = 0; u < 4; ++u) gr[u] = ld_stream_f4(p.g + u * Np + i0);
-    const ushort4 rt4 = *reinterpret_cast<const ushort4*>(p.rt + i0);
-
-    // one Philox block serves the four neurons (word q -> neuron i0 + q)
-    const uint4 rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24,
-                                               (uint32_t)n, (uint32_t)(n >> 32)),
-                                    p.seed_lo, p.seed_hi);
-
-    float v[4] = {v4.x, v4.y, v4.z, v4.w};
-    int a[4][4] = {{ar[0].x, ar[1].x, ar[2].x, ar[3].x}, {ar[0].y, ar[1].y, ar[2].y, ar[3].y},
-                   {ar[0].z, ar[1].z, ar[2].z, ar[3].z}, {ar[0].w, ar[1].w, ar[2].w, ar[3].w}};
-    float g[4][4] = {{gr[0].x, gr[1].x, gr[2].x, gr[3].x}, {gr[0].y, gr[1].y, gr[2].y, gr[3].y},
-                     {gr[0].z, gr[1].z, gr[2].z, gr[3].z}, {gr[0].w, gr[1].w, gr[2].w, gr[3].w}};
-    unsigned short rt[4] = {rt4.x, rt4.y, rt4.z, rt4.w};
-    const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
-
-    unsigned spike_bits = 0;
-    unsigned bg = 0, ovf = 0, rt_changed = 0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int tp = rt[q] >> 12;
-        const TypeConst& c = p.tc[tp];
-        const bool valid = (i0 + q) < p.N;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) ovf |= (unsigned)(a[q][u] > (1 << 30) || a[q][u] < -(1 << 30));
-        const int k = valid ? poisson_count(c, rw[q]) : 0;
-        bg += (unsigned)k;
-        a[q][0] = (int)((unsigned)a[q][0] + (unsigned)k * (unsigned)c.wq_bg);
-        int ref = rt[q] & kRefMask;
-        const int ref_in = ref;
-        const int s = neuron_step(c, p.scale, a[q], v[q], g[q], ref);
-        rt_changed |= (unsigned)(ref != ref_in);
-        rt[q] = (unsigned short)((tp << 12) | ref);
-        if (s && valid) spike_bits |= 1u << q;
-    }
-
-    // stores: state always, consumed ring cells and rt only where something changed
-    st_stream_f4(p.V + i0, make_float4(v[0], v[1], v[2], v[3]));
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-        st_stream_f4(p.g + u * Np + i0, make_float4(g[0][u], g[1][u], g[2][u], g[3][u]));
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-        if ((ar[u].x | ar[u].y | ar[u].z | ar[u].w) != 0) st_stream_i4(slot + u * Np, make_int4(0, 0, 0, 0));
-    if (rt_changed) *reinterpret_cast<ushort4*>(p.rt + i0) = make_ushort4(rt[0], rt[1], rt[2], rt[3]);
-    if (ovf) p.ctl->overflow = 1u;
-
-    // background-event counter: one reduction per warp, spread over many cells
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg);
-    if (lane == 0 && bg_warp)
-        atomicAdd(p.bg_parts + ((unsigned)(grp >> 5) & (kBgParts - 1)), (unsigned long long)bg_warp);
-
-    // ---- a2: compaction.  Spikes are rare (rate * dt per neuron-step): whole warps skip this.
-    const unsigned any = __ballot_sync(0xffffffffu, spike_bits != 0);
-    if (any == 0) return;
-    unsigned my_spk = __popc(spike_bits), my_work = 0, my_events = 0;
-    int len[4] = {0, 0, 0, 0};
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-        if (spike_bits & (1u << q)) {
-            len[q] = __ldg(p.row_len + i0 + q);
-            my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
-            my_events += (unsigned)len[q];
-        }
-    // inclusive warp scan of (spikes, work items) packed in one 64-bit word
-    unsigned long long pk = ((unsigned long long)my_spk << 32) | my_work;
-    unsigned long long inc = pk;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        unsigned long long o = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= (unsigned)d) inc += o;
-    }
-    const unsigned long long tot = __shfl_sync(0xffffffffu, inc, 31);
-    const unsigned ev_warp = __reduce_add_sync(0xffffffffu, my_events);
-    unsigned long long base = 0;
-    if (lane == 0) {
-        base = atomicAdd(&p.ctl->step_counts[n & 1ull], tot);
-        atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
-    }
-    base = __shfl_sync(0xffffffffu, base, 0);
-    const unsigned long long mine = base + inc - pk;          // exclusive offsets
-    unsigned long long spk_pos = spike_begin + (mine >> 32);
-    unsigned work_pos = (unsigned)mine;
-    const unsigned win = (unsigned)((n / (unsigned long long)p.window_steps) % p.max_windows);
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-        if (spike_bits & (1u << q)) {
-            const int i = i0 + q;
-            p.spike_ids[spk_pos & p.spike_mask] = i;
-            p.spike_tag[spk_pos & p.spike_mask] = (uint32_t)n;
-            ++spk_pos;
-            const int nch = (len[q] + kChunk - 1) / kChunk;
-            for (int c = 0; c < nch; ++c) p.work[work_pos++] = make_int2(i, c);
-            const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
-            atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
-        }
-}
-
-// ---------------------------------------------------------------------------
 // a3: one work item = up to kChunk consecutive synapses of one spiking neuron's
 // row, handled by one warp; each lane takes 4 synapses per 128-bit load.
 // ---------------------------------------------------------------------------
@@ -280,14 +132,6 @@ __device__ __forceinline__ void finalize_step(const SimDev& p, const unsigned lo
 // ===========================================================================
 // Mode DB_EXEC_KERNELS: two kernels per step.
 // ===========================================================================
-__global__ void __launch_bounds__(256) k_update(const __grid_constant__ SimDev p) {
-    const int grp = blockIdx.x * blockDim.x + threadIdx.x;
-    if (grp * 4 >= p.Npad) return;
-    const unsigned long long n = p.ctl->step;
-    const unsigned long long sb = p.ctl->spike_begin;
-    update_group(p, n, sb, grp);
-}
-
 template <bool kHalf>
 __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev p) {
     const unsigned long long n = p.ctl->step;
@@ -474,7 +318,7 @@ __device__ __forceinline__ void request_ring(const SimDev& p, const Stage& sg, c
 // is requested (ring planes only if kB).  tp0..tp3 are the neuron types; the caller passes the
 // same variable four times when they agree, which lets the constant loads (broadcast LDS.128)
 // be shared.  Operation order: DESIGN.md "Arithmetic contract".
-template <bool kB, bool kA>
+template <bool kB, bool kA, bool kClassic = false>
 __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem* s_tc,
                                                  const uint32_t (*s_T)[kPoissonMax], const Stage& sg,
                                                  const int tp0, const int tp1, const int tp2, const int tp3,
@@ -498,6 +342,8 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
             cp_async16(sg.sbase + (unsigned)(5 + u) * kPlaneStride, p.g + u * Np + i0 + next_off);
         }
         float gn[4] = {__uint_as_float(gb.x), __uint_as_float(gb.y), __uint_as_float(gb.z), __uint_as_float(gb.w)};
+        // kClassic (whole step n in one pass, two-kernel mode): the membrane step sees g(n), the value loaded
+        const float gc[4] = {gn[0], gn[1], gn[2], gn[3]};
         if (kB) {
             int a[4] = {(int)ab.x, (int)ab.y, (int)ab.z, (int)ab.w};
             if ((a[0] | a[1] | a[2] | a[3]) != 0) {  // consumed: zero the cells again, check the overflow bound
@@ -529,7 +375,7 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const float4 r = s_tc[tp[q]].rec[u];
-                const float t = __fmul_rn(__fmul_rn(r.x, gn[q]), __fsub_rn(r.y, v[q]));
+                const float t = __fmul_rn(__fmul_rn(r.x, kClassic ? gc[q] : gn[q]), __fsub_rn(r.y, v[q]));
                 I[q] = (u == 0) ? t : __fadd_rn(I[q], t);
             }
         }
@@ -892,6 +738,125 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
         atomicAdd(p.bg_parts + ((blockIdx.x * c.n_warps + c.warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
 }
 
+// ===========================================================================
+// Mode DB_EXEC_KERNELS, update kernel: the neuron update of ONE step (a1 + a2 + a4) with the machinery
+// of the persistent kernel -- one block per SM, fixed contiguous task ranges, every plane staged
+// through shared memory with cp.async and requested one task ahead -- instead of one thread block
+// per 1024 neurons: no tail wave, deeper prefetch.  Whole step n in one pass (classic order: the
+// membrane step sees g(n), then slot n is consumed into g(n+1)); spikes go to the global work list
+// of k_deliver as in update_group.
+// ===========================================================================
+__device__ __noinline__ void emit_global(const SimDev& p, const unsigned long long n, const unsigned long long spike_begin,
+                                         const int i0, const unsigned lane, const unsigned spike_bits) {
+    unsigned my_spk = __popc(spike_bits), my_work = 0, my_events = 0;
+    int len[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (spike_bits & (1u << q)) {
+            len[q] = __ldg(p.row_len + i0 + q);
+            my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
+            my_events += (unsigned)len[q];
+        }
+    // inclusive warp scan of (spikes, work items) packed in one 64-bit word
+    unsigned long long pk = ((unsigned long long)my_spk << 32) | my_work;
+    unsigned long long inc = pk;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        unsigned long long o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= (unsigned)d) inc += o;
+    }
+    const unsigned long long tot = __shfl_sync(0xffffffffu, inc, 31);
+    const unsigned ev_warp = __reduce_add_sync(0xffffffffu, my_events);
+    unsigned long long base = 0;
+    if (lane == 0) {
+        base = atomicAdd(&p.ctl->step_counts[n & 1ull], tot);
+        atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
+    }
+    base = __shfl_sync(0xffffffffu, base, 0);
+    const unsigned long long mine = base + inc - pk;          // exclusive offsets
+    unsigned long long spk_pos = spike_begin + (mine >> 32);
+    unsigned work_pos = (unsigned)mine;
+    const unsigned win = (unsigned)((n / (unsigned long long)p.window_steps) % p.max_windows);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (spike_bits & (1u << q)) {
+            const int i = i0 + q;
+            p.spike_ids[spk_pos & p.spike_mask] = i;
+            p.spike_tag[spk_pos & p.spike_mask] = (uint32_t)n;
+            ++spk_pos;
+            const int nch = (len[q] + kChunk - 1) / kChunk;
+            for (int c = 0; c < nch; ++c) p.work[work_pos++] = make_int2(i, c);
+            const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
+            atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
+        }
+}
+
+__global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_constant__ SimDev p, const RunCfg cfg) {
+    extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
+    __shared__ TypeSmem s_tc[kMaxTypes];
+    __shared__ uint32_t s_T[kMaxTypes][kPoissonMax];
+    const unsigned lane = threadIdx.x & 31u;
+    const int warp = (int)(threadIdx.x >> 5), n_warps = (int)(blockDim.x >> 5);
+    for (int t = (int)threadIdx.x; t < kMaxTypes; t += (int)blockDim.x) {
+        const TypeConst& tc = p.tc[t];
+        TypeSmem r;
+        for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(tc.G[u], tc.E[u], tc.alpha[u], 0.0f);
+        r.m0 = make_float4(tc.neg_gL, tc.VL, tc.kappa, tc.Iext);
+        r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
+        r.m2 = make_uint4((unsigned)tc.M, tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu, tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu,
+                          tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu);
+        s_tc[t] = r;
+    }
+    for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
+        s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
+    __syncthreads();
+
+    Stage sg;
+    sg.sbase = (uint32_t)__cvta_generic_to_shared(s_stage) + threadIdx.x * 16u;
+    sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * kPlaneStride + threadIdx.x * 8u;
+    const unsigned long long n = p.ctl->step;
+    const unsigned long long sb = p.ctl->spike_begin;
+    const int first = (int)blockIdx.x * cfg.tasks_per_block;
+    const int last = min(first + cfg.tasks_per_block, cfg.n_tasks);
+    const int task0 = first + warp;
+    if (task0 >= last) return;
+    const size_t Np = (size_t)p.Npad;
+    int32_t* const slot0 = p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np;
+    const int i00 = (task0 * 32 + (int)lane) * 4;
+    const int task_stride = n_warps * 128;
+    unsigned bg_acc = 0u;
+    request_state(p, sg, i00);
+    request_ring(p, sg, slot0 + i00);
+    cp_async_commit();
+    for (int task = task0; task < last; task += n_warps) {
+        const int next_off = (task + n_warps < last) ? task_stride : 0;
+        const int grp = task * 32 + (int)lane;
+        const int i0 = grp * 4;
+        // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
+        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)),
+                                        p.seed_lo, p.seed_hi);
+        cp_async_wait_all();
+        const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
+        const uint2 rt_bits = lds64(sg.srt);
+        if (next_off) {
+            cp_async16(sg.sbase + 4u * kPlaneStride, p.V + i0 + next_off);
+            cp_async8(sg.srt, p.rt + i0 + next_off);
+        }
+        const int tp0 = (int)((rt_bits.x >> 12) & 0xFu), tp1 = (int)(rt_bits.x >> 28);
+        const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
+        unsigned spike_bits;
+        if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
+            spike_bits = neuron_group<true, true, true>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc);
+        else                            // a type boundary inside the group (rare)
+            spike_bits = neuron_group<true, true, true>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc);
+        cp_async_commit();
+        if (__ballot_sync(0xffffffffu, spike_bits != 0)) emit_global(p, n, sb, i0, lane, spike_bits);
+    }
+    const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
+    if (lane == 0 && bg_warp)
+        atomicAdd(p.bg_parts + ((blockIdx.x * (unsigned)n_warps + (unsigned)warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
+}
+
 // ---------------------------------------------------------------------------
 // State initialisation: V0 = Vreset + (Vth - Vreset) * U, U = (u >> 8) * 2^-24
 // keyed by (dyn_seed, STREAM_V0, i); g = 0, ref = 0.
@@ -916,10 +881,19 @@ cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStr
     return cudaGetLastError();
 }
 
-int update_grid(const SimDev& p) { return (p.Npad / 4 + 255) / 256; }
+void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg);
 
-cudaError_t launch_update(const SimDev& p, cudaStream_t st) {
-    k_update<<<update_grid(p), 256, 0, st>>>(p);
+cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_update_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    int grid = 0, threads = 0;
+    RunCfg cfg{};
+    run_shape(p, n_sm, &grid, &threads, &cfg);
+    k_update_stream<<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);      // no service warp here
     return cudaGetLastError();
 }
 
