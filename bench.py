@@ -211,7 +211,8 @@ def run_ours(args):
     cfg = db_inputs.config(args.config, rate_hz=(args.rate if args.config == 1 else None), scale=args.scale)
     N = cfg["net"]["N"]
     n_sim = args.sim_steps
-    mode = {"auto": db.EXEC_AUTO, "kernels": db.EXEC_KERNELS, "persistent": db.EXEC_PERSISTENT}[args.exec_mode]
+    mode = {"auto": db.EXEC_AUTO, "kernels": db.EXEC_KERNELS, "persistent": db.EXEC_PERSISTENT,
+            "deferred": db.EXEC_KERNELS_DEFERRED}[args.exec_mode]
     raster_cap = 1 << 25
     sim = db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED + rank, dyn_seed=db_inputs.DYN_SEED + rank,
                            exec_mode=mode, raster_capacity=raster_cap, device=local)
@@ -293,7 +294,7 @@ def run_ours(args):
             "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
             "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
             "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
-            "deliver": {"kernel": "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
+            "deliver": {"kernel": "k_deliver_deferred" if exec_used == 3 else "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
                         "events_per_launch": prof["events"] / prof["steps"], "bytes_per_event": ev_bytes,
                         "share_of_step": prof["deliver_ms"] / max(prof["total_ms"], 1e-12)},
         }
@@ -301,7 +302,7 @@ def run_ours(args):
             roofline = dict(two, note=note)
             if two["deliver"]["share_of_step"] > two["share_of_step"]:      # delivery-bound workloads (configs 3, 4)
                 dlv = two["deliver"]
-                roofline = {"bound": "hbm", "kernel": "k_deliver", "achieved": dlv["achieved"], "peak": peak,
+                roofline = {"bound": "hbm", "kernel": dlv["kernel"], "achieved": dlv["achieved"], "peak": peak,
                             "unit": "GB/s", "frac": dlv["frac"], "traffic": None, "peak_source": peak_src,
                             "bytes_per_launch": ev_bytes * dlv["events_per_launch"], "us_per_launch": dlv["us_per_launch"],
                             "share_of_step": dlv["share_of_step"], "update": {k: v for k, v in two.items() if k != "deliver"},
@@ -377,7 +378,7 @@ def run_ours(args):
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": dict(_config_dict(args, N, n_sim), replicas=world,
-                           exec_mode={1: "kernels+graph", 2: "persistent"}.get(exec_used, str(exec_used))),
+                           exec_mode={1: "kernels+graph", 2: "persistent", 3: "kernels+graph, deferred delivery"}.get(exec_used, str(exec_used))),
             "neuron_updates_per_s": world * N * args.steps * n_sim / secs,
             "rtf": secs / bio_s, "mean_rate_hz": rate_hz, "us_per_sim_step": 1e6 * secs / (args.steps * n_sim),
             "paper_context": "paper RTF 65 / 78.8 / 118.8 at 7 / 15 / 30 Hz for 86e9 neurons on 14,012 GPUs (dt 1 ms): "
@@ -403,7 +404,7 @@ def main():
                     help="BASELINE.json configs[i]; 1 is the bench workload, the others are timed for profiles/ only")
     ap.add_argument("--sim-steps", type=int, default=1000, help="simulation time steps per bench step")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink configs[1] (debugging only)")
-    ap.add_argument("--exec-mode", choices=["auto", "kernels", "persistent"], default="auto")
+    ap.add_argument("--exec-mode", choices=["auto", "kernels", "persistent", "deferred"], default="auto")
     ap.add_argument("--profile-steps", type=int, default=512)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -69,6 +69,10 @@ typedef struct db_type_params {
 #define DB_EXEC_AUTO       0   /* library picks */
 #define DB_EXEC_KERNELS    1   /* two kernels per step (update+compaction, delivery), CUDA-graph replayed */
 #define DB_EXEC_PERSISTENT 2   /* one cooperative persistent kernel looping over the steps */
+#define DB_EXEC_KERNELS_DEFERRED 3 /* two kernels per step; synapses with a short delay are pushed in the step before
+                                      they arrive, out of the spike lists of the last steps (rows sorted by delay), so
+                                      that all those reductions hit ONE ring slot, which stays in L2; same results.  Falls back to
+                                      DB_EXEC_KERNELS when no delay exceeds 1 or the raster ring cannot hold the spikes of 31 steps */
 
 typedef struct db_sim_params {
     uint32_t struct_size;     /* = sizeof(db_sim_params) */

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 DB_OK, DB_EINVAL, DB_ENOMEM, DB_ECUDA, DB_ERANGE, DB_ESTATE = 0, -1, -2, -3, -4, -5
-EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT = 0, 1, 2
+EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 (FIELD_V, FIELD_G_AMPA, FIELD_G_NMDA, FIELD_G_GABAA, FIELD_G_GABAB, FIELD_REF, FIELD_TYPE, FIELD_RING,
  FIELD_OUTDEG) = range(9)
 

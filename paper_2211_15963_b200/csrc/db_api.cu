@@ -136,7 +136,7 @@ int32_t check_sim_params(db_sim* sim, const db_sim_params* sp) {
     if (sp->D < 2 || sp->D > 65536 || (sp->D & (sp->D - 1))) return fail(sim, DB_EINVAL, "D must be a power of two in 2..65536");
     if (sp->window_steps < 1) return fail(sim, DB_EINVAL, "window_steps must be >= 1");
     if (sp->n_types < 1 || sp->n_types > DB_MAX_TYPES) return fail(sim, DB_EINVAL, "n_types must be 1..4");
-    if (sp->exec_mode < DB_EXEC_AUTO || sp->exec_mode > DB_EXEC_PERSISTENT) return fail(sim, DB_EINVAL, "bad exec_mode");
+    if (sp->exec_mode < DB_EXEC_AUTO || sp->exec_mode > DB_EXEC_KERNELS_DEFERRED) return fail(sim, DB_EINVAL, "bad exec_mode");
     return DB_OK;
 }
 
@@ -210,15 +210,60 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     return DB_OK;
 }
 
+// DB_EXEC_KERNELS_DEFERRED: sort every row by delay (on the device, batch by batch through scratch
+// arrays) and build the segment table.  near_max = largest delay whose push is deferred.
+int32_t build_delay_segments(db_sim* sim, int near_max) {
+    SimDev& d = sim->dev;
+    const int64_t N = d.N;
+    std::vector<int64_t> rb((size_t)N);
+    std::vector<int32_t> rl((size_t)N);
+    CK(cudaStreamSynchronize(sim->stream));
+    CK(cudaMemcpy(rb.data(), d.row_begin, (size_t)N * 8, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(rl.data(), d.row_len, (size_t)N * 4, cudaMemcpyDeviceToHost));
+    uint32_t* seg = nullptr;
+    int32_t rc = alloc_zero(sim, &seg, (size_t)N * (size_t)(near_max + 1));
+    if (rc) return rc;
+    auto row_end = [&](int64_t j) { return rb[(size_t)j] + ((int64_t)rl[(size_t)j] + kRowAlign - 1) / kRowAlign * kRowAlign; };
+    const int64_t batch = std::min<int64_t>(sim->Epad, (int64_t)1 << 28);        // synapses per batch
+    const size_t wsz = d.w_fp16 ? 2 : 4;
+    uint32_t* t_s = nullptr; uint8_t* d_s = nullptr; void* w_s = nullptr;
+    if (cudaMalloc(&t_s, (size_t)batch * 4) != cudaSuccess || cudaMalloc(&d_s, (size_t)batch) != cudaSuccess ||
+        cudaMalloc(&w_s, (size_t)batch * wsz) != cudaSuccess) {
+        cudaFree(t_s); cudaFree(d_s); cudaFree(w_s);
+        cudaGetLastError();
+        return fail(sim, DB_ENOMEM, "no device memory for the row-sorting scratch arrays");
+    }
+    int32_t out = DB_OK;
+    for (int64_t r0 = 0; r0 < N && out == DB_OK;) {
+        const int64_t s0 = rb[(size_t)r0];
+        int64_t r1 = r0 + 1;
+        while (r1 < N && row_end(r1) - s0 <= batch) ++r1;
+        const int64_t s1 = row_end(r1 - 1);
+        if (s1 - s0 > batch) { out = fail(sim, DB_EINVAL, "a row is longer than the sorting batch"); break; }
+        cudaError_t e = launch_sort_rows(d, r0, r1, s0, t_s, w_s, d_s, seg, near_max, sim->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint32_t*>(d.tgt_rec) + s0, t_s, (size_t)(s1 - s0) * 4, cudaMemcpyDeviceToDevice, sim->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint8_t*>(d.delay) + s0, d_s, (size_t)(s1 - s0), cudaMemcpyDeviceToDevice, sim->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync((char*)const_cast<void*>(d.w) + (size_t)s0 * wsz, w_s, (size_t)(s1 - s0) * wsz, cudaMemcpyDeviceToDevice, sim->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
+        if (e != cudaSuccess) out = fail(sim, DB_ECUDA, std::string("row sorting: ") + cudaGetErrorString(e));
+        r0 = r1;
+    }
+    cudaFree(t_s); cudaFree(d_s); cudaFree(w_s);
+    if (out) return out;
+    d.seg = seg;
+    d.near_max = near_max;
+    return DB_OK;
+}
+
 // After the CSR is on the device: work list, execution mode, initial state.
-int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
+int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int32_t near_hint) {
     SimDev& d = sim->dev;
     int32_t rc;
     sim->work_cap = std::max<uint64_t>(work_cap, 1);
     if ((rc = alloc_zero(sim, &d.work, (size_t)sim->work_cap))) return rc;
     sim->heavy = heavy_chunks > 0;
     CK(launch_init_state(d, sim->ntype_dev, sim->stream));
-    sim->deliver_grid = sim->n_sm * 4;
+    sim->deliver_grid = sim->n_sm * 8;
     sim->update_sm = sim->n_sm;
     int coop = 0;
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device));
@@ -229,7 +274,20 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     // out-degree >= 400: configs 3 and 4) the step is delivery-bound and the two-kernel mode, where every
     // warp of the grid pushes rows, is faster (measured: profiles/)
     const bool delivery_bound = sim->heavy || (sim->E >= 400 * (int64_t)d.N);
-    if (mode == DB_EXEC_AUTO) mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : DB_EXEC_KERNELS;
+    // deferred delivery needs the spike lists of the last near_max steps in the raster ring: a neuron fires
+    // at most once per R + 1 steps
+    const int near_max = std::min<int32_t>(31, near_hint);
+    int r_min = d.tc[0].R;
+    for (int t = 1; t < sim->params.n_types; ++t) r_min = std::min(r_min, d.tc[t].R);
+    const bool can_defer = near_max >= 2 &&
+        (uint64_t)d.N * (uint64_t)((near_max + r_min) / (r_min + 1)) <= sim->spike_cap;
+    if (mode == DB_EXEC_AUTO)
+        mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : (can_defer ? DB_EXEC_KERNELS_DEFERRED : DB_EXEC_KERNELS);
+    if (mode == DB_EXEC_KERNELS_DEFERRED && !can_defer) mode = DB_EXEC_KERNELS;   // nothing to defer, or the raster ring is too small
+    if (mode == DB_EXEC_KERNELS_DEFERRED) {
+        int32_t rc2 = build_delay_segments(sim, near_max);
+        if (rc2) return rc2;
+    }
     if (mode == DB_EXEC_PERSISTENT && (!coop || !fits))
         return fail(sim, DB_ECUDA, "cooperative launch not available for the persistent mode");
     sim->exec_mode = mode;
@@ -340,7 +398,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
         return bail(fail(sim, DB_ECUDA, std::string("CSR upload: ") + cudaGetErrorString(cudaGetLastError())));
     d.row_begin = rb_dev; d.row_len = rl_dev; d.tgt_rec = tr_dev; d.delay = dl_dev; d.w = w_dev;
     d.w_fp16 = csr->weight_fp16 ? 1 : 0;
-    if ((rc = finish_setup(sim, work_cap, heavy_chunks))) return bail(rc);
+    if ((rc = finish_setup(sim, work_cap, heavy_chunks, max_delay))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -376,7 +434,7 @@ int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
     d.w_fp16 = spec->weight_fp16 ? 1 : 0;
     sim->E = gr.E; sim->Epad = gr.Epad;
     if (gr.max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
-    if ((rc = finish_setup(sim, gr.work_cap, gr.heavy_chunks))) return bail(rc);
+    if ((rc = finish_setup(sim, gr.work_cap, gr.heavy_chunks, spec->delay_intra_max))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -578,6 +636,19 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
                 CK(cudaMemcpy(t.data(), d.ring + (sd * 4 + u) * Np + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
                 for (int64_t i = 0; i < count; ++i) o[(s * (size_t)count + (size_t)i) * 4 + u] = t[(size_t)i];
             }
+        }
+        if (d.near_max > 0) {          // deferred mode: plus the near segments not pushed yet
+            const size_t cells = (size_t)D * (size_t)count * 4;
+            int32_t* tmp = nullptr;
+            if (cudaMalloc(&tmp, cells * 4) != cudaSuccess) { cudaGetLastError(); return fail(sim, DB_ENOMEM, "no device memory for the ring read-out"); }
+            cudaError_t e = cudaMemsetAsync(tmp, 0, cells * 4, sim->stream);
+            if (e == cudaSuccess) e = launch_pending_ring(d, tmp, (int)first, (int)count, D, sim->stream);
+            std::vector<int32_t> pend(cells);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
+            if (e == cudaSuccess) e = cudaMemcpy(pend.data(), tmp, cells * 4, cudaMemcpyDeviceToHost);
+            cudaFree(tmp);
+            if (e != cudaSuccess) return fail(sim, DB_ECUDA, std::string("ring read-out: ") + cudaGetErrorString(e));
+            for (size_t k = 0; k < cells; ++k) o[k] = (int32_t)((uint32_t)o[k] + (uint32_t)pend[k]);
         }
         break;
     }

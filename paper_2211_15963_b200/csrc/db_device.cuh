@@ -66,6 +66,10 @@ struct SimDev {                      // passed by value to every kernel
     const void* w;                   // [Epad] float or __half
     const uint8_t* delay;            // [Epad]
     int32_t w_fp16;
+    // DB_EXEC_KERNELS_DEFERRED: rows sorted by delay; seg[j * (near_max + 1) + (d - 1)] = first synapse of row j
+    // (relative to row_begin) with delay >= d, for d = 1 .. near_max + 1 (the last entry starts the far part)
+    const uint32_t* seg;
+    int32_t near_max;                // 0: delivery is immediate for every synapse
     // spike list = raster ring; per-step work list
     int32_t* spike_ids;              // [spike_cap] circular
     uint32_t* spike_tag;             // [spike_cap] low 32 bits of the step of each entry (steps may interleave by one)

@@ -12,7 +12,12 @@ namespace dbk {
 // ---- db_step.cu ------------------------------------------------------------
 cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
 cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st);
-cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);
+cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);   // deferred variant when p.near_max > 0
+// DB_EXEC_KERNELS_DEFERRED: sort the rows [row0, row1) by delay into scratch arrays indexed by (synapse - s0) and fill
+// their segment tables; add the not yet pushed near segments to a DB_FIELD_RING read-out
+cudaError_t launch_sort_rows(const SimDev& p, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
+                             uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st);
+cudaError_t launch_pending_ring(const SimDev& p, int32_t* out, int first, int count, int D_api, cudaStream_t st);
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 

@@ -8,6 +8,7 @@
 // Paper: SI Eq.(3) P:L475 (conductances), CV equation P:L382 + SI Eq.(5)
 // (membrane), P:L108 / P:L481-482 (threshold, reset, refractory), Supp. Alg. 2
 // P:L879-884 and P:L490 (push delivery with atomics along the destination list).
+#include <algorithm>
 #include <cuda_fp16.h>
 #include <cooperative_groups.h>
 #include "db_device.cuh"
@@ -754,8 +755,10 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
             len[q] = __ldg(p.row_len + i0 + q);
-            my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
             my_events += (unsigned)len[q];
+            if (p.near_max > 0)        // deferred mode: only the far part of the row is pushed now
+                len[q] -= (int)__ldg(p.seg + (size_t)(i0 + q) * (size_t)(p.near_max + 1) + (size_t)p.near_max);
+            my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
         }
     // inclusive warp scan of (spikes, work items) packed in one 64-bit word
     unsigned long long pk = ((unsigned long long)my_spk << 32) | my_work;
@@ -873,6 +876,252 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
     p.rt[i] = (uint16_t)(tp << 12);
 }
 
+// ===========================================================================
+// Mode DB_EXEC_KERNELS_DEFERRED.  Pushing a spike's whole row when it fires
+// scatters 4-byte reductions over every ring slot the row's delays reach: on
+// networks whose ring is far larger than L2 every event misses (measured:
+// ~99 B of DRAM sectors per 17-byte event, profiles/).  Here the rows are
+// sorted by delay and the push of the synapses with delay d <= near_max is
+// DEFERRED: after the update of step n, the kernel walks the spike lists of
+// the steps n + 1 - d (d = 1 .. near_max; the raster keeps them) and pushes
+// from each of those rows the segment with delay d -- all of it arrives in
+// step n + 1, so every reduction hits the ONE ring slot n + 1 (16 B x N, L2
+// sized), and DRAM only streams the CSR segments.  Synapses with longer
+// delays (the far part of a row) are pushed when the neuron fires, as in the
+// other modes.  The sums are the same integers, whatever the order.
+// ===========================================================================
+
+// Sort the rows [row0, row1) by delay into scratch arrays (indexed by synapse - s0) and fill their
+// segment tables; one warp per row, counting sort over the 256 possible delays.
+constexpr int kSortWarps = 8;
+template <bool kHalf>
+__global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const int64_t* __restrict__ row_begin,
+        const int32_t* __restrict__ row_len, const uint32_t* __restrict__ tgt_rec, const void* __restrict__ w,
+        const uint8_t* __restrict__ delay, const int64_t row0, const int64_t row1, const int64_t s0,
+        uint32_t* __restrict__ tgt_out, void* __restrict__ w_out, uint8_t* __restrict__ delay_out,
+        uint32_t* __restrict__ seg, const int near_max) {
+    __shared__ unsigned s_cnt[kSortWarps][256];
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    unsigned* cnt = s_cnt[warp];
+    const long long n_warps = (long long)gridDim.x * kSortWarps;
+    for (long long j = row0 + (long long)blockIdx.x * kSortWarps + warp; j < row1; j += n_warps) {
+        const int64_t rb = row_begin[j];
+        const int len = row_len[j];
+        for (int k = (int)lane; k < 256; k += 32) cnt[k] = 0u;
+        __syncwarp();
+        for (int e = (int)lane; e < len; e += 32) atomicAdd(&cnt[delay[rb + e]], 1u);
+        __syncwarp();
+        // exclusive scan of the 256 counters: lane l owns the bins 8 l .. 8 l + 7
+        unsigned loc[8], sum = 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { loc[k] = sum; sum += cnt[lane * 8 + k]; }
+        unsigned inc = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= (unsigned)d) inc += o;
+        }
+        const unsigned base = inc - sum;
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < 8; ++k) cnt[lane * 8 + k] = base + loc[k];      // start of every delay inside the row
+        __syncwarp();
+        // segment table: first synapse with delay >= d, d = 1 .. near_max + 1 (delays are >= 1)
+        for (int d = 1 + (int)lane; d <= near_max + 1; d += 32)
+            seg[(size_t)j * (size_t)(near_max + 1) + (size_t)(d - 1)] = (d < 256) ? cnt[d] : (unsigned)len;
+        __syncwarp();
+        for (int e = (int)lane; e < len; e += 32) {
+            const unsigned d = delay[rb + e];
+            const int64_t o = rb - s0 + (int64_t)atomicAdd(&cnt[d], 1u);
+            tgt_out[o] = tgt_rec[rb + e];
+            delay_out[o] = (uint8_t)d;
+            if (kHalf) static_cast<__half*>(w_out)[o] = static_cast<const __half*>(w)[rb + e];
+            else       static_cast<float*>(w_out)[o] = static_cast<const float*>(w)[rb + e];
+        }
+        const int padded = (len + kRowAlign - 1) / kRowAlign * kRowAlign;      // keep the row padding inert
+        for (int e = len + (int)lane; e < padded; e += 32) {
+            const int64_t o = rb - s0 + e;
+            tgt_out[o] = 0u;
+            delay_out[o] = 1;
+            if (kHalf) static_cast<__half*>(w_out)[o] = __float2half(0.0f);
+            else       static_cast<float*>(w_out)[o] = 0.0f;
+        }
+        __syncwarp();
+    }
+}
+
+// Push `len` synapses starting at `rb` (any alignment), one synapse per lane and pass.
+// kFixed: all of them land in slot `slot_fixed` (a delay segment); else the slot follows the stored delay.
+template <bool kHalf, bool kFixed>
+__device__ __forceinline__ void deliver_scalar(const SimDev& p, const unsigned nlo, const unsigned slot_fixed,
+                                               const int64_t rb, const int len, const unsigned lane) {
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    for (int e = (int)lane; e < len; e += 32) {
+        const unsigned t = __ldg(p.tgt_rec + rb + e);
+        float wf;
+        if (kHalf) wf = __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e));
+        else       wf = __ldg(static_cast<const float*>(p.w) + rb + e);
+        const unsigned sl = kFixed ? slot_fixed : ((nlo + (unsigned)__ldg(p.delay + rb + e)) & Dm);
+        const int wq = __float2int_rn(__fmul_rn(wf, p.wscale));
+        red_add_s32(p.ring + ((size_t)sl * 4 + (t >> 30)) * Np + (t & 0x3FFFFFFFu), wq);
+    }
+}
+
+// Spike list of step m in the two-kernel modes: raster positions [begin, end).  `n` = current step
+// (its own entry is not in the step log yet: the count comes from the step counter).
+__device__ __forceinline__ void spike_range(const SimDev& p, const unsigned long long n, const unsigned long long counts,
+                                            const long long m, unsigned long long& begin, unsigned long long& end) {
+    begin = end = 0ull;
+    if (m < 0) return;
+    if ((unsigned long long)m == n) { begin = p.ctl->spike_begin; end = begin + (counts >> 32); return; }
+    begin = (m == 0) ? 0ull : p.step_end[(unsigned long long)(m - 1) & p.step_log_mask];
+    end = p.step_end[(unsigned long long)m & p.step_log_mask];
+}
+
+template <bool kHalf>
+__global__ void __launch_bounds__(256) k_deliver_deferred(const __grid_constant__ SimDev p) {
+    __shared__ unsigned long long s_begin[32];
+    __shared__ unsigned s_cum[33];                  // s_cum[d] = near items of the delays < d + 1 (exclusive prefix)
+    __shared__ unsigned s_pref[8][32];              // per warp: first flat synapse index of each of its 32 items
+    __shared__ long long s_rb[8][32];               // per warp: first synapse of each item
+    const unsigned long long n = p.ctl->step;
+    const unsigned long long counts = p.ctl->step_counts[n & 1ull];
+    const unsigned n_work = (unsigned)counts;       // far-part chunks of this step's spikes
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
+    const int S = p.near_max + 1;
+    if (threadIdx.x < 32) {
+        unsigned long long b = 0ull, e = 0ull;
+        if ((int)lane < p.near_max) spike_range(p, n, counts, (long long)n - (long long)lane, b, e);   // d = lane + 1
+        const unsigned c = (unsigned)(e - b);
+        unsigned inc = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= (unsigned)d) inc += o;
+        }
+        s_begin[lane] = b;
+        s_cum[lane + 1] = inc;
+        if (lane == 0) s_cum[0] = 0u;
+    }
+    __syncthreads();
+    // ---- far part of the rows that fired in this step (delay > near_max): pushed now, slot by stored delay
+    for (unsigned q = warp; q < n_work; q += n_warps) {
+        const int2 wk = p.work[q];
+        const int j = wk.x;
+        const int near_end = (int)__ldg(p.seg + (size_t)j * S + p.near_max);
+        const int off = near_end + wk.y * kChunk;
+        const int len = min(kChunk, __ldg(p.row_len + j) - off);
+        deliver_scalar<kHalf, false>(p, (unsigned)n, 0u, __ldg(p.row_begin + j) + off, len, lane);
+    }
+    // ---- near part: segment d of every row that fired in step n + 1 - d arrives in step n + 1.
+    // An item = (delay d, one spike of step n + 1 - d).  A warp takes 32 items at a time: every lane
+    // fetches the descriptor of one item (spike id -> segment bounds -> row start: all 32 chains in
+    // flight together), then the lanes walk the synapses of the 32 segments as ONE flat range, so that
+    // the loads of a pass are independent whatever the segment lengths are.
+    const unsigned total = s_cum[32];
+    const unsigned slot = (unsigned)(n + 1ull) & (unsigned)(p.D - 1);
+    const size_t Np = (size_t)p.Npad;
+    int32_t* const ring_slot = p.ring + (size_t)slot * 4 * Np;
+    unsigned* const w_pref = s_pref[threadIdx.x >> 5];
+    long long* const w_rb = s_rb[threadIdx.x >> 5];
+    for (unsigned base = warp * 32u; base < total; base += n_warps * 32u) {
+        const unsigned q = base + lane;
+        int len = 0;
+        long long rb = 0;
+        if (q < total) {
+            unsigned lo = 0u, hi = (unsigned)p.near_max;                     // largest dm1 with s_cum[dm1] <= q
+            while (hi - lo > 1u) { const unsigned mid = (lo + hi) >> 1; if (s_cum[mid] <= q) lo = mid; else hi = mid; }
+            const unsigned long long pos = s_begin[lo] + (unsigned long long)(q - s_cum[lo]);
+            const int j = p.spike_ids[pos & p.spike_mask];
+            const uint32_t* sg = p.seg + (size_t)j * S + lo;
+            const int o0 = (int)__ldg(sg), o1 = (int)__ldg(sg + 1);
+            len = o1 - o0;
+            rb = (long long)__ldg(p.row_begin + j) + o0;
+        }
+        unsigned inc = (unsigned)len;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= (unsigned)d) inc += o;
+        }
+        const unsigned flat = __shfl_sync(0xffffffffu, inc, 31);
+        w_pref[lane] = inc - (unsigned)len;
+        w_rb[lane] = rb;
+        __syncwarp();
+        for (unsigned s0 = 0u; s0 < flat; s0 += 128u) {                      // four independent passes in flight
+            unsigned t[4];
+            float wf[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned sx = s0 + (unsigned)u * 32u + lane;
+                t[u] = 0u; wf[u] = 0.0f;
+                if (sx < flat) {
+                    unsigned k = 0u;                                         // largest k with w_pref[k] <= sx
+#pragma unroll
+                    for (unsigned step = 16u; step; step >>= 1) if (w_pref[k + step] <= sx) k += step;
+                    const long long e = w_rb[k] + (long long)(sx - w_pref[k]);
+                    t[u] = __ldg(p.tgt_rec + e);
+                    if (kHalf) wf[u] = __half2float(__ldg(static_cast<const __half*>(p.w) + e));
+                    else       wf[u] = __ldg(static_cast<const float*>(p.w) + e);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (s0 + (unsigned)u * 32u + lane < flat)
+                    red_add_s32(ring_slot + (size_t)(t[u] >> 30) * Np + (t[u] & 0x3FFFFFFFu), __float2int_rn(__fmul_rn(wf[u], p.wscale)));
+        }
+        __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned ticket = atomicAdd(&p.ctl->done_blocks, 1u);
+        if (ticket == gridDim.x - 1) {            // every block has read n / counts / the step log: safe to advance
+            p.ctl->done_blocks = 0u;
+            finalize_step(p, n, counts);
+        }
+    }
+}
+
+// Read-back of the ring in deferred mode: the arrivals still to come are the ring's content PLUS the
+// near segments not pushed yet -- spikes of step m (n - near_max < m < n), delays n - m < d <= near_max,
+// arriving in step m + d.  Adds them for the targets [first, first + count) into `out`, which has the
+// layout of DB_FIELD_RING: out[(slot * count + i) * 4 + receptor], slot = arrival step mod D_api.
+template <bool kHalf>
+__global__ void __launch_bounds__(256) k_pending_ring(const __grid_constant__ SimDev p, int32_t* __restrict__ out,
+                                                      const int first, const int count, const int D_api) {
+    const unsigned long long n = p.ctl->step;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
+    const int S = p.near_max + 1;
+    for (int age = 1; age < p.near_max; ++age) {              // m = n - age: delays age + 1 .. near_max are pending
+        const long long m = (long long)n - age;
+        unsigned long long b, e;
+        spike_range(p, n, 0ull, m, b, e);
+        for (unsigned long long pos = b + warp; pos < e; pos += n_warps) {
+            const int j = p.spike_ids[pos & p.spike_mask];
+            const int64_t rb = __ldg(p.row_begin + j);
+            const int o0 = (int)__ldg(p.seg + (size_t)j * S + age);          // first synapse with delay >= age + 1
+            const int o1 = (int)__ldg(p.seg + (size_t)j * S + p.near_max);   // start of the far part
+            for (int s = o0 + (int)lane; s < o1; s += 32) {
+                const unsigned t = __ldg(p.tgt_rec + rb + s);
+                const int tg = (int)(t & 0x3FFFFFFFu) - first;
+                if (tg < 0 || tg >= count) continue;
+                float wf;
+                if (kHalf) wf = __half2float(__ldg(static_cast<const __half*>(p.w) + rb + s));
+                else       wf = __ldg(static_cast<const float*>(p.w) + rb + s);
+                const unsigned long long arrive = (unsigned long long)m + (unsigned long long)__ldg(p.delay + rb + s);
+                const size_t slot = (size_t)(arrive % (unsigned long long)D_api);
+                atomicAdd(out + (slot * (size_t)count + (size_t)tg) * 4 + (t >> 30), __float2int_rn(__fmul_rn(wf, p.wscale)));
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------
 // host-side launchers (called from db_api.cu)
 // ---------------------------------------------------------------------------
@@ -898,8 +1147,30 @@ cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st) {
 }
 
 cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
-    if (p.w_fp16) k_deliver<true><<<grid, 256, 0, st>>>(p);
-    else          k_deliver<false><<<grid, 256, 0, st>>>(p);
+    if (p.near_max > 0) {
+        if (p.w_fp16) k_deliver_deferred<true><<<grid, 256, 0, st>>>(p);
+        else          k_deliver_deferred<false><<<grid, 256, 0, st>>>(p);
+    } else {
+        if (p.w_fp16) k_deliver<true><<<grid, 256, 0, st>>>(p);
+        else          k_deliver<false><<<grid, 256, 0, st>>>(p);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sort_rows(const SimDev& p, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
+                             uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st) {
+    const int grid = (int)std::min<int64_t>((row1 - row0 + kSortWarps - 1) / kSortWarps, 148 * 16);
+    if (grid <= 0) return cudaSuccess;
+    if (p.w_fp16) k_sort_rows<true><<<grid, kSortWarps * 32, 0, st>>>(p.row_begin, p.row_len, p.tgt_rec, p.w, p.delay, row0, row1,
+                                                                     s0, tgt_out, w_out, delay_out, seg, near_max);
+    else          k_sort_rows<false><<<grid, kSortWarps * 32, 0, st>>>(p.row_begin, p.row_len, p.tgt_rec, p.w, p.delay, row0, row1,
+                                                                      s0, tgt_out, w_out, delay_out, seg, near_max);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pending_ring(const SimDev& p, int32_t* out, int first, int count, int D_api, cudaStream_t st) {
+    if (p.w_fp16) k_pending_ring<true><<<148 * 4, 256, 0, st>>>(p, out, first, count, D_api);
+    else          k_pending_ring<false><<<148 * 4, 256, 0, st>>>(p, out, first, count, D_api);
     return cudaGetLastError();
 }
 

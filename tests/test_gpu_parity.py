@@ -48,7 +48,7 @@ def _pair(db, oracle_mod, sim, net, mode, seed=db_inputs.DYN_SEED, fp16=False, *
     return g, o
 
 
-MODES = [1, 2]   # DB_EXEC_KERNELS, DB_EXEC_PERSISTENT
+MODES = [1, 2, 3]   # DB_EXEC_KERNELS, DB_EXEC_PERSISTENT, DB_EXEC_KERNELS_DEFERRED
 
 
 @pytest.mark.parametrize("mode", MODES)
@@ -114,7 +114,7 @@ def test_config0_raster_identical_200_steps_and_ring_bit_exact(db, oracle_mod, m
 
 
 @pytest.mark.parametrize("mode", MODES)
-@pytest.mark.parametrize("case", ["empty", "one", "ragged", "heavy", "regions_fp16", "maxdelay"])
+@pytest.mark.parametrize("case", ["empty", "one", "ragged", "heavy", "regions_fp16", "maxdelay", "far"])
 def test_edge_cases(db, oracle_mod, mode, case):
     sim = db_inputs.sim_params()
     strong = db_inputs.type_params(bg_weight=0.03)
@@ -134,6 +134,11 @@ def test_edge_cases(db, oracle_mod, mode, case):
         net = db_inputs.random_csr(N=2500, mean_outdeg=30, seed=7, n_regions=7, fp16=True)
         fp16 = True
         sim["window_steps"] = 7
+    elif case == "far":                       # delays beyond the 31 steps whose push the deferred mode defers
+        sim["D"] = 128
+        net = db_inputs.random_csr(N=1500, mean_outdeg=40, seed=9, max_delay=100, fp16=True)
+        fp16 = True
+        assert net["delay"].max() == 100
     else:                                     # delays 1 and D-1 both present
         net = db_inputs.random_csr(N=900, mean_outdeg=20, seed=8, max_delay=sim["D"] - 1)
         assert net["delay"].min() == 1 and net["delay"].max() == sim["D"] - 1
@@ -156,11 +161,13 @@ def test_edge_cases(db, oracle_mod, mode, case):
     assert len(cnt) == steps // sim["window_steps"]
 
 
-def test_modes_agree_and_split_stepping(db):
-    # kernels vs persistent, and db_step(a); db_step(b) == db_step(a + b) (graph replay + remainder)
+@pytest.mark.parametrize("other", [2, 3])
+def test_modes_agree_and_split_stepping(db, other):
+    # kernels vs persistent / deferred, and db_step(a); db_step(b) == db_step(a + b) (graph replay + remainder)
     cfg = db_inputs.config(0, scale=0.3)
     a = db.Sim.db_create(cfg["net"], cfg["sim"], seed=5, dyn_seed=2, exec_mode=1)
-    b = db.Sim.db_create(cfg["net"], cfg["sim"], seed=5, dyn_seed=2, exec_mode=2)
+    b = db.Sim.db_create(cfg["net"], cfg["sim"], seed=5, dyn_seed=2, exec_mode=other)
+    assert b.db_get_counters()["exec_mode"] == other
     a.db_step(100)
     for n in (1, 31, 33, 35):
         b.db_step(n)
