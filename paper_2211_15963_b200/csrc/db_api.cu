@@ -169,6 +169,10 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     d.scale = (float)std::ldexp(1.0, -sp->S);
     d.wscale = (float)std::ldexp(1.0, sp->S);
     d.seed_lo = (uint32_t)sp->dyn_seed; d.seed_hi = (uint32_t)(sp->dyn_seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        d.rk[2 * r] = d.seed_lo + (uint32_t)r * 0x9E3779B9u;
+        d.rk[2 * r + 1] = d.seed_hi + (uint32_t)r * 0xBB67AE85u;
+    }
     d.window_steps = sp->window_steps;
     d.max_windows = sp->max_windows ? sp->max_windows : 4096u;
     if (d.max_windows < 8) return fail(sim, DB_EINVAL, "max_windows must be >= 8");

@@ -54,6 +54,7 @@ struct SimDev {                      // passed by value to every kernel
     float scale;                     // 2^-S
     float wscale;                    // 2^S
     uint32_t seed_lo, seed_hi;
+    uint32_t rk[20];                 // Philox round keys of the dynamics seed: (k0, k1) + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
     // neuron state, structure of arrays
     float* V;                        // [Npad]
     float* g;                        // [4][Npad]

@@ -30,6 +30,19 @@ __host__ __device__ __forceinline__ uint4 philox4x32_10(uint4 ctr, uint32_t k0, 
     return ctr;
 }
 
+// Same function with the ten round keys taken from a table (kernel parameters: they become
+// constant-bank operands of the xor, and the key schedule costs nothing per draw).
+__device__ __forceinline__ uint4 philox4x32_10_rk(uint4 ctr, const uint32_t (&rk)[20]) {
+    constexpr uint32_t kMulA = 0xD2511F53u, kMulB = 0xCD9E8D57u;
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t hiA = __umulhi(kMulA, ctr.x), loA = kMulA * ctr.x;
+        const uint32_t hiB = __umulhi(kMulB, ctr.z), loB = kMulB * ctr.z;
+        ctr = make_uint4(hiB ^ ctr.y ^ rk[2 * round], loB, hiA ^ ctr.w ^ rk[2 * round + 1], loA);
+    }
+    return ctr;
+}
+
 __host__ __device__ __forceinline__ uint4 keyed_draw(uint32_t seed_lo, uint32_t seed_hi, uint32_t stream,
                                                      uint64_t a, uint64_t b) {
     return philox4x32_10(make_uint4((uint32_t)a, (uint32_t)(a >> 32) | (stream << 24),

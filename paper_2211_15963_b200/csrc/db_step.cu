@@ -357,8 +357,13 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
             for (int q = 0; q < 4; ++q) {
                 if (u == 0) {           // Poisson background joins the AMPA arrivals (R14)
                     // k = #{m < M : u >= T_m}; thresholds increase, so the first three decide almost always
+                    // m2.y / z / w hold 2^32 - T_m: u >= T_m is the carry of u + (2^32 - T_m)
                     const uint4 m2 = s_tc[tp[q]].m2;
-                    unsigned k = (unsigned)(rw[q] >= m2.y) + (unsigned)(rw[q] >= m2.z) + (unsigned)(rw[q] >= m2.w);
+                    unsigned k, scratch;
+                    asm("add.cc.u32 %1, %2, %3;\n\taddc.u32 %0, 0, 0;\n\t"
+                        "add.cc.u32 %1, %2, %4;\n\taddc.u32 %0, %0, 0;\n\t"
+                        "add.cc.u32 %1, %2, %5;\n\taddc.u32 %0, %0, 0;"
+                        : "=r"(k), "=r"(scratch) : "r"(rw[q]), "r"(m2.y), "r"(m2.z), "r"(m2.w));
                     if (k == 3u) {
                         if (m2.x > 3u) { while (k < m2.x && rw[q] >= s_T[tp[q]][k]) ++k; }
                         else k = m2.x;  // padded thresholds (u = 0xFFFFFFFF) do not count
@@ -434,8 +439,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     int32_t* slot = p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
     // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
     uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
-    if (kB) rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)),
-                                p.seed_lo, p.seed_hi);
+    if (kB) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
     cp_async_wait_all();
     const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
     const uint2 rt_bits = lds64(sg.srt);
@@ -705,8 +709,8 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
         for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(tc.G[u], tc.E[u], tc.alpha[u], 0.0f);
         r.m0 = make_float4(tc.neg_gL, tc.VL, tc.kappa, tc.Iext);
         r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
-        r.m2 = make_uint4((unsigned)tc.M, tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu, tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu,
-                          tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu);
+        r.m2 = make_uint4((unsigned)tc.M, 0u - (tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu), 0u - (tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu),
+                          0u - (tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu));   // negated thresholds (carry trick in neuron_group)
         s_tc[t] = r;
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
@@ -806,8 +810,8 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         for (int u = 0; u < 4; ++u) r.rec[u] = make_float4(tc.G[u], tc.E[u], tc.alpha[u], 0.0f);
         r.m0 = make_float4(tc.neg_gL, tc.VL, tc.kappa, tc.Iext);
         r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
-        r.m2 = make_uint4((unsigned)tc.M, tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu, tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu,
-                          tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu);
+        r.m2 = make_uint4((unsigned)tc.M, 0u - (tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu), 0u - (tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu),
+                          0u - (tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu));   // negated thresholds (carry trick in neuron_group)
         s_tc[t] = r;
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
@@ -836,8 +840,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int grp = task * 32 + (int)lane;
         const int i0 = grp * 4;
         // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
-        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)),
-                                        p.seed_lo, p.seed_hi);
+        const uint4 rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
         cp_async_wait_all();
         const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
         const uint2 rt_bits = lds64(sg.srt);
