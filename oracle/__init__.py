@@ -28,7 +28,8 @@ def build(force: bool = False) -> str:
 class TypeParams(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext")] + [
         ("G", C.c_double * 4), ("E", C.c_double * 4), ("tau_ms", C.c_double * 4),
-        ("bg_rate_hz", C.c_double), ("bg_weight", C.c_double)]
+        ("bg_rate_hz", C.c_double), ("bg_weight", C.c_double),
+        ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double)]
 
 
 class SimParams(C.Structure):
@@ -85,6 +86,9 @@ def lib():
         L.orc_sim_set_state.argtypes = [C.c_void_p] * 4
         L.orc_sim_get_ring.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_sim_set_ring.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_sim_get_iou.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_sim_set_iou.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_normal_table.argtypes = [C.c_void_p]
         L.orc_sim_region_counts.restype = C.c_int64
         L.orc_sim_region_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
         L.orc_sim_log_arrivals.argtypes = [C.c_void_p, C.c_int32]
@@ -241,6 +245,8 @@ def _sim_params(d: dict) -> SimParams:
         q = p.type[i]
         for k in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext", "bg_rate_hz", "bg_weight"):
             setattr(q, k, float(t[k]))
+        for k in ("ou_mu", "ou_sigma", "ou_tau_ms"):          # OU background current, off by default
+            setattr(q, k, float(t.get(k, 0.0)))
         for k in ("G", "E", "tau_ms"):
             for u in range(4):
                 getattr(q, k)[u] = float(t[k][u])
@@ -310,6 +316,16 @@ class OracleSim:
         ref = np.ascontiguousarray(ref, np.int32)
         lib().orc_sim_set_state(self.h, _p(V), _p(g), _p(ref))
 
+    def iou(self):
+        out = np.zeros(self.N, np.float64)
+        lib().orc_sim_get_iou(self.h, _p(out))
+        return out
+
+    def set_iou(self, v):
+        v = np.ascontiguousarray(v, np.float64)
+        assert v.shape == (self.N,)
+        lib().orc_sim_set_iou(self.h, _p(v))
+
     def ring(self):
         r = np.zeros((self.D, self.N, 4), np.int32)
         lib().orc_sim_get_ring(self.h, _p(r))
@@ -339,6 +355,13 @@ class OracleSim:
         a = np.zeros(n, np.int32)
         lib().orc_sim_get_arrivals(self.h, _p(a))
         return a.reshape(-1, self.N, 4)
+
+
+def normal_table() -> np.ndarray:
+    """The 65536 standard-normal quantiles (fp32) the OU increments are drawn from."""
+    tab = np.zeros(65536, np.float32)
+    lib().orc_normal_table(_p(tab))
+    return tab
 
 
 def dense_arrivals(net: dict, S: int, spikes: np.ndarray) -> np.ndarray:

@@ -79,7 +79,8 @@ enum : uint32_t {
     STREAM_SYN = 4,    // per-synapse weight / delay / receptor
     STREAM_REGION = 5, // region sizes and region matrix (host-side normals)
     STREAM_INTER = 6,  // source-region choice of an inter-region input
-    STREAM_DEG = 7     // out-degree of a neuron (out-degree mode)
+    STREAM_DEG = 7,    // out-degree of a neuron (out-degree mode)
+    STREAM_OU = 8      // Gaussian increments of the OU background current
 };
 
 u32x4 draw(uint64_t seed, uint32_t stream, uint64_t a, uint64_t b) {
@@ -197,6 +198,10 @@ struct orc_type_params {
     double tau_ms[4];   // tau_u
     double bg_rate_hz;  // Poisson background rate per neuron (R14)
     double bg_weight;   // its weight, delivered to AMPA
+    // OU background current (main Eq.(1), SI Eq.(4); mu = 0.66, sigma = 0.12, tau = 10 in
+    // Ext. Table 2), read per R3: I += (mu - I) dt/tau + sigma sqrt(2 dt/tau) xi, xi ~ N(0,1).
+    // ou_tau_ms = 0 switches it off.
+    double ou_mu, ou_sigma, ou_tau_ms;
 };
 
 struct orc_sim_params {
@@ -540,6 +545,8 @@ struct TypeConst {
     int32_t R;              // refractory steps
     int32_t wq_bg;
     uint32_t T[POISSON_MAX]; int M;
+    bool ou = false;        // OU background current on
+    real ou_mu = 0, ou_a = 0, ou_s = 0;   // mean, dt/tau, sigma sqrt(2 dt/tau): formed in double, rounded once
 };
 
 template <typename real>
@@ -556,6 +563,8 @@ struct Sim {
     std::vector<uint8_t> delay, rec;
     // state
     std::vector<real> V, g;           // g[4*i+u]
+    std::vector<real> Iou;            // OU background current (R3)
+    std::vector<float> ntab;          // 65536 standard-normal quantiles, Phi^-1((q + 0.5) / 65536), as fp32
     std::vector<int32_t> ref;
     std::vector<int32_t> ring;        // ring[(slot*N + i)*4 + u]
     // outputs
@@ -595,6 +604,16 @@ struct Sim {
             real t2 = (c.G[2] * gi[2]) * (c.E[2] - v);
             real t3 = (c.G[3] * gi[3]) * (c.E[3] - v);
             real I = (((t0 + t1) + t2) + t3) + c.Iext;
+            // 4b. OU background current (SI Eq.(4); R3): the membrane step sees I_ou(t), then
+            //     I_ou(t+dt) = I_ou + ((mu - I_ou) dt/tau + sigma sqrt(2 dt/tau) xi); one Philox block serves 4
+            //     neurons, xi = table[top 16 bits of the word]
+            if (c.ou) {
+                real io = Iou[(size_t)i];
+                I = I + io;
+                uint32_t uo = draw(seed, STREAM_OU, (uint64_t)(i >> 2), n).w[i & 3];
+                real xi = (real)ntab[uo >> 16];
+                Iou[(size_t)i] = io + ((c.ou_mu - io) * c.ou_a + c.ou_s * xi);
+            }
             // 5. membrane step: CV equation with Euler step (SI Eq.(5); R1)
             real leak = (-c.gL) * (v - c.VL);
             real vn = v + c.kappa * (leak + I);
@@ -656,8 +675,18 @@ Sim<real>* sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
         c.R = (int32_t)std::lrint(q.Tref_ms / p->dt_ms);
         c.wq_bg = (int32_t)std::lrint(q.bg_weight * std::ldexp(1.0, p->S));
         c.M = poisson_thresholds(q.bg_rate_hz * p->dt_ms * 1e-3, c.T);
+        if (q.ou_tau_ms > 0) {
+            c.ou = true;
+            c.ou_mu = (real)q.ou_mu;
+            c.ou_a = (real)(p->dt_ms / q.ou_tau_ms);
+            c.ou_s = (real)(q.ou_sigma * std::sqrt(2.0 * p->dt_ms / q.ou_tau_ms));
+        }
         s->tc.push_back(c);
     }
+    s->ntab.resize(65536);
+    for (int q = 0; q < 65536; ++q) s->ntab[(size_t)q] = (float)norm_ppf(((double)q + 0.5) / 65536.0);
+    s->Iou.resize((size_t)N);
+    for (int64_t i = 0; i < N; ++i) s->Iou[(size_t)i] = s->tc[ntype[i]].ou ? s->tc[ntype[i]].ou_mu : (real)0;
     s->V.resize((size_t)N); s->g.assign((size_t)N * 4, (real)0); s->ref.assign((size_t)N, 0);
     s->ring.assign((size_t)p->D * (size_t)N * 4, 0);
     for (int64_t i = 0; i < N; ++i) {
@@ -685,6 +714,20 @@ void* orc_sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
     return h;
 }
 void orc_sim_destroy(void* hv) { Handle* h = (Handle*)hv; delete h->f; delete h->d; delete h; }
+
+void orc_sim_get_iou(void* hv, double* out) {
+    Handle* h = (Handle*)hv;
+    const int64_t N = h->fp64 ? h->d->N : h->f->N;
+    for (int64_t i = 0; i < N; ++i) out[i] = h->fp64 ? h->d->Iou[(size_t)i] : (double)h->f->Iou[(size_t)i];
+}
+void orc_sim_set_iou(void* hv, const double* in) {
+    Handle* h = (Handle*)hv;
+    const int64_t N = h->fp64 ? h->d->N : h->f->N;
+    for (int64_t i = 0; i < N; ++i) { if (h->fp64) h->d->Iou[(size_t)i] = in[i]; else h->f->Iou[(size_t)i] = (float)in[i]; }
+}
+void orc_normal_table(float* tab /*[65536]*/) {
+    for (int q = 0; q < 65536; ++q) tab[q] = (float)norm_ppf(((double)q + 0.5) / 65536.0);
+}
 
 void orc_sim_step(void* hv, int64_t n_steps) {
     Handle* h = (Handle*)hv;

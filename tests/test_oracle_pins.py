@@ -364,3 +364,77 @@ def test_fp32_mode_tracks_fp64_mode_early(oracle_mod):
     assert np.array_equal(a.spikes()[1], b.spikes()[1])
     assert np.max(np.abs(a.state()[0] - b.state()[0])) < 1e-3
     assert np.array_equal(a.ring(), b.ring())
+
+
+# ------------------------------------------------------------------ OU background current
+def _ou_net(N):
+    return dict(N=N, E=0, n_regions=1, region_start=np.array([0, N]), ntype=np.zeros(N, np.uint8),
+                row_ptr=np.zeros(N + 1, np.int64), tgt=np.zeros(0, np.int32), w=np.zeros(0, np.float32),
+                delay=np.zeros(0, np.uint8), rec=np.zeros(0, np.uint8))
+
+
+def _ou_sim(mu, sigma, tau_ms, dt_ms=0.1, **kw):
+    t = db_inputs.type_params(bg_weight=0.0, bg_rate_hz=0.0)
+    t.update(ou_mu=mu, ou_sigma=sigma, ou_tau_ms=tau_ms, **kw)
+    return db_inputs.sim_params(dt_ms=dt_ms, types=[t])
+
+
+def test_normal_table_is_the_standard_normal_quantile_function(oracle_mod):
+    from scipy.stats import norm
+    tab = oracle_mod.normal_table()
+    want = norm.ppf((np.arange(65536) + 0.5) / 65536.0)
+    assert np.all(np.abs(tab - want) <= 2e-7 * np.maximum(1.0, np.abs(want)))      # fp32 rounding of the double quantile
+    assert np.all(np.diff(tab) > 0) and np.array_equal(tab, -tab[::-1])             # strictly increasing, antisymmetric
+    assert abs(float(tab.astype(np.float64).mean())) < 1e-9
+    assert abs(float((tab.astype(np.float64) ** 2).mean()) - 1.0) < 2e-4          # variance of the 65536-point quantisation
+
+
+def test_ou_without_noise_relaxes_geometrically_to_mu(oracle_mod):
+    # sigma = 0: I_n = mu + (I_0 - mu)(1 - dt/tau)^n, the Euler map of dI/dt = (mu - I)/tau (main Eq.(1))
+    mu, tau, dt = 0.66, 10.0, 0.1
+    o = oracle_mod.OracleSim(_ou_sim(mu, 0.0, tau, dt), _ou_net(3), 1, fp64=True)
+    o.set_iou(np.array([0.0, 2.0, mu]))
+    n = 400
+    o.step(n)
+    want = mu + (np.array([0.0, 2.0, mu]) - mu) * (1.0 - dt / tau) ** n
+    assert np.allclose(o.iou(), want, rtol=0, atol=1e-12)
+
+
+def test_ou_stationary_mean_sd_and_autocorrelation(oracle_mod):
+    # Ext. Table 2: mu = 0.66, sigma = 0.12, tau = 10.  The discrete map has stationary mean mu,
+    # variance sigma^2 (2a)/(1-(1-a)^2) = sigma^2/(1 - a/2), a = dt/tau, and lag-k autocorrelation (1-a)^k ~ e^{-k dt/tau}
+    mu, sigma, tau, dt = 0.66, 0.12, 10.0, 1.0
+    N, burn, T = 4000, 200, 400
+    sim = _ou_sim(mu, sigma, tau, dt, Vth=1e9)                  # no spikes: the membrane is irrelevant here
+    o = oracle_mod.OracleSim(sim, _ou_net(N), 7, fp64=True)
+    assert np.array_equal(o.iou(), np.full(N, mu))               # starts at its mean
+    o.step(burn)
+    xs = []
+    for _ in range(T):
+        xs.append(o.iou().copy())
+        o.step(1)
+    x = np.array(xs)                                             # [T][N]
+    a = dt / tau
+    sd_want = sigma / np.sqrt(1.0 - a / 2.0)
+    assert abs(x.mean() - mu) < 4 * sd_want / np.sqrt(N * T * a)            # about a*T*N independent samples
+    assert abs(x.std() / sd_want - 1.0) < 0.02
+    for lag in (1, 5, 10, 20):
+        c = np.mean((x[:-lag] - mu) * (x[lag:] - mu)) / x.var()
+        assert abs(c - (1.0 - a) ** lag) < 0.02
+        assert abs(c - np.exp(-lag * dt / tau)) < 0.03
+
+
+def test_ou_current_enters_the_membrane_equation_as_a_current(oracle_mod):
+    # sigma = 0 and I_ou(0) = mu: a constant current mu, so V follows the constant-current closed form
+    # V_n = V_inf + (V_0 - V_inf)(1 - dt gL / C)^n with V_inf = VL + mu / gL (below threshold here)
+    mu, dt = 0.5, 0.1
+    sim = _ou_sim(mu, 0.0, 10.0, dt)
+    tp = sim["types"][0]
+    o = oracle_mod.OracleSim(sim, _ou_net(1), 1, fp64=True)
+    V0 = o.state()[0][0]
+    n = 300
+    o.step(n)
+    Vinf = tp["VL"] + mu / tp["gL"]
+    assert Vinf < tp["Vth"]
+    want = Vinf + (V0 - Vinf) * (1.0 - dt * tp["gL"] / tp["C"]) ** n
+    assert abs(o.state()[0][0] - want) < 1e-10
