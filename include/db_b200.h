@@ -63,6 +63,10 @@ typedef struct db_type_params {
     double tau_ms[DB_N_RECEPTORS];  /* tau_u */
     double bg_rate_hz;              /* Poisson background rate per neuron (R14) */
     double bg_weight;               /* its weight; delivered to AMPA */
+    /* OU background current (main Eq.(1), SI Eq.(4); Ext. Table 2: mu 0.66, sigma
+     * 0.12, tau 10), read per R3: I += (mu - I) dt/tau + sigma sqrt(2 dt/tau) xi, xi ~ N(0,1) from a
+     * 65536-point quantile table; enters the membrane equation as a current.  ou_tau_ms = 0: off. */
+    double ou_mu, ou_sigma, ou_tau_ms;
 } db_type_params;
 
 /* Execution mode of db_step(). */
@@ -169,6 +173,7 @@ typedef struct db_phase_times {
 #define DB_FIELD_TYPE   6  /* uint8  [count] */
 #define DB_FIELD_RING   7  /* int32  [D][count][4] fixed-point arrivals, slot = step mod D */
 #define DB_FIELD_OUTDEG 8  /* int32  [count], out-degree = length of the neuron's destination list (read only) */
+#define DB_FIELD_IOU    9  /* float  [count], OU background current (zeros when no type uses it) */
 
 /* a0: generate the network on the device from `spec` (seed keys every draw of
  * the generator), build the CSR and initialise the state (V0 keyed by

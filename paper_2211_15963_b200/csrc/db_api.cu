@@ -124,6 +124,13 @@ int32_t make_type_consts(db_sim* sim, const db_sim_params& sp, TypeConst* tc) {
         }
         if (!saturated) return fail(sim, DB_EINVAL, "bg_rate_hz * dt too large for the Poisson table");
         c.M = M;
+        if (!(q.ou_tau_ms >= 0) || !(q.ou_sigma >= 0)) return fail(sim, DB_EINVAL, "OU parameters out of range");
+        if (q.ou_tau_ms > 0) {          // OU background current (R3): constants formed in double, rounded once
+            c.ou = 1;
+            c.ou_mu = (float)q.ou_mu;
+            c.ou_a = (float)(sp.dt_ms / q.ou_tau_ms);
+            c.ou_s = (float)(q.ou_sigma * std::sqrt(2.0 * sp.dt_ms / q.ou_tau_ms));
+        }
         tc[t] = c;
     }
     return DB_OK;
@@ -194,6 +201,18 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     if ((rc = alloc_zero(sim, &d.V, Np))) return rc;
     if ((rc = alloc_zero(sim, &d.g, 4 * Np))) return rc;
     if ((rc = alloc_zero(sim, &d.rt, Np))) return rc;
+    d.ou_on = 0;
+    for (int t = 0; t < sp->n_types; ++t) d.ou_on |= d.tc[t].ou;
+    if (d.ou_on) {                      // OU state and the table of standard-normal quantiles its increments come from
+        if ((rc = alloc_zero(sim, &d.Iou, Np))) return rc;
+        float* ntab = nullptr;
+        if ((rc = alloc_zero(sim, &ntab, 65536))) return rc;
+        std::vector<float> tab(65536);
+        for (int q = 0; q < 65536; ++q) tab[(size_t)q] = (float)std_normal_quantile(((double)q + 0.5) / 65536.0);
+        CK(cudaMemcpyAsync(ntab, tab.data(), 65536 * sizeof(float), cudaMemcpyHostToDevice, sim->stream));
+        CK(cudaStreamSynchronize(sim->stream));
+        d.ntab = ntab;
+    }
     if ((rc = alloc_zero(sim, &d.ring, (size_t)d.D * 4 * Np))) return rc;
     uint64_t cap = sp->raster_capacity ? sp->raster_capacity : (1ull << 24);
     cap = next_pow2(std::max<uint64_t>(cap, (uint64_t)N));
@@ -625,6 +644,10 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
     }
     case DB_FIELD_OUTDEG:
         CK(cudaMemcpy(dst, d.row_len + first, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;
+    case DB_FIELD_IOU:
+        if (d.ou_on) CK(cudaMemcpy(dst, d.Iou + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
+        else std::memset(dst, 0, (size_t)count * 4);
+        break;
     case DB_FIELD_RING: {
         // API slot j holds the arrivals of the step t in [n, n + D) with t mod D == j; device slot = t mod d.D
         Ctl c;
@@ -673,6 +696,9 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
         CK(cudaMemcpy(d.V + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
     case DB_FIELD_G_AMPA: case DB_FIELD_G_NMDA: case DB_FIELD_G_GABAA: case DB_FIELD_G_GABAB:
         CK(cudaMemcpy(d.g + (field - DB_FIELD_G_AMPA) * Np + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
+    case DB_FIELD_IOU:
+        if (!d.ou_on) return fail(sim, DB_ESTATE, "no neuron type uses the OU background current");
+        CK(cudaMemcpy(d.Iou + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
     case DB_FIELD_REF: {
         std::vector<uint16_t> t((size_t)count);
         CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));

@@ -17,7 +17,7 @@ constexpr int kRefMask = 0x0FFF;     // rt = type << 12 | refractory steps left
 
 // Philox streams
 constexpr uint32_t kStreamV0 = 1, kStreamBG = 2, kStreamSRC = 3, kStreamSYN = 4,
-                   kStreamREGION = 5, kStreamINTER = 6, kStreamDEG = 7;
+                   kStreamREGION = 5, kStreamINTER = 6, kStreamDEG = 7, kStreamOU = 8;
 
 struct TypeConst {                   // per neuron type, rounded once on the host
     float neg_gL, VL, Vth, Vreset, kappa, Iext;
@@ -26,6 +26,8 @@ struct TypeConst {                   // per neuron type, rounded once on the hos
     int32_t wq_bg;                   // fixed-point background weight
     int32_t M;                       // number of Poisson thresholds
     uint32_t T[kPoissonMax];
+    float ou_mu, ou_a, ou_s;         // OU background: mean, dt / tau, sigma sqrt(2 dt / tau) (0 when off)
+    int32_t ou;                      // OU background on for this type
 };
 
 struct alignas(128) Ctl {            // device-resident control block
@@ -59,6 +61,9 @@ struct SimDev {                      // passed by value to every kernel
     float* V;                        // [Npad]
     float* g;                        // [4][Npad]
     uint16_t* rt;                    // [Npad] type << 12 | ref
+    float* Iou;                      // [Npad] OU background current (allocated only if some type uses it)
+    const float* ntab;               // [65536] standard-normal quantiles (same condition)
+    int32_t ou_on;
     int32_t* ring;                   // [D][4][Npad] fixed-point arrivals
     // presynaptic-major CSR
     const int64_t* row_begin;        // [N] first synapse of row j (multiple of kRowAlign)

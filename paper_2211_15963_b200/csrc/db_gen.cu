@@ -18,6 +18,8 @@ namespace {
 
 double std_normal_cdf(double z) { return 0.5 * std::erfc(-z * 0.70710678118654752440); }
 
+}  // namespace
+
 // Inverse normal CDF: Newton iterations on erfc from a logistic starting guess.
 double std_normal_quantile(double p) {
     double z = 0.0;
@@ -40,6 +42,8 @@ double std_normal_quantile(double p) {
     }
     return z;
 }
+
+namespace {
 
 double normal_from_words(uint32_t u0, uint32_t u1) {     // Box-Muller, double
     const double a = ((double)u0 + 0.5) / 4294967296.0;

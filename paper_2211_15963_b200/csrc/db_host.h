@@ -31,6 +31,8 @@ struct GenHostTables {                 // distribution tables formed on the host
     int32_t K_intra = 0, K_inter = 0;
 };
 
+double std_normal_quantile(double p);   // inverse normal CDF (Newton on erfc), double precision
+
 bool gen_host_tables(const db_network_spec& spec, uint64_t seed, GenHostTables* out, std::string* err);
 
 struct GenAlloc { void* user; void* (*alloc)(void* user, size_t bytes); };

@@ -192,6 +192,7 @@ struct alignas(16) TypeSmem {        // TypeConst regrouped into 128-bit words f
     float4 m0;                       // neg_gL, VL, kappa, Iext
     float4 m1;                       // Vth, Vreset, R (int bits), wq_bg (int bits)
     uint4 m2;                        // M, T[0], T[1], T[2] (0xFFFFFFFF where m >= M)
+    float4 m3;                       // OU background: mu, dt / tau, sigma sqrt(2 dt / tau), on (int bits)
 };
 
 constexpr int kStageBytesPerThread = 9 * 16 + 8;   // ring x4, V, g x4 (16 B each), rt (8 B)
@@ -206,6 +207,11 @@ __device__ __forceinline__ unsigned ld_cg_u32(const unsigned* p) {
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
     unsigned long long r;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
+    float4 r;
+    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
 }
 __device__ __forceinline__ void st_cg_f4(float* p, float4 v) {
@@ -319,13 +325,14 @@ __device__ __forceinline__ void request_ring(const SimDev& p, const Stage& sg, c
 // is requested (ring planes only if kB).  tp0..tp3 are the neuron types; the caller passes the
 // same variable four times when they agree, which lets the constant loads (broadcast LDS.128)
 // be shared.  Operation order: DESIGN.md "Arithmetic contract".
-template <bool kB, bool kA, bool kClassic = false>
+template <bool kB, bool kA, bool kClassic = false, bool kOU = false>
 __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem* s_tc,
                                                  const uint32_t (*s_T)[kPoissonMax], const Stage& sg,
                                                  const int tp0, const int tp1, const int tp2, const int tp3,
                                                  const int i0, int32_t* slot, const int next_off,
                                                  const uint4 v_bits, const uint2 rt_bits, const uint4 rnd,
-                                                 unsigned& bg_acc) {
+                                                 unsigned& bg_acc, float4* iou = nullptr,
+                                                 const uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u)) {
     const size_t Np = (size_t)p.Npad;
     const int tp[4] = {tp0, tp1, tp2, tp3};
     const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
@@ -394,7 +401,17 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const float4 m0 = s_tc[tp[q]].m0, m1 = s_tc[tp[q]].m1;
-            const float Iq = __fadd_rn(I[q], m0.w);
+            float Iq = __fadd_rn(I[q], m0.w);
+            if (kOU) {                 // OU background current (R3): the membrane step sees I_ou(t); then
+                const float4 m3 = s_tc[tp[q]].m3;   // I_ou += (mu - I_ou) dt/tau + sigma sqrt(2 dt/tau) xi
+                if (__float_as_int(m3.w)) {
+                    float* io = reinterpret_cast<float*>(iou) + q;
+                    const uint32_t wo = (q == 0) ? rnd_ou.x : (q == 1) ? rnd_ou.y : (q == 2) ? rnd_ou.z : rnd_ou.w;
+                    const float xi = __ldg(p.ntab + (wo >> 16));
+                    Iq = __fadd_rn(Iq, *io);
+                    *io = __fadd_rn(*io, __fadd_rn(__fmul_rn(__fsub_rn(m3.x, *io), m3.y), __fmul_rn(m3.z, xi)));
+                }
+            }
             const float leak = __fmul_rn(m0.x, __fsub_rn(v[q], m0.y));
             float w = __fadd_rn(v[q], __fmul_rn(m0.z, __fadd_rn(leak, Iq)));
             if ((rt[q] & (unsigned)kRefMask) > 0u) { w = m1.y; rt[q] -= 1u; rt_changed = 1u; }
@@ -428,7 +445,7 @@ struct BlockShared {                 // small per-block scratch of the persisten
 // One 128-neuron task of one warp in unit (kB: B of step nB, kA: A of step nA).  next_off != 0:
 // distance (in neurons) to the warp's next task of this unit, whose planes are requested while
 // this one is consumed.
-template <bool kHalf, bool kHeavy, bool kB, bool kA>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU>
 __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, const uint32_t (*s_T)[kPoissonMax],
                                          BlockShared* bs, const Stage& sg, const unsigned long long nB,
                                          const unsigned long long nA, const int task, const unsigned lane,
@@ -440,6 +457,12 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
     uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
     if (kB) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
+    float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u);
+    if (kOU && kA) {                   // OU current of the four neurons and the words its increments come from
+        iou = ld_cg_f4(p.Iou + i0);
+        rnd_ou = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
+    }
     cp_async_wait_all();
     const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
     const uint2 rt_bits = lds64(sg.srt);
@@ -451,9 +474,10 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
     unsigned spike_bits;
     if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-        spike_bits = neuron_group<kB, kA>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
     else                                // a type boundary inside the group (rare)
-        spike_bits = neuron_group<kB, kA>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+    if (kOU && kA) st_cg_f4(p.Iou + i0, iou);
     cp_async_commit();
     if (!kA) return;
 
@@ -555,7 +579,7 @@ struct RunCtx {                      // per-thread constants of the persistent k
 };
 
 // Unit j of the launch (see the header comment): B of step n0 + j - 1 (if kB), A of step n0 + j (if kA).
-template <bool kHalf, bool kHeavy, bool kB, bool kA>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU>
 __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, const RunCtx& c, const TypeSmem* s_tc,
                                          const uint32_t (*s_T)[kPoissonMax], BlockShared* bs, const Stage& sg,
                                          const unsigned j, unsigned& bg_acc) {
@@ -572,7 +596,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         cp_async_commit();
         for (int task = c.task0; task < c.last; task += (int)c.n_warps) {
             const int next_off = (task + (int)c.n_warps < c.last) ? c.task_stride : 0;
-            run_task<kHalf, kHeavy, kB, kA>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
+            run_task<kHalf, kHeavy, kB, kA, kOU>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
         }
         if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
     }
@@ -695,7 +719,7 @@ __device__ __noinline__ void service_warp(const SimDev& p, const RunCfg& cfg, co
     }
 }
 
-template <bool kHalf, bool kHeavy>
+template <bool kHalf, bool kHeavy, bool kOU>
 __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ SimDev p, const RunCfg cfg) {
     extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
@@ -711,6 +735,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
         r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
         r.m2 = make_uint4((unsigned)tc.M, 0u - (tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu), 0u - (tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu),
                           0u - (tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu));   // negated thresholds (carry trick in neuron_group)
+        r.m3 = make_float4(tc.ou_mu, tc.ou_a, tc.ou_s, __int_as_float(tc.ou));
         s_tc[t] = r;
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
@@ -733,10 +758,10 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     if (c.warp == c.n_warps) { service_warp<kHeavy>(p, cfg, c, &bs); return; }
 
     if (c.task0 < c.last) { request_state(p, sg, c.i00); cp_async_commit(); }
-    run_unit<kHalf, kHeavy, false, true>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
+    run_unit<kHalf, kHeavy, false, true, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
     for (unsigned j = 1; j < cfg.n_steps; ++j)
-        run_unit<kHalf, kHeavy, true, true>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
-    run_unit<kHalf, kHeavy, true, false>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
+        run_unit<kHalf, kHeavy, true, true, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
+    run_unit<kHalf, kHeavy, true, false, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
 
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (c.lane == 0 && bg_warp)
@@ -798,6 +823,7 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
         }
 }
 
+template <bool kOU>
 __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_constant__ SimDev p, const RunCfg cfg) {
     extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
@@ -812,6 +838,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         r.m1 = make_float4(tc.Vth, tc.Vreset, __int_as_float(tc.R), __int_as_float(tc.wq_bg));
         r.m2 = make_uint4((unsigned)tc.M, 0u - (tc.M > 0 ? tc.T[0] : 0xFFFFFFFFu), 0u - (tc.M > 1 ? tc.T[1] : 0xFFFFFFFFu),
                           0u - (tc.M > 2 ? tc.T[2] : 0xFFFFFFFFu));   // negated thresholds (carry trick in neuron_group)
+        r.m3 = make_float4(tc.ou_mu, tc.ou_a, tc.ou_s, __int_as_float(tc.ou));
         s_tc[t] = r;
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
@@ -841,6 +868,12 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int i0 = grp * 4;
         // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
         const uint4 rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+        float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u);
+        if (kOU) {
+            iou = ld_cg_f4(p.Iou + i0);
+            rnd_ou = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+        }
         cp_async_wait_all();
         const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
         const uint2 rt_bits = lds64(sg.srt);
@@ -852,9 +885,10 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
         unsigned spike_bits;
         if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-            spike_bits = neuron_group<true, true, true>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc);
+            spike_bits = neuron_group<true, true, true, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
         else                            // a type boundary inside the group (rare)
-            spike_bits = neuron_group<true, true, true>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc);
+            spike_bits = neuron_group<true, true, true, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        if (kOU) st_cg_f4(p.Iou + i0, iou);
         cp_async_commit();
         if (__ballot_sync(0xffffffffu, spike_bits != 0)) emit_global(p, n, sb, i0, lane, spike_bits);
     }
@@ -877,6 +911,7 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
     p.V[i] = (i < p.N) ? __fadd_rn(c.Vreset, __fmul_rn(__fsub_rn(c.Vth, c.Vreset), U)) : 0.0f;
     for (int u = 0; u < 4; ++u) p.g[(size_t)u * p.Npad + i] = 0.0f;
     p.rt[i] = (uint16_t)(tp << 12);
+    if (p.ou_on) p.Iou[i] = (i < p.N && c.ou) ? c.ou_mu : 0.0f;   // the OU current starts at its mean
 }
 
 // ===========================================================================
@@ -1138,14 +1173,16 @@ void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg);
 cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_update_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+        cudaError_t e = cudaFuncSetAttribute(k_update_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_update_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     int grid = 0, threads = 0;
     RunCfg cfg{};
     run_shape(p, n_sm, &grid, &threads, &cfg);
-    k_update_stream<<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);      // no service warp here
+    if (p.ou_on) k_update_stream<true><<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);      // no service warp here
+    else         k_update_stream<false><<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);
     return cudaGetLastError();
 }
 
@@ -1191,8 +1228,12 @@ void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg) 
 }
 
 static const void* run_fn(const SimDev& p, bool heavy) {
-    if (p.w_fp16) return heavy ? (const void*)k_run<true, true> : (const void*)k_run<true, false>;
-    return heavy ? (const void*)k_run<false, true> : (const void*)k_run<false, false>;
+    if (p.ou_on) {
+        if (p.w_fp16) return heavy ? (const void*)k_run<true, true, true> : (const void*)k_run<true, false, true>;
+        return heavy ? (const void*)k_run<false, true, true> : (const void*)k_run<false, false, true>;
+    }
+    if (p.w_fp16) return heavy ? (const void*)k_run<true, true, false> : (const void*)k_run<true, false, false>;
+    return heavy ? (const void*)k_run<false, true, false> : (const void*)k_run<false, false, false>;
 }
 
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok) {

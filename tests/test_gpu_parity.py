@@ -177,6 +177,38 @@ def test_modes_agree_and_split_stepping(db, other):
     assert np.array_equal(sa, sb) and np.array_equal(ia, ib) and len(ia) > 20
 
 
+@pytest.mark.parametrize("mode", MODES)
+def test_ou_background_current(db, oracle_mod, mode):
+    # the paper's OU drive (sigma 0.12, tau 10 ms as printed; mu 0.85 instead of 0.66 so that V_inf = VL + mu / gL = -46.7 mV lies above
+    # threshold and the type fires within the 40 ms of the test) on one type, Poisson drive on the other; raster, state and I_ou bit-identical to the oracle
+    sim = db_inputs.sim_params()
+    a = db_inputs.type_params(bg_weight=0.0, bg_rate_hz=0.0)
+    a.update(ou_mu=0.85, ou_sigma=0.12, ou_tau_ms=10.0)
+    b = db_inputs.type_params(bg_weight=0.02)
+    sim["types"] = [a, b]
+    N = 2000 + 77
+    net = db_inputs.random_csr(N=N, mean_outdeg=30, seed=11)
+    g, o = _pair(db, oracle_mod, sim, net, mode)
+    assert np.array_equal(g.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32))      # starts at mu (type 0) / 0
+    rng = np.random.default_rng(3)
+    I0 = np.where(net["ntype"] == 0, rng.normal(0.85, 0.12, N), 0.0).astype(np.float32)
+    g.db_write_state(db.FIELD_IOU, I0); o.set_iou(I0.astype(np.float64))
+    for upto in (1, 2, 40, 400):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        assert np.array_equal(g.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32))
+        dv, dg = _compare_state(g, o)
+        assert dv == 0.0 and dg == 0.0
+        assert np.array_equal(_ring_oracle_layout(g), o.ring())
+    n = _compare_raster(g, o, 400)
+    ids = g.db_read_spikes(0, 400)[1]
+    assert np.count_nonzero(net["ntype"][ids] == 0) > 50 and np.count_nonzero(net["ntype"][ids] == 1) > 10
+    I = g.db_read_state(db.FIELD_IOU)
+    assert np.all(I[net["ntype"] == 1] == 0.0) and abs(I[net["ntype"] == 0].mean() - 0.85) < 0.03
+    with pytest.raises(db.DbError):                              # no OU type: the field cannot be written
+        h = db.Sim.db_create_from_csr(db_inputs.sim_params(), net)
+        h.db_write_state(db.FIELD_IOU, I0)
+
+
 def test_read_spikes_ranges_and_errors(db):
     cfg = db_inputs.config(0, scale=0.2)
     s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=1, raster_capacity=1)   # capacity rounds up to N
