@@ -43,14 +43,15 @@ def type_params(bg_weight: float = BG_WEIGHT_FOR_RATE[7], bg_rate_hz: float = 10
 
 def sim_params(dt_ms: float = 0.1, S: int = 22, D: int = 32, window_steps: int = 10,
                rate_hz: int = 7, g_scale: float = 1.0, types: list | None = None,
-               bg_drive: float | None = None) -> dict:
+               bg_drive: float | None = None, spike_bin_steps: int = 1) -> dict:
     if types is None:
         # G scales with 100/K (R20); the background enters through G_AMPA too, so its
         # weight is divided by the same factor to keep the drive fixed.
         drive = BG_WEIGHT_FOR_RATE[rate_hz] if bg_drive is None else bg_drive
         t = type_params(drive / g_scale, g_scale=g_scale)
         types = [t, copy.deepcopy(t)]            # exc and inh share constants (R13)
-    return dict(dt_ms=dt_ms, S=S, D=D, window_steps=window_steps, types=types)
+    # spike_bin_steps: the paper's time bin b_t for transferring spikes (1 ms at dt = 0.1 ms: 10), R29
+    return dict(dt_ms=dt_ms, S=S, D=D, window_steps=window_steps, types=types, spike_bin_steps=spike_bin_steps)
 
 
 def _net(**kw) -> dict:

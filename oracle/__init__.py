@@ -34,7 +34,7 @@ class TypeParams(C.Structure):
 
 class SimParams(C.Structure):
     _fields_ = [("dt_ms", C.c_double), ("S", C.c_int32), ("D", C.c_int32), ("window_steps", C.c_int32),
-                ("n_types", C.c_int32), ("type", TypeParams * 4)]
+                ("n_types", C.c_int32), ("type", TypeParams * 4), ("spike_bin_steps", C.c_int32)]
 
 
 class NetSpec(C.Structure):
@@ -241,6 +241,7 @@ def _sim_params(d: dict) -> SimParams:
     p = SimParams()
     p.dt_ms, p.S, p.D, p.window_steps = d["dt_ms"], d["S"], d["D"], d["window_steps"]
     p.n_types = len(d["types"])
+    p.spike_bin_steps = int(d.get("spike_bin_steps", 1))      # time bin b_t for transferring spikes (R29), in steps
     for i, t in enumerate(d["types"]):
         q = p.type[i]
         for k in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext", "bg_rate_hz", "bg_weight"):

@@ -211,6 +211,10 @@ struct orc_sim_params {
     int32_t window_steps; // region-rate window (R24)
     int32_t n_types;
     orc_type_params type[4];
+    // Time bin for transferring spikes, b_t, in steps (SI "Numerical method"; the paper sets
+    // b_t = 1 ms even at dt = 0.1 ms).  Reading R29: A_j(t) = 1 only at the bin boundaries t = k b_t,
+    // for the neurons that fired in (t - b_t, t].  0 or 1: every step is a boundary.
+    int32_t spike_bin_steps;
 };
 
 struct orc_net_spec {
@@ -553,6 +557,8 @@ template <typename real>
 struct Sim {
     int64_t N = 0, E = 0;
     int D = 0, S = 0, window = 0, n_regions = 1;
+    int bin = 1;                      // b_t in steps (R29)
+    std::vector<int32_t> A;           // neurons that fired in the current time bin: the non-zero A_j of its boundary
     uint64_t seed = 0;
     uint64_t step = 0;
     std::vector<TypeConst<real>> tc;
@@ -635,15 +641,25 @@ struct Sim {
             while (r + 1 < n_regions && region_start[(size_t)r + 1] <= j) ++r;
             region_count[win * (size_t)n_regions + (size_t)r] += 1;
         }
-        // 9. push delivery along the destination list (Alg. 2 lines 3-4)
+        // 9. accumulated spikes A_j (SI "Numerical method"; R29): a neuron that fires inside the time
+        //    bin (t - b_t, t] is transferred at the boundary t = k b_t, once (A_j is 0 or 1).  In steps: the bin
+        //    of step n closes at the end of the step n with (n + 1) mod b_t = 0; b_t = 1 step is the plain
+        //    scheme (every step a boundary).
         for (int32_t j : L) {
-            for (int64_t s = row_ptr[(size_t)j]; s < row_ptr[(size_t)j + 1]; ++s) {
-                int32_t wq = (int32_t)std::lrintf(w[(size_t)s] * (float)std::ldexp(1.0, S));
-                size_t sl = (size_t)((n + delay[(size_t)s]) % (uint64_t)D);
-                int32_t* cell = &ring[(sl * (size_t)N + (size_t)tgt[(size_t)s]) * 4 + rec[(size_t)s]];
-                *cell = (int32_t)((uint32_t)*cell + (uint32_t)wq);      // two's-complement wrap
+            A.push_back(j);
+            n_events += (uint64_t)(row_ptr[(size_t)j + 1] - row_ptr[(size_t)j]);   // counted when the spike is emitted
+        }
+        if ((n + 1) % (uint64_t)bin == 0) {
+            // push delivery along the destination lists (Alg. 2 lines 3-4), w A_j(t) of Eq.(3)
+            for (int32_t j : A) {
+                for (int64_t s = row_ptr[(size_t)j]; s < row_ptr[(size_t)j + 1]; ++s) {
+                    int32_t wq = (int32_t)std::lrintf(w[(size_t)s] * (float)std::ldexp(1.0, S));
+                    size_t sl = (size_t)((n + delay[(size_t)s]) % (uint64_t)D);
+                    int32_t* cell = &ring[(sl * (size_t)N + (size_t)tgt[(size_t)s]) * 4 + rec[(size_t)s]];
+                    *cell = (int32_t)((uint32_t)*cell + (uint32_t)wq);      // two's-complement wrap
+                }
             }
-            n_events += (uint64_t)(row_ptr[(size_t)j + 1] - row_ptr[(size_t)j]);
+            A.clear();
         }
         step += 1;
     }
@@ -657,6 +673,7 @@ Sim<real>* sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
     Sim<real>* s = new Sim<real>();
     s->N = N; s->E = row_ptr[N]; s->D = p->D; s->S = p->S; s->window = p->window_steps;
     s->seed = seed; s->n_regions = n_regions;
+    s->bin = p->spike_bin_steps > 1 ? p->spike_bin_steps : 1;
     s->ntype.assign(ntype, ntype + N);
     s->region_start.assign(region_start, region_start + n_regions + 1);
     s->row_ptr.assign(row_ptr, row_ptr + N + 1);

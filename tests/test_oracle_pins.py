@@ -326,6 +326,80 @@ def test_delivery_equals_dense_brute_force(oracle_mod):
     assert got.sum() + s.ring().astype(np.int64).sum() == int(row_sum[ids].sum())
 
 
+# ---- time bin for transferring spikes, b_t (SI "Numerical method"; R29)
+@pytest.mark.parametrize("B", [2, 10])
+def test_binned_transfer_equals_dense_definition_of_A(oracle_mod, B):
+    # A_j(t) = 1 iff t is a bin boundary and j fired in (t - b_t, t], written out densely from
+    # the raster in numpy; the delivered sums are then the dense matrix x delayed A vectors (Eq.(3), 2nd term)
+    net = db_inputs.random_csr(N=48, mean_outdeg=9, seed=4, max_delay=20)
+    t = db_inputs.type_params(bg_weight=0.02, bg_rate_hz=1000.0)
+    sim = db_inputs.sim_params(D=64, types=[t, dict(t)], spike_bin_steps=B)
+    s = oracle_mod.OracleSim(sim, net, seed=5)
+    s.log_arrivals(True)
+    T = 1000
+    s.step(T)
+    st, ids = s.spikes()
+    assert len(ids) > 200
+    spikes = np.zeros((T, 48), np.uint8)
+    spikes[st.astype(np.int64), ids] = 1
+    A = np.zeros_like(spikes)
+    for m in range(B - 1, T, B):                     # step m closes the bin (m - B, m]
+        A[m] = spikes[m - B + 1:m + 1].max(axis=0)
+    assert A.sum() == spikes.sum()                   # T_ref > b_t: nobody fires twice in a bin
+    dense = oracle_mod.dense_arrivals(net, sim["S"], A)
+    got = s.arrivals().astype(np.int64)
+    assert np.array_equal(got, dense)
+    plain = oracle_mod.dense_arrivals(net, sim["S"], spikes)
+    assert not np.array_equal(got, plain)            # and it is not the unbinned scheme
+    outdeg = np.diff(net["row_ptr"])
+    assert s.counters()["events"] == int(outdeg[ids].sum())
+
+
+@pytest.mark.parametrize("n_s", [0, 3, 9, 10, 17])
+def test_binned_transfer_timing_of_one_event(oracle_mod, n_s):
+    # neuron 0 fires in step n_s; with b_t = 10 steps the spike is transferred at the end of the step
+    # n_k = 10 floor(n_s / 10) + 9 and, over a synapse of delay d, read in step n_k + d
+    B, d, w, rec = 10, 3, 0.0123, 0
+    t = db_inputs.type_params(bg_weight=0.0, bg_rate_hz=0.0)
+    sim = db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=B)
+    net = dict(N=2, n_regions=1, region_start=np.array([0, 2]), ntype=np.array([0, 0], np.uint8),
+               row_ptr=np.array([0, 1, 1], np.int64), tgt=np.array([1], np.int32),
+               w=np.array([w], np.float32), delay=np.array([d], np.uint8), rec=np.array([rec], np.uint8))
+    s = oracle_mod.OracleSim(sim, net, seed=1, fp64=True)
+    V, g, ref = s.state()
+    V[:] = t["VL"]
+    s.set_state(V, g, ref)
+    s.step(n_s)
+    V, g, ref = s.state()
+    V[0] = -40.0                                     # flagged in step n_s
+    s.set_state(V, g, ref)
+    na = (n_s // B) * B + B - 1 + d
+    wq = int(np.rint(np.float32(w) * np.float32(2.0 ** sim["S"])))
+    alpha = math.exp(-sim["dt_ms"] / t["tau_ms"][rec])
+    for n in range(n_s, na + 30):
+        s.step(1)
+        g1 = s.state()[1][1][rec]
+        if n < na:
+            assert g1 == 0.0
+        else:
+            want = wq * 2.0 ** -sim["S"] * alpha ** (n - na)
+            assert abs(g1 - want) <= 1e-13 * want
+    assert list(s.spikes()[0]) == [n_s]
+
+
+def test_bin_of_one_step_is_the_plain_scheme(oracle_mod):
+    net = db_inputs.random_csr(N=200, mean_outdeg=20, seed=2)
+    t = db_inputs.type_params(bg_weight=0.03)
+    out = []
+    for B in (0, 1):
+        sim = db_inputs.sim_params(types=[t, dict(t)], spike_bin_steps=B)
+        s = oracle_mod.OracleSim(sim, net, seed=5)
+        s.step(600)
+        out.append((s.spikes(), s.ring()))
+    assert np.array_equal(out[0][0][0], out[1][0][0]) and np.array_equal(out[0][0][1], out[1][0][1])
+    assert np.array_equal(out[0][1], out[1][1]) and len(out[0][0][1]) > 100
+
+
 def test_refractoriness_invariant(oracle_mod):
     net = db_inputs.random_csr(N=300, mean_outdeg=30, seed=9)
     s, sim, t = _driven_sim(oracle_mod, net, bg_weight=0.05)
