@@ -90,6 +90,13 @@ typedef struct db_sim_params {
     uint64_t raster_capacity; /* spikes kept for db_read_spikes (0 = default); older ones are overwritten */
     uint32_t max_windows;     /* region-rate windows kept (0 = default 4096) */
     int32_t  exec_mode;       /* DB_EXEC_* */
+    int32_t  spike_bin_steps; /* time bin b_t for transferring spikes, in steps (SI "Numerical method" P:L471-490:
+                                 b_t = 1 ms even at dt = 0.1 ms; reading R29): a neuron that fires in step n is
+                                 transferred at the end of its bin, step n_k = b_t floor(n / b_t) + b_t - 1, and a
+                                 synapse of delay d is read in step n_k + d.  0 or 1: every step is a boundary.
+                                 Needs b_t <= R + 1 of every type (A_j is 0 or 1) and largest delay + b_t - 1 < D;
+                                 DB_EXEC_KERNELS_DEFERRED falls back to DB_EXEC_KERNELS when b_t > 1.
+                                 DB_FIELD_RING already holds the pushes of the spikes of the open bin. */
 } db_sim_params;
 
 /* Device memory and stream plumbing supplied by the caller (the Python binding

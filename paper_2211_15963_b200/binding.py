@@ -43,7 +43,7 @@ class SimParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("dt_ms", C.c_double), ("S", C.c_int32), ("D", C.c_int32),
                 ("window_steps", C.c_int32), ("n_types", C.c_int32), ("type", TypeParams * 4),
                 ("dyn_seed", C.c_uint64), ("raster_capacity", C.c_uint64), ("max_windows", C.c_uint32),
-                ("exec_mode", C.c_int32)]
+                ("exec_mode", C.c_int32), ("spike_bin_steps", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -150,6 +150,7 @@ def _fill_sim_params(p: SimParams, d: dict, dyn_seed: int, exec_mode: int, raste
     p.raster_capacity = int(raster_capacity)
     p.max_windows = int(max_windows)
     p.exec_mode = int(exec_mode)
+    p.spike_bin_steps = int(d.get("spike_bin_steps", 1))
 
 
 class _TorchRuntime:

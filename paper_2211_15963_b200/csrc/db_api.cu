@@ -144,6 +144,7 @@ int32_t check_sim_params(db_sim* sim, const db_sim_params* sp) {
     if (sp->window_steps < 1) return fail(sim, DB_EINVAL, "window_steps must be >= 1");
     if (sp->n_types < 1 || sp->n_types > DB_MAX_TYPES) return fail(sim, DB_EINVAL, "n_types must be 1..4");
     if (sp->exec_mode < DB_EXEC_AUTO || sp->exec_mode > DB_EXEC_KERNELS_DEFERRED) return fail(sim, DB_EINVAL, "bad exec_mode");
+    if (sp->spike_bin_steps < 0 || sp->spike_bin_steps > 4096) return fail(sim, DB_EINVAL, "spike_bin_steps must be within 0..4096");
     return DB_OK;
 }
 
@@ -171,7 +172,10 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     d.Npad = (int32_t)(((N + kNeuronPad - 1) / kNeuronPad) * kNeuronPad);
     // internal ring depth: the persistent kernel lets blocks run up to two steps apart and needs
     // depth >= largest delay + 3 (db_step.cu); the API's D (slot = step mod D) is mapped on read / write
-    d.D = (max_delay + 3 > sp->D) ? 2 * sp->D : sp->D;
+    // (+ b_t - 1 with a time bin for transferring spikes: a row is pushed from the last step of its bin)
+    d.bin_steps = sp->spike_bin_steps > 1 ? sp->spike_bin_steps : 1;
+    if (max_delay + d.bin_steps - 1 >= sp->D) return fail(sim, DB_EINVAL, "largest delay + spike_bin_steps - 1 must be < D");
+    d.D = (max_delay + d.bin_steps + 2 > sp->D) ? 2 * sp->D : sp->D;
     d.S = sp->S;
     d.scale = (float)std::ldexp(1.0, -sp->S);
     d.wscale = (float)std::ldexp(1.0, sp->S);
@@ -186,6 +190,8 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     d.n_regions = n_regions;
     int32_t rc = make_type_consts(sim, *sp, d.tc);
     if (rc) return rc;
+    for (int t = 0; t < sp->n_types; ++t)          // A_j is 0 or 1: nobody may fire twice inside a bin
+        if (d.bin_steps > d.tc[t].R + 1) return fail(sim, DB_EINVAL, "spike_bin_steps must be <= round(Tref / dt) + 1 of every type");
 
     sim->region_start.assign(region_start, region_start + n_regions + 1);
     if (sim->region_start.front() != 0 || sim->region_start.back() != N)
@@ -302,7 +308,7 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int3
     const int near_max = std::min<int32_t>(31, near_hint);
     int r_min = d.tc[0].R;
     for (int t = 1; t < sim->params.n_types; ++t) r_min = std::min(r_min, d.tc[t].R);
-    const bool can_defer = near_max >= 2 &&
+    const bool can_defer = near_max >= 2 && d.bin_steps == 1 &&
         (uint64_t)d.N * (uint64_t)((near_max + r_min) / (r_min + 1)) <= sim->spike_cap;
     if (mode == DB_EXEC_AUTO)
         mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : (can_defer ? DB_EXEC_KERNELS_DEFERRED : DB_EXEC_KERNELS);

@@ -49,6 +49,23 @@ __device__ __forceinline__ void red_add_s32(int32_t* p, int32_t v) {
 // enough that no block (up to three steps ahead of the step being logged) writes into it yet.
 __device__ __forceinline__ unsigned window_clear_ahead(const int window_steps) { return 2u / (unsigned)window_steps + 1u; }
 
+// Step whose end transfers the spikes of step n: the last step of n's time bin (R29); n itself when b_t = 1.
+__device__ __forceinline__ unsigned long long transfer_step(const SimDev& p, const unsigned long long n) {
+    if (p.bin_steps == 1) return n;
+    const unsigned long long b = (unsigned long long)p.bin_steps;
+    return n - n % b + (b - 1ull);
+}
+
+// The same for the persistent kernel, low word only (slots are taken modulo the power of two D), from the phase of
+// the launch's first step (32-bit arithmetic: no 64-bit division on the spike path).
+template <bool kExt>
+__device__ __forceinline__ unsigned transfer_step_lo(const SimDev& p, const unsigned n_lo, const unsigned n0_lo,
+                                                     const unsigned phase0) {
+    if (!kExt || p.bin_steps == 1) return n_lo;
+    const unsigned b = (unsigned)p.bin_steps;
+    return n_lo - (phase0 + (n_lo - n0_lo)) % b + (b - 1u);
+}
+
 __device__ __forceinline__ int region_of(const SimDev& p, int i) {
     int lo = 0, hi = p.n_regions;                 // region_start[lo] <= i < region_start[hi]
     while (hi - lo > 1) {
@@ -141,7 +158,8 @@ __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev 
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
-    for (unsigned q = warp; q < n_work; q += n_warps) deliver_item<kHalf>(p, n, p.work[q], lane);
+    const unsigned long long nt = transfer_step(p, n);       // slot of a synapse = nt + delay
+    for (unsigned q = warp; q < n_work; q += n_warps) deliver_item<kHalf>(p, nt, p.work[q], lane);
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
@@ -174,7 +192,7 @@ __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev 
 // itself run a whole unit ahead: the barrier latency and the tail of the
 // deliveries are off the critical path.  Slots written by the fastest block
 // (up to n+1+d_max) must not meet the slot the slowest still consumes (n-1):
-// the ring depth is kept >= d_max + 3.
+// the ring depth is kept >= d_max + 3 (+ b_t - 1 with a time bin for transferring spikes).
 //
 // All global->SM traffic of the update is staged through shared memory with
 // cp.async (16 bytes per thread and plane: ring x4, V, g x4, rt), which keeps
@@ -439,13 +457,14 @@ struct BlockShared {                 // small per-block scratch of the persisten
     unsigned done[2];                // [unit & 1] update warps that have finished the unit (networks without heavy rows)
     unsigned grid_ok;                // units up to this one may start: the grid has closed everything they depend on
     unsigned heavy_n[2];             // [unit & 1] deferred heavy rows of the unit
+    unsigned n0_lo, bin_phase0;      // step at launch (low word) and its position inside its time bin (R29)
     int heavy_row[2][kHeavyListCap];
 };
 
 // One 128-neuron task of one warp in unit (kB: B of step nB, kA: A of step nA).  next_off != 0:
 // distance (in neurons) to the warp's next task of this unit, whose planes are requested while
 // this one is consumed.
-template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kExt>
 __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, const uint32_t (*s_T)[kPoissonMax],
                                          BlockShared* bs, const Stage& sg, const unsigned long long nB,
                                          const unsigned long long nA, const int task, const unsigned lane,
@@ -459,7 +478,8 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     if (kB) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
     float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u);
-    if (kOU && kA) {                   // OU current of the four neurons and the words its increments come from
+    const bool ou = kExt && kA && p.ou_on;
+    if (ou) {                          // OU current of the four neurons and the words its increments come from
         iou = ld_cg_f4(p.Iou + i0);
         rnd_ou = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
     }
@@ -474,10 +494,10 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
     unsigned spike_bits;
     if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        spike_bits = neuron_group<kB, kA, false, kExt>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
     else                                // a type boundary inside the group (rare)
-        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
-    if (kOU && kA) st_cg_f4(p.Iou + i0, iou);
+        spike_bits = neuron_group<kB, kA, false, kExt>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+    if (ou) st_cg_f4(p.Iou + i0, iou);
     cp_async_commit();
     if (!kA) return;
 
@@ -536,6 +556,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
         }                                                      // one region: added per block and unit (run_unit)
     // a3: the warp pushes the rows of its own spikes, one row at a time
     const unsigned nlo = (unsigned)nA;
+    const unsigned nto = transfer_step_lo<kExt>(p, nlo, bs->n0_lo, bs->bin_phase0);   // slot of a synapse = nto + delay
     while (any) {
         const int src = __ffs(any) - 1;
         any &= any - 1u;
@@ -554,7 +575,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
                     continue;
                 }
             }
-            deliver_span<kHalf>(p, nlo, (int64_t)b, l, lane);
+            deliver_span<kHalf>(p, nto, (int64_t)b, l, lane);
         }
     }
 }
@@ -579,7 +600,7 @@ struct RunCtx {                      // per-thread constants of the persistent k
 };
 
 // Unit j of the launch (see the header comment): B of step n0 + j - 1 (if kB), A of step n0 + j (if kA).
-template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kExt>
 __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, const RunCtx& c, const TypeSmem* s_tc,
                                          const uint32_t (*s_T)[kPoissonMax], BlockShared* bs, const Stage& sg,
                                          const unsigned j, unsigned& bg_acc) {
@@ -596,7 +617,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         cp_async_commit();
         for (int task = c.task0; task < c.last; task += (int)c.n_warps) {
             const int next_off = (task + (int)c.n_warps < c.last) ? c.task_stride : 0;
-            run_task<kHalf, kHeavy, kB, kA, kOU>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
+            run_task<kHalf, kHeavy, kB, kA, kExt>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
         }
         if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
     }
@@ -614,6 +635,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         const unsigned hp = (unsigned)nA & 1u;
         const unsigned nh = min(bs->heavy_n[hp], (unsigned)kHeavyListCap);
         if (nh) {
+            const unsigned nto = transfer_step_lo<kExt>(p, (unsigned)nA, bs->n0_lo, bs->bin_phase0);
             unsigned idx = 0;
             for (unsigned r = 0; r < nh; ++r) {
                 const int row = bs->heavy_row[hp][r];
@@ -621,7 +643,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
                 const int len = __ldg(p.row_len + row);
                 for (int off = 0; off < len; off += kChunk, ++idx)
                     if (idx % c.n_warps == c.warp)
-                        deliver_span<kHalf>(p, (unsigned)nA, rb + off, min(kChunk, len - off), c.lane);
+                        deliver_span<kHalf>(p, nto, rb + off, min(kChunk, len - off), c.lane);
             }
             __syncthreads();
         }
@@ -719,7 +741,7 @@ __device__ __noinline__ void service_warp(const SimDev& p, const RunCfg& cfg, co
     }
 }
 
-template <bool kHalf, bool kHeavy, bool kOU>
+template <bool kHalf, bool kHeavy, bool kExt>
 __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ SimDev p, const RunCfg cfg) {
     extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
@@ -740,7 +762,9 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     }
     for (int k = (int)threadIdx.x; k < kMaxTypes * kPoissonMax; k += (int)blockDim.x)
         s_T[k / kPoissonMax][k % kPoissonMax] = p.tc[k / kPoissonMax].T[k % kPoissonMax];
-    if (threadIdx.x == 0) { bs.unit_spikes[0] = bs.unit_spikes[1] = 0u; bs.staged[0] = bs.staged[1] = 0u; bs.heavy_n[0] = bs.heavy_n[1] = 0u; bs.grid_ok = 0u; bs.done[0] = bs.done[1] = 0u; bs.events = 0ull; }
+    if (threadIdx.x == 0) { bs.unit_spikes[0] = bs.unit_spikes[1] = 0u; bs.staged[0] = bs.staged[1] = 0u; bs.heavy_n[0] = bs.heavy_n[1] = 0u; bs.grid_ok = 0u; bs.done[0] = bs.done[1] = 0u; bs.events = 0ull;
+                            const unsigned long long n0 = p.ctl->step;
+                            bs.n0_lo = (unsigned)n0; bs.bin_phase0 = (unsigned)(n0 % (unsigned long long)p.bin_steps); }
     __syncthreads();
 
     Stage sg;
@@ -758,10 +782,10 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     if (c.warp == c.n_warps) { service_warp<kHeavy>(p, cfg, c, &bs); return; }
 
     if (c.task0 < c.last) { request_state(p, sg, c.i00); cp_async_commit(); }
-    run_unit<kHalf, kHeavy, false, true, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
+    run_unit<kHalf, kHeavy, false, true, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
     for (unsigned j = 1; j < cfg.n_steps; ++j)
-        run_unit<kHalf, kHeavy, true, true, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
-    run_unit<kHalf, kHeavy, true, false, kOU>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
+        run_unit<kHalf, kHeavy, true, true, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
+    run_unit<kHalf, kHeavy, true, false, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
 
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (c.lane == 0 && bg_warp)
@@ -1228,7 +1252,7 @@ void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg) 
 }
 
 static const void* run_fn(const SimDev& p, bool heavy) {
-    if (p.ou_on) {
+    if (p.ou_on || p.bin_steps > 1) {          // kExt: OU background current and / or a time bin for transferring spikes
         if (p.w_fp16) return heavy ? (const void*)k_run<true, true, true> : (const void*)k_run<true, false, true>;
         return heavy ? (const void*)k_run<false, true, true> : (const void*)k_run<false, false, true>;
     }

@@ -209,6 +209,47 @@ def test_ou_background_current(db, oracle_mod, mode):
         h.db_write_state(db.FIELD_IOU, I0)
 
 
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("B", [10, 4])
+def test_time_binned_spike_transfer(db, oracle_mod, mode, B):
+    # the paper's time bin b_t for transferring spikes (1 ms at dt = 0.1 ms; R29).  The oracle
+    # keeps the spikes of the open bin and delivers them at the boundary; the kernels push a row at spike time into the
+    # slots of its bin boundary.  State and raster must agree at every step, the ring at the bin boundaries (in between,
+    # DB_FIELD_RING already holds the pushes of the open bin), counters always.
+    N = 4000 + 55
+    net = db_inputs.random_csr(N=N, mean_outdeg=30, seed=21, max_delay=20, heavy_rows={5: 3000, 700: 1500})
+    t = db_inputs.type_params(bg_weight=0.012)
+    sim = db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=B)       # largest delay + b_t - 1 = 29 < D
+    g, o = _pair(db, oracle_mod, sim, net, mode)
+    assert g.db_get_counters()["exec_mode"] == (1 if mode == 3 else mode)         # deferred falls back to two kernels
+    for upto in (1, B - 1, B, 3 * B, 3 * B + 3, 40 * B, 40 * B + 1, 100 * B):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        dv, dg = _compare_state(g, o)
+        assert dv == 0.0 and dg == 0.0
+        if upto % B == 0:
+            assert np.array_equal(_ring_oracle_layout(g), o.ring())
+        cg, co = g.db_get_counters(), o.counters()
+        for k in ("steps", "spikes", "events", "bg_events"):
+            assert cg[k] == co[k], k
+    n = _compare_raster(g, o, 100 * B)
+    assert n > 300
+    # and the result differs from the unbinned scheme (same network, same seeds)
+    sim1 = db_inputs.sim_params(D=32, types=[t, dict(t)])
+    h = db.Sim.db_create_from_csr(sim1, net, exec_mode=mode)
+    h.db_step(100 * B)
+    assert not np.array_equal(h.db_read_spikes(0, 100 * B)[1], g.db_read_spikes(0, 100 * B)[1])
+
+
+def test_time_bin_argument_errors(db):
+    net = db_inputs.random_csr(N=500, mean_outdeg=10, seed=2, max_delay=20)
+    t = db_inputs.type_params()
+    with pytest.raises(db.DbError):          # b_t > R + 1 = 51 steps: a neuron could fire twice inside a bin
+        db.Sim.db_create_from_csr(db_inputs.sim_params(D=128, types=[t, dict(t)], spike_bin_steps=52), net)
+    with pytest.raises(db.DbError):          # largest delay + b_t - 1 = 32 is not < D
+        db.Sim.db_create_from_csr(db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=13), net)
+    db.Sim.db_create_from_csr(db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=12), net).db_step(40)
+
+
 def test_read_spikes_ranges_and_errors(db):
     cfg = db_inputs.config(0, scale=0.2)
     s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=1, raster_capacity=1)   # capacity rounds up to N
