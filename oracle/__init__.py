@@ -375,3 +375,54 @@ def dense_arrivals(net: dict, S: int, spikes: np.ndarray) -> np.ndarray:
          np.ascontiguousarray(net["rec"], np.uint8)]
     lib().orc_dense_arrivals(N, T, int(S), *[_p(x) for x in a], _p(sp), _p(out))
     return out
+
+
+# ---- Balloon-Windkessel BOLD read-out (Extended Data Table 4) ---------------------------
+# Test infrastructure like everything else in this package.  Reading R30: the table prints the
+# equations only; "BW(.) is the Euler-Maruyama discrete-time version of the Balloon-Windkessel model",
+# its noise term is not specified and is left out, so one explicit Euler step per region-rate window; the neural
+# activity z_i is "the spike rate of a pool of neurons": z = z_scale * (region rate in Hz).
+# The constants are not printed either; the defaults are the usual ones of the paper's reference 19
+# (Friston et al. 2000) -- builder's choice, "parity unpinned" for their values.
+BOLD_DEFAULTS = dict(kappa=0.65, gamma=0.41, tau=0.98, alpha=0.32, rho=0.34, V0=0.02,
+                     k1=7 * 0.34, k2=2.0, k3=2 * 0.34 - 0.2, z_scale=0.1)
+
+
+def bold_signal(state: np.ndarray, prm: dict) -> np.ndarray:
+    """y_i = V0 [k1 (1 - q) + k2 (1 - q / v) + k3 (1 - v)]   (P:L359-360); state[..., 4] = s, f, v, q."""
+    v, q = state[..., 2], state[..., 3]
+    return prm["V0"] * (prm["k1"] * (1.0 - q) + prm["k2"] * (1.0 - q / v) + prm["k3"] * (1.0 - v))
+
+
+def bold_step(state: np.ndarray, z: np.ndarray, h: float, prm: dict) -> np.ndarray:
+    """One explicit Euler step of length h (seconds) of the four equations of, all right-hand
+    sides taken at time t."""
+    s, f, v, q = (state[..., k] for k in range(4))
+    fout = v ** (1.0 / prm["alpha"])                                  # f_out = v^(1/alpha)
+    E = 1.0 - (1.0 - prm["rho"]) ** (1.0 / f)                         # E(f, rho) = 1 - (1 - rho)^(1/f)
+    ds = z - prm["kappa"] * s - prm["gamma"] * (f - 1.0)              # s' = z - kappa s - gamma (f - 1)
+    df = s                                                            # f' = s
+    dv = (f - fout) / prm["tau"]                                      # tau v' = f - v^(1/alpha)
+    dq = (f * E / prm["rho"] - fout * q / v) / prm["tau"]             # tau q' = f E / rho - v^(1/alpha) q / v
+    return np.stack([s + h * ds, f + h * df, v + h * dv, q + h * dq], axis=-1)
+
+
+def bold_rest(n_regions: int) -> np.ndarray:
+    """Resting state s = 0, f = v = q = 1 (y = 0)."""
+    st = np.ones((n_regions, 4), np.float64)
+    st[:, 0] = 0.0
+    return st
+
+
+def bold_run(counts: np.ndarray, region_sizes: np.ndarray, window_s: float, prm: dict, state: np.ndarray | None = None):
+    """Feed region spike counts [windows][regions] through the model, one Euler step per window.
+    Returns (y [windows][regions] after each step, final state [regions][4])."""
+    counts = np.asarray(counts, np.float64)
+    sizes = np.asarray(region_sizes, np.float64)
+    st = bold_rest(counts.shape[1]) if state is None else np.array(state, np.float64)
+    ys = np.zeros(counts.shape, np.float64)
+    for w in range(counts.shape[0]):
+        rate_hz = counts[w] / (sizes * window_s)                      # R24
+        st = bold_step(st, prm["z_scale"] * rate_hz, window_s, prm)
+        ys[w] = bold_signal(st, prm)
+    return ys, st
