@@ -69,6 +69,16 @@ typedef struct db_type_params {
     double ou_mu, ou_sigma, ou_tau_ms;
 } db_type_params;
 
+/* Balloon-Windkessel BOLD read-out per region (Extended Data Table 4; reading R30): one explicit Euler
+ * step per completed region-rate window (step length = window_steps * dt), z = z_scale * region rate in Hz, state
+ * (s, f, v, q) starts at rest (0, 1, 1, 1).  The paper prints no constants; the usual ones of its reference 19
+ * are kappa 0.65 /s, gamma 0.41 /s, tau 0.98 s, alpha 0.32, rho 0.34, V0 0.02, k1 7 rho, k2 2, k3 2 rho - 0.2. */
+typedef struct db_bold_params {
+    int32_t enabled;                /* 0: no BOLD read-out (db_read_bold returns DB_ESTATE) */
+    int32_t reserved;
+    double kappa, gamma, tau, alpha, rho, V0, k1, k2, k3, z_scale;
+} db_bold_params;
+
 /* Execution mode of db_step(). */
 #define DB_EXEC_AUTO       0   /* library picks */
 #define DB_EXEC_KERNELS    1   /* two kernels per step (update+compaction, delivery), CUDA-graph replayed */
@@ -97,6 +107,7 @@ typedef struct db_sim_params {
                                  Needs b_t <= R + 1 of every type (A_j is 0 or 1) and largest delay + b_t - 1 < D;
                                  DB_EXEC_KERNELS_DEFERRED falls back to DB_EXEC_KERNELS when b_t > 1.
                                  DB_FIELD_RING already holds the pushes of the spikes of the open bin. */
+    db_bold_params bold;      /* BOLD read-out per region, fed by the region-rate windows (off by default) */
 } db_sim_params;
 
 /* Device memory and stream plumbing supplied by the caller (the Python binding
@@ -219,6 +230,11 @@ int32_t db_region_rates(db_sim* sim, float* rates_hz, uint64_t cap_windows,
 /* The integer counts behind them (same indexing). */
 int32_t db_region_counts(db_sim* sim, uint32_t* counts, uint64_t cap_windows,
                          uint64_t* n_windows, uint64_t* first_window);
+
+/* BOLD signal of every region after the last completed region-rate window: y [n_regions] and, if `state` is not
+ * NULL, the model state [n_regions][4] = (s, f, v, q); HOST buffers owned by the caller, fp64.  *n_windows (may be
+ * NULL) = windows consumed so far.  Synchronises the stream.  DB_ESTATE when the read-out was not enabled. */
+int32_t db_read_bold(db_sim* sim, double* y, double* state, uint64_t* n_windows);
 
 int32_t db_export_csr(db_sim* sim, db_csr_host* out);
 int32_t db_free_csr(db_csr_host* csr);

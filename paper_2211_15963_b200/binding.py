@@ -21,7 +21,7 @@ EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 
 EXPORTS = [
     "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_step_profiled", "db_read_spikes",
-    "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_export_csr",
+    "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_export_csr",
     "db_free_csr", "db_get_counters", "db_synchronize", "db_last_error",
 ]
 
@@ -39,11 +39,18 @@ class TypeParams(C.Structure):
         ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double)]
 
 
+BOLD_KEYS = ("kappa", "gamma", "tau", "alpha", "rho", "V0", "k1", "k2", "k3", "z_scale")
+
+
+class BoldParams(C.Structure):
+    _fields_ = [("enabled", C.c_int32), ("reserved", C.c_int32)] + [(k, C.c_double) for k in BOLD_KEYS]
+
+
 class SimParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("dt_ms", C.c_double), ("S", C.c_int32), ("D", C.c_int32),
                 ("window_steps", C.c_int32), ("n_types", C.c_int32), ("type", TypeParams * 4),
                 ("dyn_seed", C.c_uint64), ("raster_capacity", C.c_uint64), ("max_windows", C.c_uint32),
-                ("exec_mode", C.c_int32), ("spike_bin_steps", C.c_int32)]
+                ("exec_mode", C.c_int32), ("spike_bin_steps", C.c_int32), ("bold", BoldParams)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -115,6 +122,7 @@ def load():
         L.db_read_state.argtypes = [C.c_void_p, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p]
         L.db_write_state.argtypes = [C.c_void_p, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p]
         L.db_region_rates.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        L.db_read_bold.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]
         L.db_region_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         L.db_export_csr.argtypes = [C.c_void_p, C.POINTER(CsrHost)]
         L.db_free_csr.argtypes = [C.POINTER(CsrHost)]
@@ -151,6 +159,10 @@ def _fill_sim_params(p: SimParams, d: dict, dyn_seed: int, exec_mode: int, raste
     p.max_windows = int(max_windows)
     p.exec_mode = int(exec_mode)
     p.spike_bin_steps = int(d.get("spike_bin_steps", 1))
+    if d.get("bold"):                                         # Balloon-Windkessel read-out: dict with BOLD_KEYS
+        p.bold.enabled = 1
+        for k in BOLD_KEYS:
+            setattr(p.bold, k, float(d["bold"][k]))
 
 
 class _TorchRuntime:
@@ -308,6 +320,14 @@ class Sim:
         out = np.empty((n.value, self.R), np.uint32)
         self._ck(self.L.db_region_counts(self.h, _p(out), n.value, C.byref(n), C.byref(first)))
         return out, first.value
+
+    def db_read_bold(self):
+        """(y [regions], state [regions][4] = s, f, v, q, windows consumed), fp64."""
+        n = C.c_uint64()
+        y = np.empty(self.R, np.float64)
+        st = np.empty((self.R, 4), np.float64)
+        self._ck(self.L.db_read_bold(self.h, _p(y), _p(st), C.byref(n)))
+        return y, st, n.value
 
     def db_region_rates(self):
         n, first = C.c_uint64(), C.c_uint64()

@@ -42,6 +42,8 @@ struct db_sim {
     int graph_steps = 0;
     uint64_t launches = 0;
     std::vector<cudaEvent_t> prof_events;
+    BoldDev bold{};                 // BOLD read-out (params.bold.enabled)
+    uint32_t bold_batch = 0;        // steps after which the read-out must catch up (history ring of the region counts)
     std::string err;
 };
 
@@ -233,6 +235,32 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     CK(cudaMemcpyAsync(rs_dev, rs32.data(), rs32.size() * sizeof(int32_t), cudaMemcpyHostToDevice, sim->stream));
     d.region_start = rs_dev;
     if ((rc = alloc_zero(sim, &d.region_counts, (size_t)d.max_windows * (size_t)n_regions))) return rc;
+    if (sp->bold.enabled) {             // Balloon-Windkessel read-out per region (R30)
+        const db_bold_params& bp = sp->bold;
+        if (!(bp.tau > 0) || !(bp.alpha > 0) || !(bp.rho > 0 && bp.rho < 1))
+            return fail(sim, DB_EINVAL, "BOLD parameters out of range (tau > 0, alpha > 0, 0 < rho < 1)");
+        BoldDev& b = sim->bold;
+        double* scale = nullptr;
+        if ((rc = alloc_zero(sim, &b.state, 4 * (size_t)n_regions))) return rc;
+        if ((rc = alloc_zero(sim, &b.y, (size_t)n_regions))) return rc;
+        if ((rc = alloc_zero(sim, &scale, (size_t)n_regions))) return rc;
+        if ((rc = alloc_zero(sim, &b.cursor, 1))) return rc;
+        const double win_s = (double)sp->window_steps * sp->dt_ms * 1e-3;
+        std::vector<double> sc((size_t)n_regions);
+        for (int r = 0; r < n_regions; ++r) {
+            const double size = (double)(sim->region_start[(size_t)r + 1] - sim->region_start[(size_t)r]);
+            sc[(size_t)r] = size > 0 ? bp.z_scale / (size * win_s) : 0.0;
+        }
+        CK(cudaMemcpyAsync(scale, sc.data(), sc.size() * sizeof(double), cudaMemcpyHostToDevice, sim->stream));
+        CK(cudaStreamSynchronize(sim->stream));
+        b.scale = scale;
+        b.kappa = bp.kappa; b.gamma = bp.gamma; b.tau = bp.tau; b.alpha = bp.alpha; b.rho = bp.rho;
+        b.V0 = bp.V0; b.k1 = bp.k1; b.k2 = bp.k2; b.k3 = bp.k3; b.h = win_s;
+        CK(launch_bold_init(b, n_regions, sim->stream));
+        // windows kept as history: max_windows - 1 - (cleared ahead); catch up after at most half of them
+        const uint64_t keep = (uint64_t)d.max_windows - 2 - 2u / (uint64_t)d.window_steps;
+        sim->bold_batch = (uint32_t)std::min<uint64_t>((keep / 2) * (uint64_t)d.window_steps, 1u << 20);
+    }
     if ((rc = alloc_zero(sim, &d.bg_parts, (size_t)kBgParts))) return rc;
     if ((rc = alloc_zero(sim, &d.ctl, 1))) return rc;
     if ((rc = alloc_zero(sim, &sim->ntype_dev, Np))) return rc;
@@ -479,10 +507,25 @@ int32_t db_destroy(db_sim* sim) {
     return DB_OK;
 }
 
+static int32_t step_batch(db_sim* sim, uint32_t n_steps);
+
 int32_t db_step(db_sim* sim, uint32_t n_steps) {
     if (!sim) return DB_EINVAL;
     if (n_steps == 0) return DB_OK;
     CK(cudaSetDevice(sim->device));
+    if (!sim->params.bold.enabled) return step_batch(sim, n_steps);
+    for (uint32_t left = n_steps; left;) {          // the BOLD read-out catches up before the count history wraps
+        const uint32_t b = std::min(left, sim->bold_batch);
+        int32_t rc = step_batch(sim, b);
+        if (rc) return rc;
+        CK(launch_bold(sim->dev, sim->bold, sim->stream));
+        sim->launches += 2;
+        left -= b;
+    }
+    return DB_OK;
+}
+
+static int32_t step_batch(db_sim* sim, uint32_t n_steps) {
     if (sim->exec_mode == DB_EXEC_PERSISTENT) {
         const uint32_t cap = 1u << 20;     // keeps the arrival counter of one launch far below 2^32
         for (uint32_t left = n_steps; left;) {
@@ -784,6 +827,24 @@ int32_t db_region_rates(db_sim* sim, float* rates_hz, uint64_t cap_windows, uint
         const int r = (int)(k % (size_t)R);
         const double size = (double)(sim->region_start[(size_t)r + 1] - sim->region_start[(size_t)r]);
         rates_hz[k] = size > 0 ? (float)((double)c[k] / (size * win_s)) : 0.0f;
+    }
+    return DB_OK;
+}
+
+int32_t db_read_bold(db_sim* sim, double* y, double* state, uint64_t* n_windows) {
+    if (!sim) return DB_EINVAL;
+    if (!sim->params.bold.enabled) return fail(sim, DB_ESTATE, "the BOLD read-out was not enabled (db_sim_params.bold.enabled)");
+    CK(cudaSetDevice(sim->device));
+    CK(launch_bold(sim->dev, sim->bold, sim->stream));     // steps taken through db_step_profiled() are caught up here
+    sim->launches += 2;
+    CK(cudaStreamSynchronize(sim->stream));
+    const size_t R = (size_t)sim->dev.n_regions;
+    if (y) CK(cudaMemcpy(y, sim->bold.y, R * sizeof(double), cudaMemcpyDeviceToHost));
+    if (state) CK(cudaMemcpy(state, sim->bold.state, 4 * R * sizeof(double), cudaMemcpyDeviceToHost));
+    if (n_windows) {
+        unsigned long long c = 0;
+        CK(cudaMemcpy(&c, sim->bold.cursor, sizeof(c), cudaMemcpyDeviceToHost));
+        *n_windows = c;
     }
     return DB_OK;
 }

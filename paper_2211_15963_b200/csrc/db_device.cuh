@@ -96,4 +96,13 @@ struct SimDev {                      // passed by value to every kernel
     TypeConst tc[kMaxTypes];
 };
 
+struct BoldDev {                     // Balloon-Windkessel read-out (db_bold.cu); kept out of SimDev: not on the step path
+    double* state;                   // [n_regions][4] s, f, v, q
+    double* y;                       // [n_regions]
+    const double* scale;             // [n_regions] z_scale / (region size * window seconds)
+    unsigned long long* cursor;      // next window to consume
+    double kappa, gamma, tau, alpha, rho, V0, k1, k2, k3;
+    double h;                        // Euler step = window seconds
+};
+
 }  // namespace dbk

@@ -21,6 +21,10 @@ cudaError_t launch_pending_ring(const SimDev& p, int32_t* out, int first, int co
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 
+// ---- db_bold.cu ------------------------------------------------------------
+cudaError_t launch_bold_init(const BoldDev& b, int n_regions, cudaStream_t st);
+cudaError_t launch_bold(const SimDev& p, const BoldDev& b, cudaStream_t st);   // consume the completed windows
+
 // ---- db_gen.cu -------------------------------------------------------------
 struct GenHostTables {                 // distribution tables formed on the host in double
     std::vector<int64_t> region_start; // [R + 1]

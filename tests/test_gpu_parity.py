@@ -250,6 +250,37 @@ def test_time_bin_argument_errors(db):
     db.Sim.db_create_from_csr(db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=12), net).db_step(40)
 
 
+@pytest.mark.parametrize("mode", MODES)
+def test_bold_readout_matches_oracle(db, oracle_mod, mode):
+    # Balloon-Windkessel read-out per region (Extended Data Table 4; R30), fed by the region-rate
+    # windows.  fp64 on both sides in the same operation order; pow() differs by a few ulp between the two maths
+    # libraries and the model is contracting, so 1e-10 absolute on O(1) states is slack (observed: ~1e-15).
+    N, R = 3000, 5
+    net = db_inputs.random_csr(N=N, mean_outdeg=25, seed=8, n_regions=R)
+    t = db_inputs.type_params(bg_weight=0.02)
+    sim = db_inputs.sim_params(types=[t, dict(t)])
+    sim["bold"] = dict(oracle_mod.BOLD_DEFAULTS)
+    # a short count history (16 windows): db_step has to let the read-out catch up every 7 windows
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode, max_windows=16)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    sizes = np.diff(net["region_start"])
+    win_s = sim["window_steps"] * sim["dt_ms"] * 1e-3
+    y0, st0, n0 = g.db_read_bold()
+    assert n0 == 0 and np.all(y0 == 0.0) and np.array_equal(st0, oracle_mod.bold_rest(R))
+    for upto in (9, 10, 25, 1000, 3007):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        y, st, n = g.db_read_bold()
+        assert n == upto // sim["window_steps"]
+        ys, so = oracle_mod.bold_run(o.region_counts()[:n], sizes, win_s, sim["bold"])
+        if n:
+            assert np.max(np.abs(st - so)) < 1e-10 and np.max(np.abs(y - ys[-1])) < 1e-10
+    assert np.all(st[:, 1] > 1.0) and np.all(np.abs(y) > 1e-6)          # the model has left its resting state
+    _compare_raster(g, o, 3007)
+    h = db.Sim.db_create_from_csr(db_inputs.sim_params(), net)           # not enabled: the call says so
+    with pytest.raises(db.DbError):
+        h.db_read_bold()
+
+
 def test_read_spikes_ranges_and_errors(db):
     cfg = db_inputs.config(0, scale=0.2)
     s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=1, raster_capacity=1)   # capacity rounds up to N
