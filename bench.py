@@ -209,6 +209,9 @@ def run_ours(args):
     db.load()
 
     cfg = db_inputs.config(args.config, rate_hz=(args.rate if args.config == 1 else None), scale=args.scale)
+    if args.drive == "ou":                      # the paper's production drive instead of Poisson
+        db_inputs.ou_drive(cfg["sim"], args.rate)
+    cfg["sim"]["spike_bin_steps"] = args.spike_bin
     N = cfg["net"]["N"]
     n_sim = args.sim_steps
     mode = {"auto": db.EXEC_AUTO, "kernels": db.EXEC_KERNELS, "persistent": db.EXEC_PERSISTENT,
@@ -256,13 +259,14 @@ def run_ours(args):
 
     # ---------------- roofline of the dominant kernel of the timed region ---------------------------
     peak, peak_src = _peaks()
+    upd_per = UPDATE_BYTES_PER_NEURON_STEP + (8 if args.drive == "ou" else 0)   # + read and write of I_ou
     ev_bytes = DELIVER_BYTES_PER_EVENT[fp16]
     note = ("per-step working set (state 22 MB + one ring slot 16 MB) fits the 126 MB L2 at this size: achieved is "
             "algorithmic bytes / time; `traffic` is the DRAM traffic ncu saw (profiles/)")
     if exec_used == db.EXEC_PERSISTENT:
         # k_run: ONE launch = n_sim fused steps (a1 + a2 + a3 + a4); algorithmic bytes per launch =
         # n_sim * 58 B * N (update) + 17 B (15 B fp16) * events of the launch (delivery)
-        upd_bytes = float(UPDATE_BYTES_PER_NEURON_STEP) * N * n_sim
+        upd_bytes = float(upd_per) * N * n_sim
         del_bytes = float(ev_bytes) * events / max(args.steps, 1)
         dur_s = float(np.mean(launch_ms)) * 1e-3
         gbs = (upd_bytes + del_bytes) / dur_s / 1e9
@@ -286,12 +290,12 @@ def run_ours(args):
         prof = sim.db_step_profiled(args.profile_steps)
         upd_s = prof["update_ms"] * 1e-3 / prof["steps"]
         del_s = prof["deliver_ms"] * 1e-3 / prof["steps"]
-        upd_gbs = UPDATE_BYTES_PER_NEURON_STEP * N / upd_s / 1e9
+        upd_gbs = upd_per * N / upd_s / 1e9
         del_gbs = ev_bytes * prof["events"] / prof["steps"] / del_s / 1e9
         two = {
             "bound": "hbm", "kernel": "k_update_stream", "achieved": upd_gbs, "peak": peak, "unit": "GB/s",
             "frac": upd_gbs / peak, "traffic": None, "peak_source": peak_src,
-            "bytes_per_launch": UPDATE_BYTES_PER_NEURON_STEP * N, "us_per_launch": upd_s * 1e6,
+            "bytes_per_launch": upd_per * N, "us_per_launch": upd_s * 1e6,
             "achieved_survey_76B": UPDATE_BYTES_SURVEY * N / upd_s / 1e9,
             "share_of_step": prof["update_ms"] / max(prof["total_ms"], 1e-12),
             "deliver": {"kernel": "k_deliver_deferred" if exec_used == 3 else "k_deliver", "achieved": del_gbs, "frac": del_gbs / peak, "us_per_launch": del_s * 1e6,
@@ -377,7 +381,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": dict(_config_dict(args, N, n_sim), replicas=world,
+            "config": dict(_config_dict(args, N, n_sim), replicas=world, drive=args.drive, spike_bin_steps=args.spike_bin,
                            exec_mode={1: "kernels+graph", 2: "persistent", 3: "kernels+graph, deferred delivery"}.get(exec_used, str(exec_used))),
             "neuron_updates_per_s": world * N * args.steps * n_sim / secs,
             "rtf": secs / bio_s, "mean_rate_hz": rate_hz, "us_per_sim_step": 1e6 * secs / (args.steps * n_sim),
@@ -405,6 +409,9 @@ def main():
     ap.add_argument("--sim-steps", type=int, default=1000, help="simulation time steps per bench step")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink configs[1] (debugging only)")
     ap.add_argument("--exec-mode", choices=["auto", "kernels", "persistent", "deferred"], default="auto")
+    ap.add_argument("--drive", choices=["poisson", "ou"], default="poisson",
+                    help="background drive: Poisson events into AMPA (BASELINE configs) or the paper's OU current (7 Hz only)")
+    ap.add_argument("--spike-bin", type=int, default=1, help="time bin b_t for transferring spikes, in steps (paper: 10)")
     ap.add_argument("--profile-steps", type=int, default=512)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

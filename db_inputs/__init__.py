@@ -29,6 +29,20 @@ BG_WEIGHT_FOR_RATE = {7: 0.0072, 15: 0.0110, 30: 0.0240}
 BG_DRIVE_FOR_CONFIG = {(2, 7): 0.00773, (3, 15): 0.0171, (4, 30): 0.0378}
 
 
+# OU background current (the paper's production drive; sigma 0.12, tau 10 ms as printed in Ext. Table 2):
+# mean that gives the target rate on configs[1] with the constants of R13 and no Poisson drive (the printed mean 0.66
+# gives 2.6 Hz there); swept on the GPU at N = 200,000: 0.66 -> 2.6, 0.74 -> 5.1, 0.82 -> 7.3, 0.90 -> 9.2 Hz.
+OU_SIGMA, OU_TAU_MS = 0.12, 10.0
+OU_MU_FOR_RATE = {7: 0.81}
+
+
+def ou_drive(sim: dict, rate_hz: int = 7) -> dict:
+    """Replace the Poisson drive of every type of `sim` by the OU current calibrated for `rate_hz`."""
+    for t in sim["types"]:
+        t.update(bg_weight=0.0, bg_rate_hz=0.0, ou_mu=OU_MU_FOR_RATE[rate_hz], ou_sigma=OU_SIGMA, ou_tau_ms=OU_TAU_MS)
+    return sim
+
+
 def type_params(bg_weight: float = BG_WEIGHT_FOR_RATE[7], bg_rate_hz: float = 1000.0,
                 g_scale: float = 1.0) -> dict:
     """One neuron type (paper property table, Supp. Table 5)."""

@@ -12,7 +12,7 @@ HEADERS = ["db_device.cuh", "db_philox.cuh", "db_host.h", os.path.join("..", "..
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "4",
 ]
 
 

@@ -210,7 +210,8 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     if ((rc = alloc_zero(sim, &d.g, 4 * Np))) return rc;
     if ((rc = alloc_zero(sim, &d.rt, Np))) return rc;
     d.ou_on = 0;
-    for (int t = 0; t < sp->n_types; ++t) d.ou_on |= d.tc[t].ou;
+    d.bg_on = 0;
+    for (int t = 0; t < sp->n_types; ++t) { d.ou_on |= d.tc[t].ou; d.bg_on |= (d.tc[t].M > 0); }
     if (d.ou_on) {                      // OU state and the table of standard-normal quantiles its increments come from
         if ((rc = alloc_zero(sim, &d.Iou, Np))) return rc;
         float* ntab = nullptr;

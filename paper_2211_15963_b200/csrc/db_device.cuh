@@ -64,6 +64,7 @@ struct SimDev {                      // passed by value to every kernel
     float* Iou;                      // [Npad] OU background current (allocated only if some type uses it)
     const float* ntab;               // [65536] standard-normal quantiles (same condition)
     int32_t ou_on;
+    int32_t bg_on;                   // some type has a Poisson background (else its Philox draw is skipped)
     int32_t bin_steps;               // time bin b_t for transferring spikes, in steps (>= 1; R29)
     int32_t* ring;                   // [D][4][Npad] fixed-point arrivals
     // presynaptic-major CSR

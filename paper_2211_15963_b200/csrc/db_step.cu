@@ -58,10 +58,10 @@ __device__ __forceinline__ unsigned long long transfer_step(const SimDev& p, con
 
 // The same for the persistent kernel, low word only (slots are taken modulo the power of two D), from the phase of
 // the launch's first step (32-bit arithmetic: no 64-bit division on the spike path).
-template <bool kExt>
+template <bool kBin>
 __device__ __forceinline__ unsigned transfer_step_lo(const SimDev& p, const unsigned n_lo, const unsigned n0_lo,
                                                      const unsigned phase0) {
-    if (!kExt || p.bin_steps == 1) return n_lo;
+    if (!kBin) return n_lo;
     const unsigned b = (unsigned)p.bin_steps;
     return n_lo - (phase0 + (n_lo - n0_lo)) % b + (b - 1u);
 }
@@ -350,7 +350,7 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
                                                  const int i0, int32_t* slot, const int next_off,
                                                  const uint4 v_bits, const uint2 rt_bits, const uint4 rnd,
                                                  unsigned& bg_acc, float4* iou = nullptr,
-                                                 const uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u)) {
+                                                 const float4 xi_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f)) {
     const size_t Np = (size_t)p.Npad;
     const int tp[4] = {tp0, tp1, tp2, tp3};
     const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
@@ -424,8 +424,7 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
                 const float4 m3 = s_tc[tp[q]].m3;   // I_ou += (mu - I_ou) dt/tau + sigma sqrt(2 dt/tau) xi
                 if (__float_as_int(m3.w)) {
                     float* io = reinterpret_cast<float*>(iou) + q;
-                    const uint32_t wo = (q == 0) ? rnd_ou.x : (q == 1) ? rnd_ou.y : (q == 2) ? rnd_ou.z : rnd_ou.w;
-                    const float xi = __ldg(p.ntab + (wo >> 16));
+                    const float xi = (q == 0) ? xi_ou.x : (q == 1) ? xi_ou.y : (q == 2) ? xi_ou.z : xi_ou.w;
                     Iq = __fadd_rn(Iq, *io);
                     *io = __fadd_rn(*io, __fadd_rn(__fmul_rn(__fsub_rn(m3.x, *io), m3.y), __fmul_rn(m3.z, xi)));
                 }
@@ -464,7 +463,7 @@ struct BlockShared {                 // small per-block scratch of the persisten
 // One 128-neuron task of one warp in unit (kB: B of step nB, kA: A of step nA).  next_off != 0:
 // distance (in neurons) to the warp's next task of this unit, whose planes are requested while
 // this one is consumed.
-template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kExt>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU, bool kBin>
 __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, const uint32_t (*s_T)[kPoissonMax],
                                          BlockShared* bs, const Stage& sg, const unsigned long long nB,
                                          const unsigned long long nA, const int task, const unsigned lane,
@@ -475,13 +474,16 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     int32_t* slot = p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * Np + i0;
     // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
     uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
-    if (kB) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
+    if (kB && (!kOU || p.bg_on))       // (with the OU drive the Poisson background is usually off: no draw then)
+        rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
     float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u);
-    const bool ou = kExt && kA && p.ou_on;
-    if (ou) {                          // OU current of the four neurons and the words its increments come from
-        iou = ld_cg_f4(p.Iou + i0);
-        rnd_ou = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
+    float4 rnd_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    const bool ou = kOU && kA;
+    if (ou) {                          // OU current of the four neurons and their N(0,1) draws (quantile table, top 16 bits of
+        iou = ld_cg_f4(p.Iou + i0);    // a Philox word each); gathered here so that the latency hides behind the staged copies
+        const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
+        rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
+                             __ldg(p.ntab + (wo.w >> 16)));
     }
     cp_async_wait_all();
     const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
@@ -494,9 +496,9 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
     unsigned spike_bits;
     if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-        spike_bits = neuron_group<kB, kA, false, kExt>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
     else                                // a type boundary inside the group (rare)
-        spike_bits = neuron_group<kB, kA, false, kExt>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
     if (ou) st_cg_f4(p.Iou + i0, iou);
     cp_async_commit();
     if (!kA) return;
@@ -556,7 +558,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
         }                                                      // one region: added per block and unit (run_unit)
     // a3: the warp pushes the rows of its own spikes, one row at a time
     const unsigned nlo = (unsigned)nA;
-    const unsigned nto = transfer_step_lo<kExt>(p, nlo, bs->n0_lo, bs->bin_phase0);   // slot of a synapse = nto + delay
+    const unsigned nto = transfer_step_lo<kBin>(p, nlo, bs->n0_lo, bs->bin_phase0);   // slot of a synapse = nto + delay
     while (any) {
         const int src = __ffs(any) - 1;
         any &= any - 1u;
@@ -600,7 +602,7 @@ struct RunCtx {                      // per-thread constants of the persistent k
 };
 
 // Unit j of the launch (see the header comment): B of step n0 + j - 1 (if kB), A of step n0 + j (if kA).
-template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kExt>
+template <bool kHalf, bool kHeavy, bool kB, bool kA, bool kOU, bool kBin>
 __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, const RunCtx& c, const TypeSmem* s_tc,
                                          const uint32_t (*s_T)[kPoissonMax], BlockShared* bs, const Stage& sg,
                                          const unsigned j, unsigned& bg_acc) {
@@ -617,7 +619,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         cp_async_commit();
         for (int task = c.task0; task < c.last; task += (int)c.n_warps) {
             const int next_off = (task + (int)c.n_warps < c.last) ? c.task_stride : 0;
-            run_task<kHalf, kHeavy, kB, kA, kExt>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
+            run_task<kHalf, kHeavy, kB, kA, kOU, kBin>(p, s_tc, s_T, bs, sg, nB, nA, task, c.lane, next_off, bg_acc);
         }
         if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
     }
@@ -635,7 +637,7 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         const unsigned hp = (unsigned)nA & 1u;
         const unsigned nh = min(bs->heavy_n[hp], (unsigned)kHeavyListCap);
         if (nh) {
-            const unsigned nto = transfer_step_lo<kExt>(p, (unsigned)nA, bs->n0_lo, bs->bin_phase0);
+            const unsigned nto = transfer_step_lo<kBin>(p, (unsigned)nA, bs->n0_lo, bs->bin_phase0);
             unsigned idx = 0;
             for (unsigned r = 0; r < nh; ++r) {
                 const int row = bs->heavy_row[hp][r];
@@ -741,7 +743,7 @@ __device__ __noinline__ void service_warp(const SimDev& p, const RunCfg& cfg, co
     }
 }
 
-template <bool kHalf, bool kHeavy, bool kExt>
+template <bool kHalf, bool kHeavy, bool kOU, bool kBin>
 __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ SimDev p, const RunCfg cfg) {
     extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
@@ -782,10 +784,10 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_run(const __grid_constant__ 
     if (c.warp == c.n_warps) { service_warp<kHeavy>(p, cfg, c, &bs); return; }
 
     if (c.task0 < c.last) { request_state(p, sg, c.i00); cp_async_commit(); }
-    run_unit<kHalf, kHeavy, false, true, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
+    run_unit<kHalf, kHeavy, false, true, kOU, kBin>(p, cfg, c, s_tc, s_T, &bs, sg, 0u, bg_acc);
     for (unsigned j = 1; j < cfg.n_steps; ++j)
-        run_unit<kHalf, kHeavy, true, true, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
-    run_unit<kHalf, kHeavy, true, false, kExt>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
+        run_unit<kHalf, kHeavy, true, true, kOU, kBin>(p, cfg, c, s_tc, s_T, &bs, sg, j, bg_acc);
+    run_unit<kHalf, kHeavy, true, false, kOU, kBin>(p, cfg, c, s_tc, s_T, &bs, sg, cfg.n_steps, bg_acc);
 
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (c.lane == 0 && bg_warp)
@@ -891,12 +893,15 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int grp = task * 32 + (int)lane;
         const int i0 = grp * 4;
         // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
-        const uint4 rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+        uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
+        if (!kOU || p.bg_on) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
         float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        uint4 rnd_ou = make_uint4(0u, 0u, 0u, 0u);
+        float4 rnd_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (kOU) {
             iou = ld_cg_f4(p.Iou + i0);
-            rnd_ou = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+            const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+            rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
+                                 __ldg(p.ntab + (wo.w >> 16)));
         }
         cp_async_wait_all();
         const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
@@ -1251,13 +1256,16 @@ void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg) 
     *threads = (warps + 1) * 32;
 }
 
+template <bool kOU, bool kBin>
+static const void* run_fn2(const SimDev& p, bool heavy) {
+    if (p.w_fp16) return heavy ? (const void*)k_run<true, true, kOU, kBin> : (const void*)k_run<true, false, kOU, kBin>;
+    return heavy ? (const void*)k_run<false, true, kOU, kBin> : (const void*)k_run<false, false, kOU, kBin>;
+}
+
 static const void* run_fn(const SimDev& p, bool heavy) {
-    if (p.ou_on || p.bin_steps > 1) {          // kExt: OU background current and / or a time bin for transferring spikes
-        if (p.w_fp16) return heavy ? (const void*)k_run<true, true, true> : (const void*)k_run<true, false, true>;
-        return heavy ? (const void*)k_run<false, true, true> : (const void*)k_run<false, false, true>;
-    }
-    if (p.w_fp16) return heavy ? (const void*)k_run<true, true, false> : (const void*)k_run<true, false, false>;
-    return heavy ? (const void*)k_run<false, true, false> : (const void*)k_run<false, false, false>;
+    const bool bin = p.bin_steps > 1;       // OU drive and time-binned transfer are template arms: the plain kernel pays for neither
+    if (p.ou_on) return bin ? run_fn2<true, true>(p, heavy) : run_fn2<true, false>(p, heavy);
+    return bin ? run_fn2<false, true>(p, heavy) : run_fn2<false, false>(p, heavy);
 }
 
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok) {
