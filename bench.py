@@ -314,6 +314,22 @@ def run_ours(args):
                                     "sectors, DRAM traffic per event is several times the 17 (15) algorithmic bytes"}
         else:
             roofline["two_kernel_mode"] = two
+    # the ceilings of scatter delivery (a3) on this device: random 4-byte reductions into a region the size of the ring
+    # (far larger than L2: random DRAM sectors) and into one the size of ONE ring slot (L2-resident), measured live
+    if rank == 0 and not args.no_scatter_probe:
+        ring_bytes = min(int(cfg["sim"]["D"]) * 16 * N, 8 << 30)
+        slot_bytes = 16 * N
+        pr = {"what": "db_probe_scatter: red.global.add.s32 to uniformly random cells, ops/s",
+              "ring_sized_region": {"bytes": ring_bytes, "ops_per_s": db.binding.db_probe_scatter(ring_bytes, device=local)},
+              "one_slot_region": {"bytes": slot_bytes, "ops_per_s": db.binding.db_probe_scatter(slot_bytes, device=local)}}
+        if roofline is not None:
+            roofline["scatter_probe"] = pr
+            dlv = roofline if roofline.get("kernel", "").startswith("k_deliver") else roofline.get("two_kernel_mode", roofline).get("deliver")
+            if dlv and dlv.get("us_per_launch"):
+                ev_s = dlv.get("events_per_launch", 0) / (dlv["us_per_launch"] * 1e-6) if "events_per_launch" in dlv else \
+                    roofline["bytes_per_launch"] / ev_bytes / (roofline["us_per_launch"] * 1e-6)
+                pr["delivery_kernel_events_per_s"] = ev_s
+                pr["frac_of_ring_sized_probe"] = ev_s / pr["ring_sized_region"]["ops_per_s"]
     if roofline is None:
         roofline = {"bound": "hbm", "kernel": "k_update_stream + k_deliver", "achieved": None, "peak": peak, "unit": "GB/s",
                     "frac": None, "traffic": None, "note": "run with --profile-steps > 0 for per-kernel times"}
@@ -415,6 +431,7 @@ def main():
     ap.add_argument("--profile-steps", type=int, default=512)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-scatter-probe", action="store_true")
     ap.add_argument("--ref-scale", type=float, default=0.25, help="oracle sample: fraction of configs[1]'s neurons")
     ap.add_argument("--ref-warm-steps", type=int, default=1000, help="oracle: untimed steps past the start-up transient")
     ap.add_argument("--ref-sim-steps", type=int, default=50, help="oracle arm: time steps per bench step")
