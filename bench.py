@@ -385,11 +385,12 @@ def run_ours(args):
     # ---------------- CPU baseline: the oracle on the host cores (rank 0, N = 1 only) ----------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        res, ocfg = oracle_sample(args.rate, args.ref_scale, warm_steps=args.ref_warm_steps, timed_steps=300)
+        cpu_steps = 2000                    # ~12 s of single-thread work at the default 250,000-neuron sample
+        res, ocfg = oracle_sample(args.rate, args.ref_scale, warm_steps=args.ref_warm_steps, timed_steps=cpu_steps)
         dt_o, ev_o, up_o = res[0]
         cpu = {"value": ev_o / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
                "neuron_updates_per_s": up_o / dt_o,
-               "sample": f"configs[1] shrunk to N={ocfg['net']['N']} (in-degree 100, same distributions), 300 time "
+               "sample": f"configs[1] shrunk to N={ocfg['net']['N']} (in-degree 100, same distributions), {cpu_steps} time "
                          f"steps after {args.ref_warm_steps} warm-up steps, single thread, {dt_o:.1f} s (+ network generation)"}
 
     if rank == 0:
