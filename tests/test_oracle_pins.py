@@ -477,7 +477,15 @@ def test_ou_without_noise_relaxes_geometrically_to_mu(oracle_mod):
 def test_ou_stationary_mean_sd_and_autocorrelation(oracle_mod):
     # Ext. Table 2: mu = 0.66, sigma = 0.12, tau = 10.  The discrete map has stationary mean mu,
     # variance sigma^2 (2a)/(1-(1-a)^2) = sigma^2/(1 - a/2), a = dt/tau, and lag-k autocorrelation (1-a)^k ~ e^{-k dt/tau}
-    mu, sigma, tau, dt = 0.66, 0.12, 10.0, 1.0
+    import os
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "ou_extended_data_table2.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                vals[k] = float(v)
+    mu, sigma, tau, dt = vals["mu_ext"], vals["sigma_ext"], vals["tau_ext"], 1.0     # the paper's printed values
+    assert (mu, sigma, tau) == (0.66, 0.12, 10.0)
     N, burn, T = 4000, 200, 400
     sim = _ou_sim(mu, sigma, tau, dt, Vth=1e9)                  # no spikes: the membrane is irrelevant here
     o = oracle_mod.OracleSim(sim, _ou_net(N), 7, fp64=True)
