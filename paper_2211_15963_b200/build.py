@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdb_b200.so")
-SOURCES = ["db_step.cu", "db_gen.cu", "db_api.cu", "db_bold.cu", "db_probe.cu"]
+SOURCES = ["db_step.cu", "db_gen.cu", "db_api.cu", "db_bold.cu", "db_probe.cu", "db_raster.cu"]
 HEADERS = ["db_device.cuh", "db_philox.cuh", "db_host.h", os.path.join("..", "..", "include", "db_b200.h")]
 
 NVCC_FLAGS = [

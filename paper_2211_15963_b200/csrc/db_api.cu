@@ -646,6 +646,17 @@ int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint
     *n_out = n;
     if (n == 0 || cap == 0) return DB_OK;
     const uint64_t m = scan_end - scan_begin;
+    if (m >= 2048) {                    // long ranges: select and sort on the device (db_raster.cu)
+        std::vector<unsigned long long> keys;
+        CK(raster_sorted_keys(sim->dev, scan_begin, m, (uint32_t)step_begin, (uint32_t)(step_end - step_begin), n, &keys, sim->stream));
+        if (keys.size() < n || keys[(size_t)n - 1] == ~0ull || (keys.size() > n && keys[(size_t)n] != ~0ull))
+            return fail(sim, DB_ESTATE, "raster log is inconsistent");
+        for (uint64_t o = 0; o < n && o < cap; ++o) {
+            if (steps) steps[o] = step_begin + (keys[(size_t)o] >> 32);
+            if (ids) ids[o] = (int32_t)(uint32_t)keys[(size_t)o];
+        }
+        return DB_OK;
+    }
     std::vector<int32_t> id_raw((size_t)m);
     std::vector<uint32_t> tag_raw((size_t)m);
     for (uint64_t k = 0; k < m;) {
