@@ -24,13 +24,23 @@ cudaError_t raster_sorted_keys(const SimDev& p, uint64_t scan_begin, uint64_t m,
     unsigned long long *a = nullptr, *b = nullptr;
     void* tmp = nullptr;
     size_t tmp_bytes = 0;
-    cudaError_t e = cudaMalloc(&a, (size_t)m * 8);
-    if (e == cudaSuccess) e = cudaMalloc(&b, (size_t)m * 8);
+    static bool pool_set = false;                       // keep the scratch of the last calls in the stream-ordered pool
+    if (!pool_set) {                                    // (default: everything goes back to the OS at every synchronize)
+        int dev = 0;
+        cudaMemPool_t pool = nullptr;
+        unsigned long long keep = 256ull << 20;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess)
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        cudaGetLastError();
+        pool_set = true;
+    }
+    cudaError_t e = cudaMallocAsync(&a, (size_t)m * 8, st);
+    if (e == cudaSuccess) e = cudaMallocAsync(&b, (size_t)m * 8, st);
     int end_bit = 33;                                   // bits of (span - 1) above the id word, + the sentinel's
     while (end_bit < 64 && ((uint64_t)span >> (end_bit - 32)) != 0) ++end_bit;
     end_bit = end_bit < 64 ? end_bit + 1 : 64;          // one more bit tells the all-ones sentinel from any valid key
     if (e == cudaSuccess) e = cub::DeviceRadixSort::SortKeys(nullptr, tmp_bytes, a, b, (int64_t)m, 0, end_bit, st);
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, tmp_bytes ? tmp_bytes : 16);
+    if (e == cudaSuccess) e = cudaMallocAsync(&tmp, tmp_bytes ? tmp_bytes : 16, st);
     if (e == cudaSuccess) {
         const unsigned grid = (unsigned)std::min<uint64_t>((m + 255) / 256, 148ull * 16);
         k_raster_keys<<<grid, 256, 0, st>>>(p, scan_begin, m, lo, span, a);
@@ -41,8 +51,11 @@ cudaError_t raster_sorted_keys(const SimDev& p, uint64_t scan_begin, uint64_t m,
         keys_host->resize((size_t)std::min<uint64_t>(n + 1, m));
         e = cudaMemcpyAsync(keys_host->data(), b, keys_host->size() * 8, cudaMemcpyDeviceToHost, st);
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(a); cudaFree(b); cudaFree(tmp);
+    if (a) cudaFreeAsync(a, st);
+    if (b) cudaFreeAsync(b, st);
+    if (tmp) cudaFreeAsync(tmp, st);
+    const cudaError_t e2 = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = e2;
     return e;
 }
 
