@@ -281,6 +281,35 @@ def test_bold_readout_matches_oracle(db, oracle_mod, mode):
         h.db_read_bold()
 
 
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("fp16", [False, True])
+def test_production_combination_ou_bin_bold_regions(db, oracle_mod, mode, fp16):
+    # the paper's production mode in one run: OU drive on both types, b_t = 10 steps, several regions
+    # with the BOLD read-out (Ext. Table 4), binary16 weights as in configs[3] -- the k_run<.., OU, bin> instantiation
+    N, R, B = 5000 + 13, 4, 10
+    net = db_inputs.random_csr(N=N, mean_outdeg=35, seed=41, n_regions=R, fp16=fp16)
+    t = db_inputs.type_params(bg_weight=0.0, bg_rate_hz=0.0)
+    t.update(ou_mu=0.9, ou_sigma=0.12, ou_tau_ms=10.0)
+    sim = db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=B)
+    sim["bold"] = dict(oracle_mod.BOLD_DEFAULTS)
+    g, o = _pair(db, oracle_mod, sim, net, mode, fp16=fp16)
+    sizes = np.diff(net["region_start"])
+    win_s = sim["window_steps"] * sim["dt_ms"] * 1e-3
+    for upto in (B, 7 * B + 3, 60 * B, 150 * B):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        dv, dg = _compare_state(g, o)
+        assert dv == 0.0 and dg == 0.0
+        assert np.array_equal(g.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32))
+        if upto % B == 0:
+            assert np.array_equal(_ring_oracle_layout(g), o.ring())
+        y, st, n = g.db_read_bold()
+        ys, so = oracle_mod.bold_run(o.region_counts()[:n], sizes, win_s, sim["bold"])
+        assert n == upto // sim["window_steps"] and np.max(np.abs(st - so)) < 1e-10 and np.max(np.abs(y - ys[-1])) < 1e-10
+    assert _compare_raster(g, o, 150 * B) > 300
+    cnt, first = g.db_region_counts()
+    assert first == 0 and np.array_equal(cnt, o.region_counts()[:len(cnt)])
+
+
 def test_read_spikes_ranges_and_errors(db):
     cfg = db_inputs.config(0, scale=0.2)
     s = db.Sim.db_create(cfg["net"], cfg["sim"], seed=1, raster_capacity=1)   # capacity rounds up to N
