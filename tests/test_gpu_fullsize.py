@@ -95,6 +95,28 @@ def test_config1_full_size_closed_loop(db, oracle_mod):
     for key in ("steps", "spikes", "events", "bg_events"):
         assert cg[key] == co[key], key
     s.db_destroy()
+    o.close()
+    _free()
+    # the same network in the paper's production mode (`bench.py --drive ou --spike-bin 10`): OU drive, b_t = 10 steps
+    import copy
+    sim2 = db_inputs.ou_drive(copy.deepcopy(cfg["sim"]))
+    sim2["spike_bin_steps"] = 10
+    s = db.Sim.db_create(cfg["net"], sim2, seed=db_inputs.GEN_SEED, dyn_seed=db_inputs.DYN_SEED, raster_capacity=1 << 25)
+    assert s.db_get_counters()["exec_mode"] == db.EXEC_PERSISTENT
+    o = oracle_mod.OracleSim(sim2, net, db_inputs.DYN_SEED)
+    s.db_step(40)
+    o.step(40)
+    sg, ig = s.db_read_spikes(0, 40)
+    so, io = o.spikes()
+    k = np.lexsort((io, so))
+    assert len(ig) > 300 and np.array_equal(sg, so[k]) and np.array_equal(ig, io[k])
+    Vg, gg, rg = s.state()
+    Vo, go, ro = o.state()
+    assert np.array_equal(Vg, Vo.astype(np.float32)) and np.array_equal(gg, go.astype(np.float32)) and np.array_equal(rg, ro)
+    assert np.array_equal(s.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32))
+    assert np.array_equal(s.db_read_state(db.FIELD_RING), o.ring())                 # 40 is a bin boundary
+    s.db_destroy()
+    o.close()
     _free()
 
 
