@@ -12,7 +12,7 @@ constexpr int kNeuronPad = 1024;     // Npad is a multiple of this: whole warps,
 constexpr int kRowAlign = 4;         // CSR rows start on a multiple of 4 synapses (128-bit target loads)
 constexpr int kChunk = 512;          // synapses per delivery work item (one warp)
 constexpr int kInlineMax = 1024;     // persistent kernel: rows up to this length are delivered by the warp that found the spike
-constexpr int kRunThreads = 896;     // persistent kernel: most threads per block (one block per SM)
+constexpr int kRunThreads = 640;     // persistent kernel: most threads per block (one block per SM); 96 registers per thread (measured: 512 .. 1024 threads, profiles/r1s_threads_per_block.md)
 constexpr int kRefMask = 0x0FFF;     // rt = type << 12 | refractory steps left
 
 // Philox streams
