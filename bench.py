@@ -50,7 +50,7 @@ DELIVER_BYTES_PER_EVENT = {0: 17, 1: 15}   # tgt|rec 4 + w 4 (fp32) / 2 (fp16) +
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full`
 # captures under profiles/ (bytes per launch in that capture's configuration; see the .md beside each)
 NCU_TRAFFIC = {"k_update": 38.1e6,          # profiles/r1a_two_kernel_baseline.md (one time step)
-               "k_run_per_sim_step": 25.6e6}  # profiles/r1k_round1_final.md (5.11 GB per 200-step launch)
+               "k_run_per_sim_step": 24.95e6}  # profiles/r1t_launches.md (4.99 GB per 200-step launch)
 
 
 def _peaks():
