@@ -154,3 +154,31 @@ def random_csr(N: int, mean_outdeg: float, seed: int, max_delay: int = 20, n_reg
     rec = (2 * src_type + slow).astype(np.uint8)
     return dict(N=N, E=E, n_regions=n_regions, region_start=bounds, ntype=ntype,
                 row_ptr=row_ptr, tgt=tgt, w=w, delay=delay, rec=rec)
+
+
+def bulk_csr(N: int, base_outdeg: int, seed: int, heavy_rows: dict | None = None, max_delay: int = 20,
+             n_regions: int = 1) -> dict:
+    """A large numpy-random network built without a Python loop over rows (from-CSR tests at sizes where a block of
+    the persistent kernel owns thousands of neurons): every row has `base_outdeg` synapses, the rows of
+    `heavy_rows` ({row: out_degree}) are longer.  Targets are uniform (self and repeated targets are allowed: the sums
+    are the same integers either way); types 80/20 by id inside every region."""
+    rng = np.random.default_rng(seed)
+    deg = np.full(N, base_outdeg, np.int64)
+    for r, d in (heavy_rows or {}).items():
+        deg[r] = d
+    row_ptr = np.zeros(N + 1, np.int64)
+    row_ptr[1:] = np.cumsum(deg)
+    E = int(row_ptr[-1])
+    bounds = np.linspace(0, N, n_regions + 1).astype(np.int64)
+    ntype = np.zeros(N, np.uint8)
+    for r in range(n_regions):
+        lo, hi = int(bounds[r]), int(bounds[r + 1])
+        ntype[lo + int(round(0.8 * (hi - lo))):hi] = 1
+    tgt = rng.integers(0, N, E).astype(np.int32)
+    src_type = np.repeat(ntype, deg)
+    w = (0.01 * rng.lognormal(-1.0, 0.5, E)).astype(np.float32)
+    w = np.where(src_type == 1, w * np.float32(4.0), w).astype(np.float32)
+    delay = rng.integers(1, max_delay + 1, E).astype(np.uint8)
+    rec = (2 * src_type + (rng.random(E) < 0.2)).astype(np.uint8)
+    return dict(N=N, E=E, n_regions=n_regions, region_start=bounds, ntype=ntype, row_ptr=row_ptr, tgt=tgt, w=w,
+                delay=delay, rec=rec)

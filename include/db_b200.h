@@ -236,13 +236,6 @@ int32_t db_region_counts(db_sim* sim, uint32_t* counts, uint64_t cap_windows,
  * NULL) = windows consumed so far.  Synchronises the stream.  DB_ESTATE when the read-out was not enabled. */
 int32_t db_read_bold(db_sim* sim, double* y, double* state, uint64_t* n_windows);
 
-/* Measurement aid (not on the step path; SURVEY 8(d) "atomic throughput"): rate, in operations per second, at which
- * `device` retires 4-byte integer reductions -- the instruction of a3 -- to uniformly random cells of a scratch
- * region of `region_bytes` (allocated and freed inside; >= 4).  `n_ops` reductions per launch, `reps` timed launches
- * after one warm-up, CUDA events on the default stream.  A region far larger than L2 gives the device's random
- * DRAM-sector rate, one that fits gives the L2 rate: the two ceilings of scatter delivery.  *ops_per_s: HOST. */
-int32_t db_probe_scatter(int32_t device, uint64_t region_bytes, uint64_t n_ops, uint32_t reps, double* ops_per_s);
-
 int32_t db_export_csr(db_sim* sim, db_csr_host* out);
 int32_t db_free_csr(db_csr_host* csr);
 

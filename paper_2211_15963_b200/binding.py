@@ -21,7 +21,7 @@ EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 
 EXPORTS = [
     "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_step_profiled", "db_read_spikes",
-    "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_probe_scatter", "db_export_csr",
+    "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_export_csr",
     "db_free_csr", "db_get_counters", "db_synchronize", "db_last_error",
 ]
 
@@ -122,7 +122,6 @@ def load():
         L.db_read_state.argtypes = [C.c_void_p, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p]
         L.db_write_state.argtypes = [C.c_void_p, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p]
         L.db_region_rates.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
-        L.db_probe_scatter.argtypes = [C.c_int32, C.c_uint64, C.c_uint64, C.c_uint32, C.POINTER(C.c_double)]
         L.db_read_bold.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]
         L.db_region_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         L.db_export_csr.argtypes = [C.c_void_p, C.POINTER(CsrHost)]
@@ -194,10 +193,20 @@ class _TorchRuntime:
                           C.c_void_p(torch.cuda.current_stream(device).cuda_stream), device)
 
 
+_probe_lib = None
+
+
 def db_probe_scatter(region_bytes: int, n_ops: int = 1 << 24, reps: int = 5, device: int = 0) -> float:
-    """Random 4-byte reductions per second into a region of `region_bytes` (measurement aid, include/db_b200.h)."""
+    """Random 4-byte reductions per second into a region of `region_bytes`: bench-only measurement helper
+    (libdb_probe.so, csrc/db_probe.cu), not part of the product ABI."""
+    global _probe_lib
+    if _probe_lib is None:
+        _build.build()
+        _probe_lib = C.CDLL(_build.PROBE_LIB)
+        _probe_lib.db_probe_scatter.argtypes = [C.c_int32, C.c_uint64, C.c_uint64, C.c_uint32, C.POINTER(C.c_double)]
+        _probe_lib.db_probe_scatter.restype = C.c_int32
     out = C.c_double()
-    rc = load().db_probe_scatter(int(device), int(region_bytes), int(n_ops), int(reps), C.byref(out))
+    rc = _probe_lib.db_probe_scatter(int(device), int(region_bytes), int(n_ops), int(reps), C.byref(out))
     if rc != DB_OK:
         raise DbError(rc, "db_probe_scatter failed")
     return out.value

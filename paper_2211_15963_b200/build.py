@@ -7,7 +7,9 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdb_b200.so")
-SOURCES = ["db_step.cu", "db_gen.cu", "db_api.cu", "db_bold.cu", "db_probe.cu", "db_raster.cu"]
+SOURCES = ["db_step.cu", "db_gen.cu", "db_api.cu", "db_bold.cu", "db_raster.cu"]
+PROBE_LIB = os.path.join(HERE, "libdb_probe.so")      # bench-only measurement helper, not part of the product ABI
+PROBE_SOURCES = ["db_probe.cu"]
 HEADERS = ["db_device.cuh", "db_philox.cuh", "db_host.h", os.path.join("..", "..", "include", "db_b200.h")]
 
 NVCC_FLAGS = [
@@ -16,11 +18,11 @@ NVCC_FLAGS = [
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(lib: str = LIB, sources=None) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
-    files = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
+    t = os.path.getmtime(lib)
+    files = [os.path.join(CSRC, f) for f in (SOURCES + HEADERS if sources is None else sources)]
     return any(os.path.getmtime(f) > t for f in files)
 
 
@@ -32,6 +34,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             cmd.insert(1, "-Xptxas")
             cmd.insert(2, "-v")
         subprocess.check_call(cmd)
+    if force or _stale(PROBE_LIB, PROBE_SOURCES):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.check_call([nvcc, *NVCC_FLAGS, "-o", PROBE_LIB, *[os.path.join(CSRC, f) for f in PROBE_SOURCES]])
     return LIB
 
 

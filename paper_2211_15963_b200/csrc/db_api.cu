@@ -298,7 +298,7 @@ int32_t build_delay_segments(db_sim* sim, int near_max) {
         while (r1 < N && row_end(r1) - s0 <= batch) ++r1;
         const int64_t s1 = row_end(r1 - 1);
         if (s1 - s0 > batch) { out = fail(sim, DB_EINVAL, "a row is longer than the sorting batch"); break; }
-        cudaError_t e = launch_sort_rows(d, r0, r1, s0, t_s, w_s, d_s, seg, near_max, sim->stream);
+        cudaError_t e = launch_sort_rows(d, sim->n_sm, r0, r1, s0, t_s, w_s, d_s, seg, near_max, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint32_t*>(d.tgt_rec) + s0, t_s, (size_t)(s1 - s0) * 4, cudaMemcpyDeviceToDevice, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint8_t*>(d.delay) + s0, d_s, (size_t)(s1 - s0), cudaMemcpyDeviceToDevice, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync((char*)const_cast<void*>(d.w) + (size_t)s0 * wsz, w_s, (size_t)(s1 - s0) * wsz, cudaMemcpyDeviceToDevice, sim->stream);
@@ -326,6 +326,8 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int3
     int coop = 0;
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device));
     bool fits = false;
+    CK(prepare_kernels());              // function attributes and the memory pool belong to the device: once per handle
+    CK(raster_pool_setup(sim->device));
     CK(persistent_fits(d, sim->heavy, sim->n_sm, &fits));
     int mode = sim->params.exec_mode;
     // AUTO: the persistent kernel wins while the update dominates the step; with long rows (mean
@@ -359,11 +361,17 @@ int32_t build_graph(db_sim* sim) {
     cudaStream_t cap = nullptr;
     CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
     CK(cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
-    for (int s = 0; s < steps; ++s) {
-        launch_update(sim->dev, sim->update_sm, cap);
-        launch_deliver(sim->dev, sim->deliver_grid, cap);
+    cudaError_t le = cudaSuccess;
+    for (int s = 0; s < steps && le == cudaSuccess; ++s) {
+        le = launch_update(sim->dev, sim->update_sm, cap);
+        if (le == cudaSuccess) le = launch_deliver(sim->dev, sim->deliver_grid, cap);
     }
     cudaError_t e = cudaStreamEndCapture(cap, &graph);
+    if (le != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaStreamDestroy(cap);
+        return fail(sim, DB_ECUDA, std::string("graph capture (launch): ") + cudaGetErrorString(le));
+    }
     if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail(sim, DB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
     e = cudaGraphInstantiate(&sim->graph_exec, graph, 0);
     cudaGraphDestroy(graph);
@@ -390,6 +398,9 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     if (!out) return fail(nullptr, DB_EINVAL, "out is NULL");
     *out = nullptr;
     if (!csr || !csr->row_ptr || !csr->ntype || !csr->region_start) return fail(nullptr, DB_EINVAL, "csr is incomplete");
+    if (csr->N < 1 || csr->N >= (1ll << 30)) return fail(nullptr, DB_EINVAL, "N must be within 1..2^30-1");
+    if (csr->E < 0) return fail(nullptr, DB_EINVAL, "E must be >= 0");
+    if (csr->n_regions < 1 || csr->n_regions > 65536) return fail(nullptr, DB_EINVAL, "n_regions must be 1..65536");
     db_sim* sim = new (std::nothrow) db_sim();
     if (!sim) return fail(nullptr, DB_ENOMEM, "host allocation failed");
     auto bail = [&](int32_t rc) { g_create_error = sim->err; dev_free_all(sim); delete sim; return rc; };
@@ -397,8 +408,10 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     if ((rc = check_sim_params(sim, sp))) return bail(rc);
     if ((rc = open_device(sim, rt))) return bail(rc);
     const int64_t N = csr->N, E = csr->E;
-    if (E < 0 || csr->row_ptr[0] != 0 || csr->row_ptr[N] != E) return bail(fail(sim, DB_EINVAL, "row_ptr must run from 0 to E"));
+    if (csr->row_ptr[0] != 0 || csr->row_ptr[N] != E) return bail(fail(sim, DB_EINVAL, "row_ptr must run from 0 to E"));
     if (E > 0 && (!csr->tgt || !csr->w || !csr->delay || !csr->rec)) return bail(fail(sim, DB_EINVAL, "csr arrays missing"));
+    for (int64_t j = 0; j < N; ++j)                     // before any array is walked up to E
+        if (csr->row_ptr[j + 1] < csr->row_ptr[j]) return bail(fail(sim, DB_EINVAL, "row_ptr must be non-decreasing"));
     int32_t max_delay = 0;
     for (int64_t e = 0; e < E; ++e) max_delay = std::max<int32_t>(max_delay, csr->delay[e]);
     if (max_delay >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
@@ -563,9 +576,9 @@ int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
     while (sim->prof_events.size() < 2 * batch + 1) {
         cudaEvent_t e; CK(cudaEventCreate(&e)); sim->prof_events.push_back(e);
     }
-    uint32_t left = n_steps;
+    uint32_t left = n_steps, since_bold = 0;
     while (left) {
-        const uint32_t b = std::min(left, batch);
+        const uint32_t b = std::min(std::min(left, batch), sim->params.bold.enabled ? std::max(sim->bold_batch, 1u) : batch);
         CK(cudaEventRecord(sim->prof_events[0], sim->stream));
         for (uint32_t s = 0; s < b; ++s) {
             CK(launch_update(sim->dev, sim->update_sm, sim->stream));
@@ -585,6 +598,12 @@ int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
         CK(cudaEventElapsedTime(&t, sim->prof_events[0], sim->prof_events[2 * b]));
         out->total_ms += t;
         left -= b;
+        since_bold += b;
+        if (sim->params.bold.enabled && (since_bold + batch > sim->bold_batch || left == 0)) {   // before the count history wraps
+            CK(launch_bold(sim->dev, sim->bold, sim->stream));
+            sim->launches += 2;
+            since_bold = 0;
+        }
     }
     if ((rc = read_ctl(sim, &c1))) return rc;
     out->steps = c1.step - c0.step; out->spikes = c1.spike_begin - c0.spike_begin; out->events = c1.events - c0.events;
@@ -648,7 +667,7 @@ int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint
     const uint64_t m = scan_end - scan_begin;
     if (m >= 2048) {                    // long ranges: select and sort on the device (db_raster.cu)
         std::vector<unsigned long long> keys;
-        CK(raster_sorted_keys(sim->dev, scan_begin, m, (uint32_t)step_begin, (uint32_t)(step_end - step_begin), n, &keys, sim->stream));
+        CK(raster_sorted_keys(sim->dev, sim->n_sm, scan_begin, m, (uint32_t)step_begin, (uint32_t)(step_end - step_begin), n, &keys, sim->stream));
         if (keys.size() < n || keys[(size_t)n - 1] == ~0ull || (keys.size() > n && keys[(size_t)n] != ~0ull))
             return fail(sim, DB_ESTATE, "raster log is inconsistent");
         for (uint64_t o = 0; o < n && o < cap; ++o) {
@@ -730,7 +749,7 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
             int32_t* tmp = nullptr;
             if (cudaMalloc(&tmp, cells * 4) != cudaSuccess) { cudaGetLastError(); return fail(sim, DB_ENOMEM, "no device memory for the ring read-out"); }
             cudaError_t e = cudaMemsetAsync(tmp, 0, cells * 4, sim->stream);
-            if (e == cudaSuccess) e = launch_pending_ring(d, tmp, (int)first, (int)count, D, sim->stream);
+            if (e == cudaSuccess) e = launch_pending_ring(d, sim->n_sm, tmp, (int)first, (int)count, D, sim->stream);
             std::vector<int32_t> pend(cells);
             if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
             if (e == cudaSuccess) e = cudaMemcpy(pend.data(), tmp, cells * 4, cudaMemcpyDeviceToHost);
@@ -775,6 +794,10 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
         Ctl c;
         int32_t rc = read_ctl(sim, &c);
         if (rc) return rc;
+        // deferred mode: what DB_FIELD_RING shows is the device ring plus the near segments not pushed yet; once spikes
+        // may be pending a write could not be read back as written (and the old segments would still be pushed)
+        if (d.near_max > 0 && c.step > 0)
+            return fail(sim, DB_ESTATE, "DB_FIELD_RING is writable only before the first step in DB_EXEC_KERNELS_DEFERRED mode");
         const int D = sim->params.D;
         std::vector<int32_t> t((size_t)count);
         const int32_t* in = static_cast<const int32_t*>(src);
@@ -921,15 +944,6 @@ int32_t db_export_csr(db_sim* sim, db_csr_host* out) {
     }
     return DB_OK;
 }
-
-#ifdef DB_TRACE
-// Debugging builds only (not part of the ABI): per-block phase timestamps of the persistent kernel.
-int32_t db_debug_set_trace(db_sim* sim, void* dev_buf) {
-    if (!sim) return DB_EINVAL;
-    sim->dev.trace = static_cast<unsigned long long*>(dev_buf);
-    return DB_OK;
-}
-#endif
 
 int32_t db_free_csr(db_csr_host* c) {
     if (!c) return DB_EINVAL;

@@ -93,7 +93,6 @@ struct SimDev {                      // passed by value to every kernel
     uint32_t max_windows;
     unsigned long long* bg_parts;    // [kBgParts]
     Ctl* ctl;
-    unsigned long long* trace;       // debugging builds (-DDB_TRACE) only: per-block phase timestamps
     TypeConst tc[kMaxTypes];
 };
 

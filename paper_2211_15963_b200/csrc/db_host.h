@@ -11,20 +11,22 @@ namespace dbk {
 
 // ---- db_step.cu ------------------------------------------------------------
 cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
+cudaError_t prepare_kernels();                                            // per handle, on its device: opt-in shared-memory sizes
 cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st);
 cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);   // deferred variant when p.near_max > 0
 // DB_EXEC_KERNELS_DEFERRED: sort the rows [row0, row1) by delay into scratch arrays indexed by (synapse - s0) and fill
 // their segment tables; add the not yet pushed near segments to a DB_FIELD_RING read-out
-cudaError_t launch_sort_rows(const SimDev& p, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
+cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
                              uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st);
-cudaError_t launch_pending_ring(const SimDev& p, int32_t* out, int first, int count, int D_api, cudaStream_t st);
+cudaError_t launch_pending_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st);
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 
 // ---- db_raster.cu ----------------------------------------------------------
 // sorted keys (step - step_begin) << 32 | id of the raster entries at positions [scan_begin, scan_begin + m) whose step
 // lies in [lo, lo + span); entries of other steps sort behind them as ~0
-cudaError_t raster_sorted_keys(const SimDev& p, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
+cudaError_t raster_pool_setup(int device);                                 // per handle: keep the read-back scratch in the stream-ordered pool
+cudaError_t raster_sorted_keys(const SimDev& p, int n_sm, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
                                std::vector<unsigned long long>* keys_host, cudaStream_t st);
 
 // ---- db_bold.cu ------------------------------------------------------------

@@ -3,7 +3,18 @@
 // delivery is a scatter of such reductions; when the ring is far larger than L2 every one of them is a random
 // 32-byte-sector DRAM access, and the bound that matters is the device's random-access rate, not its streaming
 // bandwidth.  bench.py reports the delivery kernels against this number next to the HBM roofline.
-#include "db_host.h"
+//
+// Built into its own bench-only helper library (libdb_probe.so), NOT into libdb_b200.so: it is not part of the product ABI.
+//   int32_t db_probe_scatter(int32_t device, uint64_t region_bytes, uint64_t n_ops, uint32_t reps, double* ops_per_s)
+//   `n_ops` reductions per launch into a scratch region of `region_bytes` (allocated and freed inside; >= 4), `reps` timed
+//   launches after one warm-up, CUDA events on the default stream; *ops_per_s: HOST.  Returns 0, or -1 bad argument,
+//   -2 out of memory, -3 CUDA error.
+#include <cstdint>
+#include <cuda_runtime.h>
+#define DB_OK 0
+#define DB_EINVAL (-1)
+#define DB_ENOMEM (-2)
+#define DB_ECUDA (-3)
 
 namespace dbk {
 

@@ -19,21 +19,21 @@ __global__ void __launch_bounds__(256) k_raster_keys(const __grid_constant__ Sim
 }
 
 // keys_host gets min(n + 1, m) keys (the one after the last is there for the consistency check of the caller).
-cudaError_t raster_sorted_keys(const SimDev& p, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
+// Keep the scratch of the last calls in the device's stream-ordered pool (default: everything goes back to the OS at
+// every synchronize).  The pool belongs to the device: set once per handle, on the handle's device.
+cudaError_t raster_pool_setup(int device) {
+    cudaMemPool_t pool = nullptr;
+    unsigned long long keep = 256ull << 20;
+    cudaError_t e = cudaDeviceGetDefaultMemPool(&pool, device);
+    if (e == cudaSuccess) e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    return e;
+}
+
+cudaError_t raster_sorted_keys(const SimDev& p, int n_sm, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
                                std::vector<unsigned long long>* keys_host, cudaStream_t st) {
     unsigned long long *a = nullptr, *b = nullptr;
     void* tmp = nullptr;
     size_t tmp_bytes = 0;
-    static bool pool_set = false;                       // keep the scratch of the last calls in the stream-ordered pool
-    if (!pool_set) {                                    // (default: everything goes back to the OS at every synchronize)
-        int dev = 0;
-        cudaMemPool_t pool = nullptr;
-        unsigned long long keep = 256ull << 20;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess)
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        cudaGetLastError();
-        pool_set = true;
-    }
     cudaError_t e = cudaMallocAsync(&a, (size_t)m * 8, st);
     if (e == cudaSuccess) e = cudaMallocAsync(&b, (size_t)m * 8, st);
     int end_bit = 33;                                   // bits of (span - 1) above the id word, + the sentinel's
@@ -42,7 +42,7 @@ cudaError_t raster_sorted_keys(const SimDev& p, uint64_t scan_begin, uint64_t m,
     if (e == cudaSuccess) e = cub::DeviceRadixSort::SortKeys(nullptr, tmp_bytes, a, b, (int64_t)m, 0, end_bit, st);
     if (e == cudaSuccess) e = cudaMallocAsync(&tmp, tmp_bytes ? tmp_bytes : 16, st);
     if (e == cudaSuccess) {
-        const unsigned grid = (unsigned)std::min<uint64_t>((m + 255) / 256, 148ull * 16);
+        const unsigned grid = (unsigned)std::min<uint64_t>((m + 255) / 256, (uint64_t)n_sm * 16);
         k_raster_keys<<<grid, 256, 0, st>>>(p, scan_begin, m, lo, span, a);
         e = cudaGetLastError();
     }

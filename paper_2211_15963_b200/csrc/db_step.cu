@@ -582,18 +582,6 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     }
 }
 
-#ifdef DB_TRACE
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-#define DB_TRACE_MARK(s, k) do { if (p.trace && threadIdx.x == 0 && (s) < 64u) \
-    p.trace[((size_t)blockIdx.x * 64u + (s)) * 4u + (k)] = globaltimer_ns(); } while (0)
-#else
-#define DB_TRACE_MARK(s, k) do { } while (0)
-#endif
-
 struct RunCtx {                      // per-thread constants of the persistent kernel
     unsigned long long n0;           // step at launch
     int task0, last, i00, task_stride;
@@ -613,7 +601,6 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         __syncwarp();
         __threadfence_block();
     }
-    DB_TRACE_MARK(j, 0);
     if (c.task0 < c.last) {
         if (kB) request_ring(p, sg, p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * (size_t)p.Npad + c.i00);
         cp_async_commit();
@@ -623,7 +610,6 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
         }
         if (j < cfg.n_steps) { request_state(p, sg, c.i00); cp_async_commit(); }   // own data: no need to wait for the grid
     }
-    DB_TRACE_MARK(j, 1);
     if (!kHeavy) {                     // no block barrier: the warp reports to the service warp and moves on
         __syncwarp();
         if (c.lane == 0) {
@@ -650,8 +636,6 @@ __device__ __forceinline__ void run_unit(const SimDev& p, const RunCfg& cfg, con
             __syncthreads();
         }
     }
-    DB_TRACE_MARK(j, 2);
-    DB_TRACE_MARK(j, 3);
 }
 
 // The service warp of a block (its last warp; it owns no neurons).  Per unit j:
@@ -730,6 +714,7 @@ __device__ __noinline__ void service_warp(const SimDev& p, const RunCfg& cfg, co
                 p.spike_tag[(base + k2) & p.spike_mask] = (uint32_t)nA;
             }
         }
+        __syncwarp();                               // lane 0 must not let the unit that reuses spk[par] start while the others still copy
     }
     if (c.lane == 0) {
         if (bs->events) atomicAdd(&ctl->events, bs->events);     // every emit of the block lies before the last barrier
@@ -1199,14 +1184,14 @@ cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStr
 
 void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg);
 
+// Function attributes belong to the device context: called once per handle (finish_setup), on the handle's device.
+cudaError_t prepare_kernels() {
+    cudaError_t e = cudaFuncSetAttribute(k_update_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_update_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+    return e;
+}
+
 cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_update_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_update_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     int grid = 0, threads = 0;
     RunCfg cfg{};
     run_shape(p, n_sm, &grid, &threads, &cfg);
@@ -1226,9 +1211,9 @@ cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_sort_rows(const SimDev& p, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
+cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
                              uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st) {
-    const int grid = (int)std::min<int64_t>((row1 - row0 + kSortWarps - 1) / kSortWarps, 148 * 16);
+    const int grid = (int)std::min<int64_t>((row1 - row0 + kSortWarps - 1) / kSortWarps, (int64_t)n_sm * 16);
     if (grid <= 0) return cudaSuccess;
     if (p.w_fp16) k_sort_rows<true><<<grid, kSortWarps * 32, 0, st>>>(p.row_begin, p.row_len, p.tgt_rec, p.w, p.delay, row0, row1,
                                                                      s0, tgt_out, w_out, delay_out, seg, near_max);
@@ -1237,9 +1222,9 @@ cudaError_t launch_sort_rows(const SimDev& p, int64_t row0, int64_t row1, int64_
     return cudaGetLastError();
 }
 
-cudaError_t launch_pending_ring(const SimDev& p, int32_t* out, int first, int count, int D_api, cudaStream_t st) {
-    if (p.w_fp16) k_pending_ring<true><<<148 * 4, 256, 0, st>>>(p, out, first, count, D_api);
-    else          k_pending_ring<false><<<148 * 4, 256, 0, st>>>(p, out, first, count, D_api);
+cudaError_t launch_pending_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st) {
+    if (p.w_fp16) k_pending_ring<true><<<n_sm * 4, 256, 0, st>>>(p, out, first, count, D_api);
+    else          k_pending_ring<false><<<n_sm * 4, 256, 0, st>>>(p, out, first, count, D_api);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,216 @@
+"""Parity cases for the kernel paths VERDICT round 1 found unreached: I_ext != 0 with different constants per neuron
+type, the paper's production step dt = 1 ms (long Poisson table, R = 5 steps), region-rate windows of 1, 2 and 3 steps,
+a synchronised burst that overflows the per-block spike and heavy-row lists of the persistent kernel, and the ring's
+wrap / overflow flag.  Same bars as tests/test_gpu_parity.py (ring and counters bit-exact, raster identical, state
+within 1e-5 -- in fact equal), through the C ABI, in all three execution modes."""
+import numpy as np
+import pytest
+
+import db_inputs
+
+pytestmark = pytest.mark.gpu
+
+MODES = [1, 2, 3]   # DB_EXEC_KERNELS, DB_EXEC_PERSISTENT, DB_EXEC_KERNELS_DEFERRED
+
+
+@pytest.fixture(scope="module")
+def db():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2211_15963_b200 as m
+    m.load()
+    return m
+
+
+def _check(g, o, steps, ring=True, rel=1e-5):
+    Vg, gg, rg = g.state()
+    Vo, go, ro = o.state()
+    assert np.array_equal(rg, ro)
+    assert np.all(np.abs(Vg - Vo) <= rel * np.abs(Vo)) and np.all(np.abs(gg - go) <= rel * np.abs(go))
+    assert np.array_equal(Vg, Vo.astype(np.float32)) and np.array_equal(gg, go.astype(np.float32))
+    if ring:
+        assert np.array_equal(g.db_read_state(7), o.ring())
+    sg, ig = g.db_read_spikes(0, steps)
+    so, io = o.spikes()
+    order = np.lexsort((io, so))
+    assert np.array_equal(sg, so[order]) and np.array_equal(ig, io[order])
+    cg, co = g.db_get_counters(), o.counters()
+    for k in ("steps", "spikes", "events", "bg_events"):
+        assert cg[k] == co[k], k
+    assert cg["ring_overflow"] == co["overflow"]
+    return len(ig)
+
+
+def _distinct_types():
+    exc = db_inputs.type_params(bg_weight=0.009)
+    exc.update(Iext=0.21, G=[1.1, 0.3, 0.9, 1.2], E=[2.0, -3.0, -72.0, -95.0], tau_ms=[2.5, 35.0, 8.0, 60.0])
+    inh = db_inputs.type_params(bg_weight=0.006, bg_rate_hz=1500.0)
+    inh.update(Iext=-0.05, C=0.8, gL=0.04, VL=-70.0, Vth=-52.0, Vreset=-60.0, Tref_ms=2.0,
+               G=[0.8, 0.2, 1.3, 0.7], E=[0.0, 1.0, -75.0, -90.0], tau_ms=[1.5, 50.0, 12.0, 40.0])
+    return exc, inh
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_iext_and_different_constants_per_type(db, oracle_mod, mode):
+    # I_ext is non-zero and of opposite sign on the two types; every other constant differs too
+    exc, inh = _distinct_types()
+    sim = db_inputs.sim_params(types=[exc, inh])
+    N = 6000 + 19
+    net = db_inputs.random_csr(N=N, mean_outdeg=30, seed=31, n_regions=3)       # type boundaries inside 4-neuron groups
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    for upto in (1, 2, 60, 500):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        n = _check(g, o, upto)
+    ids = g.db_read_spikes(0, 500)[1]
+    assert np.count_nonzero(net["ntype"][ids] == 0) > 100 and np.count_nonzero(net["ntype"][ids] == 1) > 100
+    # the external current matters: without it the raster is another one
+    exc0, inh0 = dict(exc, Iext=0.0), dict(inh, Iext=0.0)
+    h = db.Sim.db_create_from_csr(db_inputs.sim_params(types=[exc0, inh0]), net, exec_mode=mode)
+    h.db_step(500)
+    assert len(h.db_read_spikes(0, 500)[1]) != n
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("bin_steps", [1])
+def test_production_step_dt_1ms(db, oracle_mod, mode, bin_steps):
+    # the paper's production step: dt = 1 ms, so lambda = 1 background event per step (the long Poisson
+    # table: up to 12 thresholds are walked), R = 5 steps, b_t = 1 step = 1 ms, delays 1..20 ms
+    t = db_inputs.type_params(bg_weight=0.005, bg_rate_hz=1000.0)
+    sim = db_inputs.sim_params(dt_ms=1.0, D=32, window_steps=5, types=[t, dict(t)], spike_bin_steps=bin_steps)
+    N = 8000 + 5
+    net = db_inputs.random_csr(N=N, mean_outdeg=40, seed=17, heavy_rows={3: 2500})
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    for upto in (1, 5, 100, 1000):                                  # 1 s of biological time
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        n = _check(g, o, upto)
+    rate = n / N / 1.0
+    assert 1.0 < rate < 60.0, rate
+    assert g.db_get_counters()["bg_events"] > 0.9 * N * 1000
+    cnt, first = g.db_region_counts()
+    assert np.array_equal(cnt, o.region_counts()[first:first + len(cnt)]) and len(cnt) == 200
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("window", [1, 2, 3])
+def test_region_windows_shorter_than_the_pipeline(db, oracle_mod, mode, window):
+    # windows of 1, 2 and 3 steps with several regions: the persistent kernel's blocks run up to two units apart, so the
+    # window that is cleared ahead and the windows still being counted are only a few cells apart
+    t = db_inputs.type_params(bg_weight=0.03)
+    sim = db_inputs.sim_params(window_steps=window, types=[t, dict(t)])
+    N, R = 20000 + 3, 6
+    net = db_inputs.random_csr(N=N, mean_outdeg=15, seed=23, n_regions=R)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode, max_windows=64)     # a short history: it wraps many times
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    done = 0
+    for upto in (1, 2, 3, 7, 150, 151, 400):
+        g.db_step(upto - done); o.step(upto - done)
+        done = upto
+        cnt, first = g.db_region_counts()
+        want = o.region_counts()
+        assert len(cnt) == min(upto // window, 64 - 1 - (2 // window + 1))
+        assert first + len(cnt) == upto // window
+        assert np.array_equal(cnt, want[first:first + len(cnt)]), (upto, first)
+    assert cnt.sum() > 100 and np.all(cnt.sum(axis=0) > 0)
+    _check(g, o, 400)
+    # single region, same windows (counted per block and unit in the persistent kernel)
+    net1 = db_inputs.random_csr(N=5000, mean_outdeg=15, seed=24)
+    g1 = db.Sim.db_create_from_csr(sim, net1, exec_mode=mode, max_windows=32)
+    o1 = oracle_mod.OracleSim(sim, net1, db_inputs.DYN_SEED)
+    g1.db_step(333); o1.step(333)
+    cnt, first = g1.db_region_counts()
+    assert np.array_equal(cnt, o1.region_counts()[first:first + len(cnt)]) and cnt.sum() > 50
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_synchronised_burst_overflows_the_block_lists(db, oracle_mod, mode):
+    # P:L490 worries about synchronised activity; here EVERY neuron of a 400,037-neuron network fires in step 0.  One block
+    # of the persistent kernel owns ~2,800 neurons (> kSpkCap = 1024 staged spikes: the rest reserve raster positions
+    # straight from the global cursor) and 640 of the first 2,700 rows are longer than kInlineMax = 1024 synapses
+    # (> kHeavyListCap = 512 deferred heavy rows: the rest are pushed by the warp that found them).
+    N = 400_000 + 37
+    rng = np.random.default_rng(5)
+    heavy = {int(r): int(d) for r, d in zip(rng.choice(2700, 640, replace=False), rng.integers(1025, 1400, 640))}
+    heavy.update({150_000: 20_000, 399_999: 3000})
+    net = db_inputs.bulk_csr(N, base_outdeg=3, seed=9, heavy_rows=heavy)
+    t = db_inputs.type_params(bg_weight=0.03)
+    sim = db_inputs.sim_params(types=[t, dict(t)])
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    assert g.db_get_counters()["exec_mode"] == mode
+    V, gg, ref = o.state()
+    V[:] = -45.0                                                   # above threshold: flagged in step 0
+    o.set_state(V, gg, ref); g.set_state(V.astype(np.float32), gg.astype(np.float32), ref)
+    g.db_step(1); o.step(1)
+    assert g.db_get_counters()["spikes"] == N
+    assert _check(g, o, 1) == N
+    g.db_step(1); o.step(1)
+    _check(g, o, 2)
+    g.db_step(118); o.step(118)                                    # past the refractory period: ordinary activity again
+    n = _check(g, o, 120)
+    assert n > N + 1000
+    # a second burst in the middle of a run (odd unit parity of the kernel's double-buffered lists)
+    V, gg, ref = o.state()
+    V[:] = -45.0
+    ref[:] = 0
+    o.set_state(V, gg, ref); g.set_state(V.astype(np.float32), gg.astype(np.float32), ref)
+    g.db_step(3); o.step(3)
+    assert g.db_get_counters()["spikes"] >= n + N
+    _check(g, o, 123)        # (deferred mode: the near segments pending across the state write are still pushed)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_ring_wrap_and_overflow_flag(db, oracle_mod, mode):
+    # R28: the same two's-complement wrap and the same sticky flag on both sides (tests/test_oracle_pins_current.py pins
+    # the oracle's: three pushes of 300 * 2^22 wrap to -520,093,696; a consumed cell beyond 2^30 raises the flag)
+    t = db_inputs.type_params(bg_weight=0.0, bg_rate_hz=0.0)
+    sim = db_inputs.sim_params(D=8, types=[t, dict(t)])
+    net = dict(N=4, n_regions=1, region_start=np.array([0, 4]), ntype=np.zeros(4, np.uint8),
+               row_ptr=np.array([0, 1, 2, 3, 3], np.int64), tgt=np.array([3, 3, 3], np.int32),
+               w=np.array([300.0] * 3, np.float32), delay=np.array([2, 2, 2], np.uint8), rec=np.zeros(3, np.uint8))
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    V, gg, ref = o.state()
+    V[:3], V[3] = -40.0, t["VL"]
+    o.set_state(V, gg, ref); g.set_state(V.astype(np.float32), gg.astype(np.float32), ref)
+    g.db_step(1); o.step(1)
+    ring = g.db_read_state(7)
+    assert ring[2, 3, 0] == -520093696 and np.array_equal(ring, o.ring())
+    g.db_step(2); o.step(2)
+    _check(g, o, 3)
+    assert g.db_get_counters()["ring_overflow"] == 0
+    g.db_step(3); o.step(3)
+    _check(g, o, 6)
+    # trip the flag: a cell of 2^30 + 1 (and -2^30 - 1), consumed in the next step; 2^30 itself does not trip it
+    lone = dict(net, row_ptr=np.zeros(5, np.int64), tgt=np.zeros(0, np.int32), w=np.zeros(0, np.float32),
+                delay=np.zeros(0, np.uint8), rec=np.zeros(0, np.uint8))
+    for val, trips in ((1 << 30, 0), (-(1 << 30), 0), ((1 << 30) + 1, 1), (-(1 << 30) - 1, 1)):
+        g = db.Sim.db_create_from_csr(sim, lone, exec_mode=mode)
+        o = oracle_mod.OracleSim(sim, lone, db_inputs.DYN_SEED)
+        r = np.zeros((8, 4, 4), np.int32)
+        r[0, 1, 2] = val
+        g.db_write_state(7, r); o.set_ring(r)
+        g.db_step(1); o.step(1)
+        assert g.db_get_counters()["ring_overflow"] == trips == o.counters()["overflow"]
+        g.db_step(4); o.step(4)
+        assert g.db_get_counters()["ring_overflow"] == trips == o.counters()["overflow"]     # sticky
+        assert np.array_equal(g.state()[1], o.state()[1].astype(np.float32))
+
+
+def test_deferred_mode_ring_write_after_the_first_step_is_refused(db):
+    # in deferred mode the ring the API shows is the device ring plus the near segments not pushed yet; once spikes may be
+    # pending a write could not be read back as written, so it is refused (include/db_b200.h, db_write_state)
+    net = db_inputs.random_csr(N=600, mean_outdeg=10, seed=2)
+    sim = db_inputs.sim_params()
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=3)
+    assert g.db_get_counters()["exec_mode"] == 3
+    r = np.zeros((sim["D"], 600, 4), np.int32)
+    r[3, 5, 1] = 77
+    g.db_write_state(7, r)                         # step 0: nothing pending
+    assert np.array_equal(g.db_read_state(7), r)
+    g.db_step(2)
+    with pytest.raises(db.DbError) as e:
+        g.db_write_state(7, r)
+    assert e.value.code == db.binding.DB_ESTATE
+    g.db_write_state(0, np.full(600, -60.0, np.float32))            # the other fields stay writable
