@@ -83,10 +83,11 @@ typedef struct db_bold_params {
 #define DB_EXEC_AUTO       0   /* library picks */
 #define DB_EXEC_KERNELS    1   /* two kernels per step (update+compaction, delivery), CUDA-graph replayed */
 #define DB_EXEC_PERSISTENT 2   /* one cooperative persistent kernel looping over the steps */
-#define DB_EXEC_KERNELS_DEFERRED 3 /* two kernels per step; synapses with a short delay are pushed in the step before
-                                      they arrive, out of the spike lists of the last steps (rows sorted by delay), so
-                                      that all those reductions hit ONE ring slot, which stays in L2; same results.  Falls back to
-                                      DB_EXEC_KERNELS when no delay exceeds 1 or the raster ring cannot hold the spikes of 31 steps */
+#define DB_EXEC_KERNELS_DEFERRED 3 /* two kernels per step with ARRIVAL LISTS: a row is read once, when its neuron fires, and every
+                                      synapse becomes an 8-byte record in the list of its arrival step (rows sorted by delay, one
+                                      atomic per run); the kernel of step n streams the list of step n + 1 into ring slot n + 1, the
+                                      only slot that takes reductions, so they stay in L2 and DRAM only streams.  Same results.
+                                      Falls back to DB_EXEC_KERNELS when no delay exceeds 1 step or memory is short */
 
 typedef struct db_sim_params {
     uint32_t struct_size;     /* = sizeof(db_sim_params) */
@@ -105,8 +106,7 @@ typedef struct db_sim_params {
                                  transferred at the end of its bin, step n_k = b_t floor(n / b_t) + b_t - 1, and a
                                  synapse of delay d is read in step n_k + d.  0 or 1: every step is a boundary.
                                  Needs b_t <= R + 1 of every type (A_j is 0 or 1) and largest delay + b_t - 1 < D;
-                                 DB_EXEC_KERNELS_DEFERRED falls back to DB_EXEC_KERNELS when b_t > 1.
-                                 DB_FIELD_RING already holds the pushes of the spikes of the open bin. */
+                                                                  DB_FIELD_RING already holds the pushes of the spikes of the open bin. */
     db_bold_params bold;      /* BOLD read-out per region, fed by the region-rate windows (off by default) */
 } db_sim_params;
 
@@ -172,6 +172,8 @@ typedef struct db_counters {
     uint32_t ring_overflow;/* sticky: some consumed ring cell exceeded 2^30 in magnitude (R28) */
     uint32_t exec_mode;    /* DB_EXEC_* actually in use */
     uint64_t launches;     /* kernels launched by db_step / db_step_profiled on this handle */
+    uint64_t list_spilled; /* DB_EXEC_KERNELS_DEFERRED: records that found their arrival list full and were reduced into
+                              the ring directly (exact either way; a capacity diagnostic) */
 } db_counters;
 
 /* Per-phase device time of the last db_step_profiled() call, in milliseconds. */

@@ -88,7 +88,7 @@ class CsrHost(C.Structure):
 
 class Counters(C.Structure):
     _fields_ = [("steps", C.c_uint64), ("spikes", C.c_uint64), ("events", C.c_uint64), ("bg_events", C.c_uint64),
-                ("ring_overflow", C.c_uint32), ("exec_mode", C.c_uint32), ("launches", C.c_uint64)]
+                ("ring_overflow", C.c_uint32), ("exec_mode", C.c_uint32), ("launches", C.c_uint64), ("list_spilled", C.c_uint64)]
 
 
 class PhaseTimes(C.Structure):

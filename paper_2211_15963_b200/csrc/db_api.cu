@@ -37,9 +37,12 @@ struct db_sim {
     int exec_mode = DB_EXEC_KERNELS;
     int deliver_grid = 0;
     bool heavy = false;             // some row is longer than kInlineMax
+    int32_t max_delay = 0;          // largest synaptic delay, in steps
+    double list_rate_hz = 0.0;      // arrival lists: mean firing rate their capacity was sized for
     int update_sm = 0;              // two-kernel mode: SM count the update kernel is shaped for
     cudaGraphExec_t graph_exec = nullptr;
     int graph_steps = 0;
+    uint64_t host_step = 0;         // steps launched so far (two-kernel modes: parity of the work-list half)
     uint64_t launches = 0;
     std::vector<cudaEvent_t> prof_events;
     BoldDev bold{};                 // BOLD read-out (params.bold.enabled)
@@ -268,19 +271,74 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
     return DB_OK;
 }
 
-// DB_EXEC_KERNELS_DEFERRED: sort every row by delay (on the device, batch by batch through scratch
-// arrays) and build the segment table.  near_max = largest delay whose push is deferred.
-int32_t build_delay_segments(db_sim* sim, int near_max) {
+// DB_EXEC_KERNELS_DEFERRED: size and allocate the arrival lists, then sort every row by (delay, target window) on the
+// device, batch by batch through scratch arrays.  *ok = false (and nothing changed) when the network has nothing to
+// list or the lists do not fit in memory: the caller falls back to DB_EXEC_KERNELS.
+int32_t build_arrival_lists(db_sim* sim, bool* ok) {
     SimDev& d = sim->dev;
+    *ok = false;
     const int64_t N = d.N;
+    const int max_ahead = sim->max_delay + d.bin_steps - 1;        // furthest arrival, in steps after the spike
+    if (max_ahead <= 1 || sim->Epad < 16) return DB_OK;
+    // synapses per delay
+    unsigned long long* hist_dev = nullptr;
+    int32_t rc = alloc_zero(sim, &hist_dev, 256);
+    if (rc) return rc;
+    CK(launch_delay_hist(d.delay, sim->Epad, hist_dev, sim->n_sm, sim->stream));
+    unsigned long long hist[256];
+    CK(cudaStreamSynchronize(sim->stream));
+    CK(cudaMemcpy(hist, hist_dev, sizeof(hist), cudaMemcpyDeviceToHost));
+    const int Dn = std::min(d.D, 32), near_lim = std::max(Dn - 3, 0);
+    double e_near = 0.0, e_far = 0.0;
+    for (int dl = 1; dl < 256; ++dl) ((dl + d.bin_steps - 1 <= near_lim) ? e_near : e_far) += (double)hist[dl];
+    // target windows: one ring slot (16 B per neuron) is swept window by window, each window small enough to stay in L2
+    int W = 1;
+    while (W < 4 && 16.0 * (double)d.Npad / W > 48.0 * 1048576.0) W *= 2;
+    // parallel lists per (slot, window): atomics on one cursor serialise in L2 (~90 ns each, profiles/), so the records
+    // of a step are spread over enough cursors that each sees a few dozen reservations per step
+    const double ev_step = (e_near + e_far) * 30.0 * sim->params.dt_ms * 1e-3;      // records per step at 30 Hz
+    int P = 8;
+    while (P < 256 && ev_step / (W * P) > 16384.0) P *= 2;
+    const int64_t win = ((((int64_t)d.Npad + W - 1) / W + kNeuronPad - 1) / kNeuronPad) * kNeuronPad;
+    // capacity: the records of one step at the design rate, split over the lists of a slot; any excess spills into the
+    // dense ring (exact, only slower).  Halve the design rate until the lists fit into half of the free memory.
+    size_t free_b = 0, total_b = 0;
+    CK(cudaMemGetInfo(&free_b, &total_b));
+    const double dt_s = sim->params.dt_ms * 1e-3;
+    uint64_t cap_near = 0, cap_far = 0, n_near = (uint64_t)Dn * W * P, n_far = e_far > 0 ? (uint64_t)d.D * W * P : 0;
+    double rate = 60.0;
+    for (;; rate *= 0.5) {
+        if (rate < 4.0) return DB_OK;                              // no room for useful lists
+        auto cap_of = [&](double synapses) {
+            const double per_list = synapses * rate * dt_s / (double)(W * P);
+            return (uint64_t)std::max(1024.0, std::ceil(per_list / 16.0) * 16.0);
+        };
+        cap_near = cap_of(e_near);
+        cap_far = n_far ? cap_of(e_far) : 0;
+        if ((double)(n_near * cap_near + n_far * cap_far) * 8.0 <= 0.5 * (double)free_b) break;
+    }
+    if (cap_near > 0xFFFFFFF0ull || cap_far > 0xFFFFFFF0ull) return DB_OK;
+    uint2* rec = nullptr;
+    unsigned* cnt = nullptr;
+    const size_t n_rec = (size_t)(n_near * cap_near + n_far * cap_far);
+    rec = static_cast<uint2*>(dev_alloc(sim, n_rec * sizeof(uint2)));
+    if (!rec) return DB_OK;                                        // fall back rather than fail
+    if ((rc = alloc_zero(sim, &cnt, (size_t)(n_near + n_far) * 8))) return rc;
+    d.ev_direct = 1; d.ev_near_lim = near_lim; d.ev_near_d = std::max(near_lim - (d.bin_steps - 1), 0); d.ev_Dn = Dn; d.ev_D = d.D; d.ev_W = W; d.ev_P = P;
+    d.ev_n_near = (int32_t)n_near; d.ev_n_far = (int32_t)n_far;
+    d.ev_cap_near = (uint32_t)cap_near; d.ev_cap_far = (uint32_t)cap_far;
+    for (int k = 0; k < 3; ++k) d.ev_wb[k] = (k + 1 < W) ? (uint32_t)std::min<int64_t>((int64_t)(k + 1) * win, 0x7FFFFFFF) : 0xFFFFFFFFu;
+    d.ev_rec = rec; d.ev_cnt = cnt;
+    sim->list_rate_hz = rate;
+    uint32_t* seg = nullptr;
+    if ((rc = alloc_zero(sim, &seg, (size_t)N * (size_t)(d.ev_near_d * W + 1)))) return rc;
+    d.seg = seg;
+
+    // sort the rows
     std::vector<int64_t> rb((size_t)N);
     std::vector<int32_t> rl((size_t)N);
-    CK(cudaStreamSynchronize(sim->stream));
     CK(cudaMemcpy(rb.data(), d.row_begin, (size_t)N * 8, cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(rl.data(), d.row_len, (size_t)N * 4, cudaMemcpyDeviceToHost));
-    uint32_t* seg = nullptr;
-    int32_t rc = alloc_zero(sim, &seg, (size_t)N * (size_t)(near_max + 1));
-    if (rc) return rc;
     auto row_end = [&](int64_t j) { return rb[(size_t)j] + ((int64_t)rl[(size_t)j] + kRowAlign - 1) / kRowAlign * kRowAlign; };
     const int64_t batch = std::min<int64_t>(sim->Epad, (int64_t)1 << 28);        // synapses per batch
     const size_t wsz = d.w_fp16 ? 2 : 4;
@@ -298,7 +356,7 @@ int32_t build_delay_segments(db_sim* sim, int near_max) {
         while (r1 < N && row_end(r1) - s0 <= batch) ++r1;
         const int64_t s1 = row_end(r1 - 1);
         if (s1 - s0 > batch) { out = fail(sim, DB_EINVAL, "a row is longer than the sorting batch"); break; }
-        cudaError_t e = launch_sort_rows(d, sim->n_sm, r0, r1, s0, t_s, w_s, d_s, seg, near_max, sim->stream);
+        cudaError_t e = launch_sort_rows(d, sim->n_sm, r0, r1, s0, t_s, w_s, d_s, seg, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint32_t*>(d.tgt_rec) + s0, t_s, (size_t)(s1 - s0) * 4, cudaMemcpyDeviceToDevice, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(const_cast<uint8_t*>(d.delay) + s0, d_s, (size_t)(s1 - s0), cudaMemcpyDeviceToDevice, sim->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync((char*)const_cast<void*>(d.w) + (size_t)s0 * wsz, w_s, (size_t)(s1 - s0) * wsz, cudaMemcpyDeviceToDevice, sim->stream);
@@ -308,17 +366,19 @@ int32_t build_delay_segments(db_sim* sim, int near_max) {
     }
     cudaFree(t_s); cudaFree(d_s); cudaFree(w_s);
     if (out) return out;
-    d.seg = seg;
-    d.near_max = near_max;
+    d.ev_on = 1;
+    sim->deliver_grid = sim->n_sm * 4;      // k_deliver_lists: four blocks of 256 threads per SM, all resident
+    *ok = true;
     return DB_OK;
 }
 
 // After the CSR is on the device: work list, execution mode, initial state.
-int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int32_t near_hint) {
+int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     SimDev& d = sim->dev;
     int32_t rc;
     sim->work_cap = std::max<uint64_t>(work_cap, 1);
-    if ((rc = alloc_zero(sim, &d.work, (size_t)sim->work_cap))) return rc;
+    d.work_half = sim->work_cap;
+    if ((rc = alloc_zero(sim, &d.work, 2 * (size_t)sim->work_cap))) return rc;
     sim->heavy = heavy_chunks > 0;
     CK(launch_init_state(d, sim->ntype_dev, sim->stream));
     sim->deliver_grid = sim->n_sm * 8;
@@ -334,19 +394,13 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int3
     // out-degree >= 400: configs 3 and 4) the step is delivery-bound and the two-kernel mode, where every
     // warp of the grid pushes rows, is faster (measured: profiles/)
     const bool delivery_bound = sim->heavy || (sim->E >= 400 * (int64_t)d.N);
-    // deferred delivery needs the spike lists of the last near_max steps in the raster ring: a neuron fires
-    // at most once per R + 1 steps
-    const int near_max = std::min<int32_t>(31, near_hint);
-    int r_min = d.tc[0].R;
-    for (int t = 1; t < sim->params.n_types; ++t) r_min = std::min(r_min, d.tc[t].R);
-    const bool can_defer = near_max >= 2 && d.bin_steps == 1 &&
-        (uint64_t)d.N * (uint64_t)((near_max + r_min) / (r_min + 1)) <= sim->spike_cap;
     if (mode == DB_EXEC_AUTO)
-        mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : (can_defer ? DB_EXEC_KERNELS_DEFERRED : DB_EXEC_KERNELS);
-    if (mode == DB_EXEC_KERNELS_DEFERRED && !can_defer) mode = DB_EXEC_KERNELS;   // nothing to defer, or the raster ring is too small
+        mode = (coop && fits && !delivery_bound) ? DB_EXEC_PERSISTENT : DB_EXEC_KERNELS_DEFERRED;
     if (mode == DB_EXEC_KERNELS_DEFERRED) {
-        int32_t rc2 = build_delay_segments(sim, near_max);
+        bool ok = false;
+        int32_t rc2 = build_arrival_lists(sim, &ok);
         if (rc2) return rc2;
+        if (!ok) mode = DB_EXEC_KERNELS;            // nothing to list (no delay beyond 1), or no memory for the lists
     }
     if (mode == DB_EXEC_PERSISTENT && (!coop || !fits))
         return fail(sim, DB_ECUDA, "cooperative launch not available for the persistent mode");
@@ -355,27 +409,66 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks, int3
     return DB_OK;
 }
 
+// One step on `st` (no overlap): update, delivery.  List mode: the update kernel is a unit (k_update_stream): `first`
+// marks the first step of a db_step call (A only).
+cudaError_t launch_step(db_sim* sim, bool first, cudaStream_t st) {
+    const int mode = sim->dev.ev_on ? (first ? 1 : 2) : 0;
+    cudaError_t e = launch_update(sim->dev, sim->update_sm, mode, st);
+    if (e == cudaSuccess) e = launch_deliver(sim->dev, sim->deliver_grid, (unsigned)(sim->host_step & 1ull), st);
+    sim->launches += 2;
+    sim->host_step += 1;
+    return e;
+}
+
+// A CUDA graph of 32 steps (an even number: it is replayed from even steps only, so the parity of a step inside it is
+// fixed).  In list mode the delivery kernel of step s runs on a second branch, beside the update kernel of step s + 1;
+// the update kernel of step s + 2 waits for it.
 int32_t build_graph(db_sim* sim) {
     const int steps = 32;
+    const bool fork = sim->dev.ev_on != 0;
+    const int mode = fork ? 2 : 0;
     cudaGraph_t graph = nullptr;
-    cudaStream_t cap = nullptr;
-    CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
-    CK(cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal));
-    cudaError_t le = cudaSuccess;
+    cudaStream_t cap = nullptr, side = nullptr;
+    std::vector<cudaEvent_t> ev;
+    auto cleanup = [&]() {
+        for (cudaEvent_t x : ev) cudaEventDestroy(x);
+        if (side) cudaStreamDestroy(side);
+        if (cap) cudaStreamDestroy(cap);
+    };
+    int prio_lo = 0, prio_hi = 0;                       // the update kernels get the SMs first; the delivery kernels fill in
+    CK(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    CK(cudaStreamCreateWithPriority(&cap, cudaStreamNonBlocking, prio_hi));
+    if (fork) {
+        if (cudaStreamCreateWithPriority(&side, cudaStreamNonBlocking, prio_lo) != cudaSuccess) { cleanup(); return fail(sim, DB_ECUDA, "stream creation failed"); }
+        ev.resize(2 * (size_t)steps);
+        for (auto& x : ev) if (cudaEventCreateWithFlags(&x, cudaEventDisableTiming) != cudaSuccess) { cleanup(); return fail(sim, DB_ECUDA, "event creation failed"); }
+    }
+    cudaError_t le = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (le != cudaSuccess) { cleanup(); return fail(sim, DB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(le)); }
     for (int s = 0; s < steps && le == cudaSuccess; ++s) {
-        le = launch_update(sim->dev, sim->update_sm, cap);
-        if (le == cudaSuccess) le = launch_deliver(sim->dev, sim->deliver_grid, cap);
+        if (fork) {
+            if (s >= 2) le = cudaStreamWaitEvent(cap, ev[2 * (size_t)(s - 2) + 1], 0);                  // delivery of step s - 2 done
+            if (le == cudaSuccess) le = launch_update(sim->dev, sim->update_sm, mode, cap);
+            if (le == cudaSuccess) le = cudaEventRecord(ev[2 * (size_t)s], cap);                       // update kernel of step s done
+            if (le == cudaSuccess) le = cudaStreamWaitEvent(side, ev[2 * (size_t)s], 0);
+            if (le == cudaSuccess) le = launch_deliver(sim->dev, sim->deliver_grid, (unsigned)(s & 1), side);
+            if (le == cudaSuccess) le = cudaEventRecord(ev[2 * (size_t)s + 1], side);
+        } else {
+            le = launch_update(sim->dev, sim->update_sm, mode, cap);
+            if (le == cudaSuccess) le = launch_deliver(sim->dev, sim->deliver_grid, (unsigned)(s & 1), cap);
+        }
     }
+    if (fork && le == cudaSuccess) le = cudaStreamWaitEvent(cap, ev[2 * (size_t)steps - 1], 0);        // join (the side branch is in order)
     cudaError_t e = cudaStreamEndCapture(cap, &graph);
-    if (le != cudaSuccess) {
+    if (le != cudaSuccess || e != cudaSuccess) {
         if (graph) cudaGraphDestroy(graph);
-        cudaStreamDestroy(cap);
-        return fail(sim, DB_ECUDA, std::string("graph capture (launch): ") + cudaGetErrorString(le));
+        cleanup();
+        cudaGetLastError();
+        return fail(sim, DB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(le != cudaSuccess ? le : e));
     }
-    if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail(sim, DB_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e)); }
     e = cudaGraphInstantiate(&sim->graph_exec, graph, 0);
     cudaGraphDestroy(graph);
-    cudaStreamDestroy(cap);
+    cleanup();
     if (e != cudaSuccess) return fail(sim, DB_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e));
     sim->graph_steps = steps;
     return DB_OK;
@@ -416,6 +509,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     for (int64_t e = 0; e < E; ++e) max_delay = std::max<int32_t>(max_delay, csr->delay[e]);
     if (max_delay >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
     if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start, max_delay))) return bail(rc);
+    sim->max_delay = max_delay;
     SimDev& d = sim->dev;
 
     // padded row layout + validation
@@ -469,7 +563,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
         return bail(fail(sim, DB_ECUDA, std::string("CSR upload: ") + cudaGetErrorString(cudaGetLastError())));
     d.row_begin = rb_dev; d.row_len = rl_dev; d.tgt_rec = tr_dev; d.delay = dl_dev; d.w = w_dev;
     d.w_fp16 = csr->weight_fp16 ? 1 : 0;
-    if ((rc = finish_setup(sim, work_cap, heavy_chunks, max_delay))) return bail(rc);
+    if ((rc = finish_setup(sim, work_cap, heavy_chunks))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -505,7 +599,8 @@ int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
     d.w_fp16 = spec->weight_fp16 ? 1 : 0;
     sim->E = gr.E; sim->Epad = gr.Epad;
     if (gr.max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
-    if ((rc = finish_setup(sim, gr.work_cap, gr.heavy_chunks, spec->delay_intra_max))) return bail(rc);
+    sim->max_delay = gr.max_delay;
+    if ((rc = finish_setup(sim, gr.work_cap, gr.heavy_chunks))) return bail(rc);
     *out = sim;
     return DB_OK;
 }
@@ -546,21 +641,32 @@ static int32_t step_batch(db_sim* sim, uint32_t n_steps) {
             const uint32_t b = std::min(left, cap);
             CK(launch_persistent(sim->dev, sim->heavy, b, sim->n_sm, sim->stream));
             sim->launches += 1;
+            sim->host_step += b;
             left -= b;
         }
         return DB_OK;
     }
-    if (!sim->graph_exec && n_steps >= 32) { int32_t rc = build_graph(sim); if (rc) return rc; }
+    if (!sim->graph_exec && n_steps >= 34) { int32_t rc = build_graph(sim); if (rc) return rc; }
     uint32_t left = n_steps;
+    const bool lists = sim->dev.ev_on != 0;
+    if (lists) {                                       // unit form: the first kernel of the call has no B part
+        CK(launch_step(sim, true, sim->stream));
+        left -= 1;
+    }
+    if (sim->graph_exec && left > (uint32_t)sim->graph_steps && (sim->host_step & 1ull)) {   // the graph starts on even steps
+        CK(launch_step(sim, false, sim->stream));
+        left -= 1;
+    }
     while (sim->graph_exec && left >= (uint32_t)sim->graph_steps) {
         CK(cudaGraphLaunch(sim->graph_exec, sim->stream));
         left -= (uint32_t)sim->graph_steps;
         sim->launches += 2ull * (uint64_t)sim->graph_steps;
+        sim->host_step += (uint64_t)sim->graph_steps;
     }
-    for (; left; --left) {
-        CK(launch_update(sim->dev, sim->update_sm, sim->stream));
-        CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
-        sim->launches += 2;
+    for (; left; --left) CK(launch_step(sim, false, sim->stream));
+    if (lists) {                                       // ... and the last one only a B part: the state is complete again
+        CK(launch_update(sim->dev, sim->update_sm, 3, sim->stream));
+        sim->launches += 1;
     }
     return DB_OK;
 }
@@ -580,12 +686,18 @@ int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
     while (left) {
         const uint32_t b = std::min(std::min(left, batch), sim->params.bold.enabled ? std::max(sim->bold_batch, 1u) : batch);
         CK(cudaEventRecord(sim->prof_events[0], sim->stream));
-        for (uint32_t s = 0; s < b; ++s) {
-            CK(launch_update(sim->dev, sim->update_sm, sim->stream));
+        for (uint32_t s = 0; s < b; ++s) {              // every kernel on the handle's stream, nothing overlapped
+            const int mode = sim->dev.ev_on ? (s == 0 ? 1 : 2) : 0;
+            CK(launch_update(sim->dev, sim->update_sm, mode, sim->stream));
             CK(cudaEventRecord(sim->prof_events[2 * s + 1], sim->stream));
-            CK(launch_deliver(sim->dev, sim->deliver_grid, sim->stream));
+            CK(launch_deliver(sim->dev, sim->deliver_grid, (unsigned)(sim->host_step & 1ull), sim->stream));
             CK(cudaEventRecord(sim->prof_events[2 * s + 2], sim->stream));
             sim->launches += 2;
+            sim->host_step += 1;
+        }
+        if (sim->dev.ev_on) {                           // (the B part of the batch's last step: not timed)
+            CK(launch_update(sim->dev, sim->update_sm, 3, sim->stream));
+            sim->launches += 1;
         }
         CK(cudaStreamSynchronize(sim->stream));
         for (uint32_t s = 0; s < b; ++s) {
@@ -628,6 +740,7 @@ int32_t db_get_counters(db_sim* sim, db_counters* out) {
     out->steps = c.step; out->spikes = c.spike_begin; out->events = c.events; out->bg_events = bg;
     out->ring_overflow = c.overflow; out->exec_mode = (uint32_t)sim->exec_mode;
     out->launches = sim->launches;
+    out->list_spilled = c.ev_spilled;
     return DB_OK;
 }
 
@@ -744,12 +857,12 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
                 for (int64_t i = 0; i < count; ++i) o[(s * (size_t)count + (size_t)i) * 4 + u] = t[(size_t)i];
             }
         }
-        if (d.near_max > 0) {          // deferred mode: plus the near segments not pushed yet
+        if (d.ev_on) {                 // list mode: plus the records waiting in the arrival lists
             const size_t cells = (size_t)D * (size_t)count * 4;
             int32_t* tmp = nullptr;
             if (cudaMalloc(&tmp, cells * 4) != cudaSuccess) { cudaGetLastError(); return fail(sim, DB_ENOMEM, "no device memory for the ring read-out"); }
             cudaError_t e = cudaMemsetAsync(tmp, 0, cells * 4, sim->stream);
-            if (e == cudaSuccess) e = launch_pending_ring(d, sim->n_sm, tmp, (int)first, (int)count, D, sim->stream);
+            if (e == cudaSuccess) e = launch_lists_to_ring(d, sim->n_sm, tmp, (int)first, (int)count, D, sim->stream);
             std::vector<int32_t> pend(cells);
             if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
             if (e == cudaSuccess) e = cudaMemcpy(pend.data(), tmp, cells * 4, cudaMemcpyDeviceToHost);
@@ -794,9 +907,9 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
         Ctl c;
         int32_t rc = read_ctl(sim, &c);
         if (rc) return rc;
-        // deferred mode: what DB_FIELD_RING shows is the device ring plus the near segments not pushed yet; once spikes
-        // may be pending a write could not be read back as written (and the old segments would still be pushed)
-        if (d.near_max > 0 && c.step > 0)
+        // list mode: what DB_FIELD_RING shows is the device ring plus the records waiting in the arrival lists; once
+        // records may be waiting a write could not be read back as written
+        if (d.ev_on && c.step > 0)
             return fail(sim, DB_ESTATE, "DB_FIELD_RING is writable only before the first step in DB_EXEC_KERNELS_DEFERRED mode");
         const int D = sim->params.D;
         std::vector<int32_t> t((size_t)count);

@@ -33,12 +33,15 @@ struct TypeConst {                   // per neuron type, rounded once on the hos
 struct alignas(128) Ctl {            // device-resident control block
     unsigned long long step;         // current time step n
     unsigned long long spike_begin;  // spikes emitted before step n
-    unsigned long long step_counts[2];  // [n & 1] of step n: high 32 = spikes, low 32 = work items (one atomic)
+    unsigned long long step_counts[4];  // [n & 3] of step n: high 32 = spikes, low 32 = work items (one atomic); cleared when step n + 1 closes
     unsigned long long events;       // synaptic events delivered so far
     unsigned long long spike_cursor; // persistent kernel: next free raster position (= spike_begin between steps)
     unsigned int overflow;           // sticky ring overflow flag
     unsigned int done_blocks;        // delivery kernel: finished-block ticket
-    unsigned int pad0[18];
+    unsigned long long ev_spilled;   // list mode: records that found their list full and went into the ring instead
+    unsigned long long work_step[2]; // [n & 1]: the step whose work list sits in half n & 1 (left by the update kernel for kernel C)
+    unsigned int done_lists;         // kernel C: finished-block ticket
+    unsigned int pad0[7];
     // persistent kernel (see db_step.cu), on a 128-byte line of their own (every block polls it):
     // arrivals of the blocks that closed unit j go to the monotonic counter [j & 3] (blocks are at most
     // two units apart), the spike count of the step produced by unit j to unit_spikes[j & 3]
@@ -74,15 +77,28 @@ struct SimDev {                      // passed by value to every kernel
     const void* w;                   // [Epad] float or __half
     const uint8_t* delay;            // [Epad]
     int32_t w_fp16;
-    // DB_EXEC_KERNELS_DEFERRED: rows sorted by delay; seg[j * (near_max + 1) + (d - 1)] = first synapse of row j
-    // (relative to row_begin) with delay >= d, for d = 1 .. near_max + 1 (the last entry starts the far part)
-    const uint32_t* seg;
-    int32_t near_max;                // 0: delivery is immediate for every synapse
+    // DB_EXEC_KERNELS_DEFERRED: arrival lists (db_step.cu).  8-byte records (receptor << 30 | target, fixed-point weight)
+    // waiting for their arrival step; list ((slot * ev_W + window) * ev_P + part), near family first, cursor of list l
+    // at ev_cnt[8 l] (one per 32-byte sector)
+    int32_t ev_on;                   // 0: every synapse is pushed into the ring when its neuron fires
+    int32_t ev_direct;               // arrivals <= this many steps ahead (1) go straight into the ring
+    int32_t ev_near_lim;             // arrivals <= this many steps ahead go to the near family (ring of ev_Dn slots)
+    int32_t ev_near_d;               // delays <= this are near whatever the position in the time bin: ev_near_lim - (b_t - 1)
+    const uint32_t* seg;             // [N][ev_near_d * ev_W + 1] rows sorted by (delay, window): first synapse (relative to the row) of every
+                                     // (delay, window) run of the near part; the last entry starts the far part
+    int32_t ev_Dn, ev_D;             // slots of the near / far family (powers of two; ev_D = D)
+    int32_t ev_W, ev_P;              // target windows per slot (1, 2 or 4), parallel lists per window (power of two)
+    int32_t ev_n_near, ev_n_far;     // lists per family (ev_n_far = 0: no delay beyond ev_near_lim)
+    uint32_t ev_cap_near, ev_cap_far;// records per list
+    uint32_t ev_wb[3];               // first neuron of the windows 1, 2, 3 (0xFFFFFFFF when unused)
+    uint2* ev_rec;                   // near lists, then far lists
+    unsigned* ev_cnt;
     // spike list = raster ring; per-step work list
     int32_t* spike_ids;              // [spike_cap] circular
     uint32_t* spike_tag;             // [spike_cap] low 32 bits of the step of each entry (steps may interleave by one)
     unsigned long long spike_mask;
-    int2* work;                      // [work_cap] (neuron, chunk) of this step
+    int2* work;                      // [2][work_half] (neuron, chunk) of the steps n & 1 = 0 / 1 (kernel B of step n may run beside the update of n + 1)
+    unsigned long long work_half;
     unsigned long long* step_end;    // [step_log_cap] circular: spikes emitted up to and including step n
     uint32_t step_log_mask;
     // regions

@@ -12,13 +12,14 @@ namespace dbk {
 // ---- db_step.cu ------------------------------------------------------------
 cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
 cudaError_t prepare_kernels();                                            // per handle, on its device: opt-in shared-memory sizes
-cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st);
-cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st);   // deferred variant when p.near_max > 0
-// DB_EXEC_KERNELS_DEFERRED: sort the rows [row0, row1) by delay into scratch arrays indexed by (synapse - s0) and fill
-// their segment tables; add the not yet pushed near segments to a DB_FIELD_RING read-out
+cudaError_t launch_update(const SimDev& p, int n_sm, int mode, cudaStream_t st);   // mode: see k_update_stream
+cudaError_t launch_deliver(const SimDev& p, int grid, unsigned parity, cudaStream_t st);   // parity = step & 1 (list mode: which work-list half)
+// DB_EXEC_KERNELS_DEFERRED: sort the rows [row0, row1) by (delay, target window) into scratch arrays indexed by
+// (synapse - s0); add the records waiting in the arrival lists to a DB_FIELD_RING read-out
 cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
-                             uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st);
-cudaError_t launch_pending_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st);
+                             uint8_t* delay_out, uint32_t* seg, cudaStream_t st);
+cudaError_t launch_delay_hist(const uint8_t* delay, int64_t n, unsigned long long* hist /*[256], zeroed*/, int n_sm, cudaStream_t st);
+cudaError_t launch_lists_to_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st);
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 

@@ -139,7 +139,7 @@ __device__ __forceinline__ void finalize_step(const SimDev& p, const unsigned lo
     c->spike_begin = end;
     c->spike_cursor = end;
     p.step_end[n & p.step_log_mask] = end;
-    c->step_counts[n & 1ull] = 0ull;
+    c->step_counts[(n + 2ull) & 3ull] = 0ull;            // the cell of step n - 2: every kernel of that step is done; next used by step n + 2
     if ((n + 1) % (unsigned long long)p.window_steps == 0) {
         const unsigned w = (unsigned)(((n + 1) / (unsigned long long)p.window_steps + window_clear_ahead(p.window_steps)) % p.max_windows);
         for (int r = 0; r < p.n_regions; ++r) p.region_counts[(size_t)w * p.n_regions + r] = 0u;
@@ -153,13 +153,14 @@ __device__ __forceinline__ void finalize_step(const SimDev& p, const unsigned lo
 template <bool kHalf>
 __global__ void __launch_bounds__(256) k_deliver(const __grid_constant__ SimDev p) {
     const unsigned long long n = p.ctl->step;
-    const unsigned long long counts = p.ctl->step_counts[n & 1ull];
+    const unsigned long long counts = p.ctl->step_counts[n & 3ull];
     const unsigned n_work = (unsigned)counts;
     const unsigned lane = threadIdx.x & 31u;
     const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
     const unsigned long long nt = transfer_step(p, n);       // slot of a synapse = nt + delay
-    for (unsigned q = warp; q < n_work; q += n_warps) deliver_item<kHalf>(p, nt, p.work[q], lane);
+    const int2* const work = p.work + (size_t)(n & 1ull) * p.work_half;
+    for (unsigned q = warp; q < n_work; q += n_warps) deliver_item<kHalf>(p, nt, work[q], lane);
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
@@ -225,6 +226,11 @@ __device__ __forceinline__ unsigned ld_cg_u32(const unsigned* p) {
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
     unsigned long long r;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ uint4 ld_cg_u4(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
 }
 __device__ __forceinline__ float4 ld_cg_f4(const float* p) {
@@ -796,8 +802,6 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
         if (spike_bits & (1u << q)) {
             len[q] = __ldg(p.row_len + i0 + q);
             my_events += (unsigned)len[q];
-            if (p.near_max > 0)        // deferred mode: only the far part of the row is pushed now
-                len[q] -= (int)__ldg(p.seg + (size_t)(i0 + q) * (size_t)(p.near_max + 1) + (size_t)p.near_max);
             my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
         }
     // inclusive warp scan of (spikes, work items) packed in one 64-bit word
@@ -812,7 +816,7 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
     const unsigned ev_warp = __reduce_add_sync(0xffffffffu, my_events);
     unsigned long long base = 0;
     if (lane == 0) {
-        base = atomicAdd(&p.ctl->step_counts[n & 1ull], tot);
+        base = atomicAdd(&p.ctl->step_counts[n & 3ull], tot);
         atomicAdd(&p.ctl->events, (unsigned long long)ev_warp);
     }
     base = __shfl_sync(0xffffffffu, base, 0);
@@ -828,14 +832,21 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
             p.spike_tag[spk_pos & p.spike_mask] = (uint32_t)n;
             ++spk_pos;
             const int nch = (len[q] + kChunk - 1) / kChunk;
-            for (int c = 0; c < nch; ++c) p.work[work_pos++] = make_int2(i, c);
+            for (int c = 0; c < nch; ++c) p.work[(size_t)(n & 1ull) * p.work_half + work_pos++] = make_int2(i, c);
             const int r = (p.n_regions > 1) ? region_of(p, i) : 0;
             atomicAdd(p.region_counts + (size_t)win * p.n_regions + r, 1u);
         }
 }
 
-template <bool kOU>
+// kMode 0: whole step n in one pass, classic order (DB_EXEC_KERNELS; the delivery kernel closes the step).
+// List mode runs the UNITS of the persistent kernel instead (see its header: A_n = membrane step and spikes of step n,
+// B_n = consume ring slot n), so that slot n is read one kernel later than in the classic order and the delivery of the
+// spikes of step n -- all of it, delay 1 included -- has the whole next update kernel to run beside:
+//   kMode 1: A_n only (first kernel of a db_step call);  kMode 2: B_(n-1) then A_n;  kMode 3: B_(n-1) only (last kernel of a
+//   call: the state is complete again).  n = Ctl::step; the kernels with an A part close step n themselves.
+template <bool kOU, int kMode>
 __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_constant__ SimDev p, const RunCfg cfg) {
+    constexpr bool kClassic = (kMode == 0), kB = (kMode != 1), kA = (kMode != 3);
     extern __shared__ uint4 s_stage[];                 // kStageBytes: plane k of thread t at k * kPlaneStride + 16 t
     __shared__ TypeSmem s_tc[kMaxTypes];
     __shared__ uint32_t s_T[kMaxTypes][kPoissonMax];
@@ -859,30 +870,33 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
     Stage sg;
     sg.sbase = (uint32_t)__cvta_generic_to_shared(s_stage) + threadIdx.x * 16u;
     sg.srt = (uint32_t)__cvta_generic_to_shared(s_stage) + 9u * kPlaneStride + threadIdx.x * 8u;
-    const unsigned long long n = p.ctl->step;
+    const unsigned long long n = p.ctl->step;              // step of the A part
+    const unsigned long long nB = kClassic ? n : n - 1ull;  // step whose ring slot is consumed
     const unsigned long long sb = p.ctl->spike_begin;
+    if (kA && blockIdx.x == 0 && threadIdx.x == 0) p.ctl->work_step[n & 1ull] = n;     // for the delivery kernel of this step (list mode)
     const int first = (int)blockIdx.x * cfg.tasks_per_block;
     const int last = min(first + cfg.tasks_per_block, cfg.n_tasks);
     const int task0 = first + warp;
-    if (task0 >= last) return;
     const size_t Np = (size_t)p.Npad;
-    int32_t* const slot0 = p.ring + (size_t)(n & (unsigned long long)(p.D - 1)) * 4 * Np;
+    int32_t* const slot0 = p.ring + (size_t)(nB & (unsigned long long)(p.D - 1)) * 4 * Np;
     const int i00 = (task0 * 32 + (int)lane) * 4;
     const int task_stride = n_warps * 128;
     unsigned bg_acc = 0u;
-    request_state(p, sg, i00);
-    request_ring(p, sg, slot0 + i00);
-    cp_async_commit();
+    if (task0 < last) {
+        request_state(p, sg, i00);
+        if (kB) request_ring(p, sg, slot0 + i00);
+        cp_async_commit();
+    }
     for (int task = task0; task < last; task += n_warps) {
         const int next_off = (task + n_warps < last) ? task_stride : 0;
         const int grp = task * 32 + (int)lane;
         const int i0 = grp * 4;
         // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
         uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
-        if (!kOU || p.bg_on) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+        if (kB && (!kOU || p.bg_on)) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
         float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         float4 rnd_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        if (kOU) {
+        if (kOU && kA) {
             iou = ld_cg_f4(p.Iou + i0);
             const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
             rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
@@ -899,16 +913,28 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
         unsigned spike_bits;
         if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-            spike_bits = neuron_group<true, true, true, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
         else                            // a type boundary inside the group (rare)
-            spike_bits = neuron_group<true, true, true, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
-        if (kOU) st_cg_f4(p.Iou + i0, iou);
+            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        if (kOU && kA) st_cg_f4(p.Iou + i0, iou);
         cp_async_commit();
-        if (__ballot_sync(0xffffffffu, spike_bits != 0)) emit_global(p, n, sb, i0, lane, spike_bits);
+        if (kA && __ballot_sync(0xffffffffu, spike_bits != 0)) emit_global(p, n, sb, i0, lane, spike_bits);
     }
     const unsigned bg_warp = __reduce_add_sync(0xffffffffu, bg_acc);
     if (lane == 0 && bg_warp)
         atomicAdd(p.bg_parts + ((blockIdx.x * (unsigned)n_warps + (unsigned)warp) & (kBgParts - 1)), (unsigned long long)bg_warp);
+    if (!kClassic && kA) {               // list mode: step n is closed here (its delivery runs beside the next update kernel)
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            const unsigned ticket = atomicAdd(&p.ctl->done_blocks, 1u);
+            if (ticket == gridDim.x - 1) {    // every block has read n and has added its spikes
+                p.ctl->done_blocks = 0u;
+                __threadfence();
+                finalize_step(p, n, *reinterpret_cast<volatile unsigned long long*>(&p.ctl->step_counts[n & 3ull]));
+            }
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------
@@ -929,44 +955,50 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
 }
 
 // ===========================================================================
-// Mode DB_EXEC_KERNELS_DEFERRED.  Pushing a spike's whole row when it fires
-// scatters 4-byte reductions over every ring slot the row's delays reach: on
-// networks whose ring is far larger than L2 every event misses (measured:
-// ~99 B of DRAM sectors per 17-byte event, profiles/).  Here the rows are
-// sorted by delay and the push of the synapses with delay d <= near_max is
-// DEFERRED: after the update of step n, the kernel walks the spike lists of
-// the steps n + 1 - d (d = 1 .. near_max; the raster keeps them) and pushes
-// from each of those rows the segment with delay d -- all of it arrives in
-// step n + 1, so every reduction hits the ONE ring slot n + 1 (16 B x N, L2
-// sized), and DRAM only streams the CSR segments.  Synapses with longer
-// delays (the far part of a row) are pushed when the neuron fires, as in the
-// other modes.  The sums are the same integers, whatever the order.
+// Mode DB_EXEC_KERNELS_DEFERRED: arrival lists.  Pushing a spike's whole row when it fires scatters 4-byte
+// reductions over every ring slot the row's delays reach: with a ring far larger than L2 every event is a random
+// 32-byte-sector read-modify-write in DRAM (~20 G/s on this device, profiles/), and pulling the (row, delay) segments
+// out of the CSR when they arrive (round 1) turns the same events into random DRAM sector READS instead.  Here a row
+// is read ONCE, when its neuron fires (contiguous: DRAM streams it), and every synapse becomes an 8-byte record
+// (receptor | target, fixed-point weight) appended to the LIST OF ITS ARRIVAL STEP; the rows are sorted by (delay,
+// target window) at db_create, so the records of a row fall into a few contiguous runs and one atomic on a list
+// cursor reserves a whole run.  In the kernel of step n the list of step n + 1 is streamed back and reduced into
+// ring slot n + 1 -- the only slot that takes reductions (16 B x N: L2-sized, window by window when it is not), so
+// the reductions run at the L2 rate and DRAM only streams: row 7-9 B + record written 8 B + record read 8 B per
+// event.  Records whose arrival step is the next one (delay 1) are reduced into the slot directly; a list that is
+// full spills into the dense ring as in the other modes.  The sums are the same integers, whatever the order.
+//   near lists: ring of ev_Dn slots for arrivals <= ev_near_lim steps ahead (most events: large capacity per slot);
+//   far lists:  ring of D slots for the others (inter-region delays: few events per slot for many slots).
 // ===========================================================================
+__device__ __forceinline__ unsigned ev_window(const SimDev& p, const unsigned tg) {
+    return (unsigned)(tg >= p.ev_wb[0]) + (unsigned)(tg >= p.ev_wb[1]) + (unsigned)(tg >= p.ev_wb[2]);
+}
 
-// Sort the rows [row0, row1) by delay into scratch arrays (indexed by synapse - s0) and fill their
-// segment tables; one warp per row, counting sort over the 256 possible delays.
+// Sort the rows [row0, row1) by (delay, target window) into scratch arrays (indexed by synapse - s0); one warp per
+// row, counting sort over 256 W keys.
 constexpr int kSortWarps = 8;
+constexpr int kSortBins = 1024;      // 256 delays x up to 4 target windows
 template <bool kHalf>
-__global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const int64_t* __restrict__ row_begin,
-        const int32_t* __restrict__ row_len, const uint32_t* __restrict__ tgt_rec, const void* __restrict__ w,
-        const uint8_t* __restrict__ delay, const int64_t row0, const int64_t row1, const int64_t s0,
-        uint32_t* __restrict__ tgt_out, void* __restrict__ w_out, uint8_t* __restrict__ delay_out,
-        uint32_t* __restrict__ seg, const int near_max) {
-    __shared__ unsigned s_cnt[kSortWarps][256];
+__global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const __grid_constant__ SimDev p, const int64_t row0,
+        const int64_t row1, const int64_t s0, uint32_t* __restrict__ tgt_out, void* __restrict__ w_out,
+        uint8_t* __restrict__ delay_out, uint32_t* __restrict__ seg) {
+    __shared__ unsigned s_cnt[kSortWarps][kSortBins];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     unsigned* cnt = s_cnt[warp];
+    const unsigned W = (unsigned)p.ev_W;
+    const int nb = 256 * (int)W, per = nb / 32;
     const long long n_warps = (long long)gridDim.x * kSortWarps;
     for (long long j = row0 + (long long)blockIdx.x * kSortWarps + warp; j < row1; j += n_warps) {
-        const int64_t rb = row_begin[j];
-        const int len = row_len[j];
-        for (int k = (int)lane; k < 256; k += 32) cnt[k] = 0u;
+        const int64_t rb = p.row_begin[j];
+        const int len = p.row_len[j];
+        for (int k = (int)lane; k < nb; k += 32) cnt[k] = 0u;
         __syncwarp();
-        for (int e = (int)lane; e < len; e += 32) atomicAdd(&cnt[delay[rb + e]], 1u);
+        for (int e = (int)lane; e < len; e += 32)
+            atomicAdd(&cnt[(unsigned)p.delay[rb + e] * W + ev_window(p, p.tgt_rec[rb + e] & 0x3FFFFFFFu)], 1u);
         __syncwarp();
-        // exclusive scan of the 256 counters: lane l owns the bins 8 l .. 8 l + 7
-        unsigned loc[8], sum = 0u;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) { loc[k] = sum; sum += cnt[lane * 8 + k]; }
+        // exclusive scan of the counters: lane l owns the bins per * l .. per * l + per - 1
+        unsigned sum = 0u;
+        for (int k = 0; k < per; ++k) { const unsigned c = cnt[(int)lane * per + k]; cnt[(int)lane * per + k] = sum; sum += c; }
         unsigned inc = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -974,21 +1006,21 @@ __global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const int64_t* __
             if (lane >= (unsigned)d) inc += o;
         }
         const unsigned base = inc - sum;
+        for (int k = 0; k < per; ++k) cnt[(int)lane * per + k] += base;       // start of every key inside the row
         __syncwarp();
-#pragma unroll
-        for (int k = 0; k < 8; ++k) cnt[lane * 8 + k] = base + loc[k];      // start of every delay inside the row
-        __syncwarp();
-        // segment table: first synapse with delay >= d, d = 1 .. near_max + 1 (delays are >= 1)
-        for (int d = 1 + (int)lane; d <= near_max + 1; d += 32)
-            seg[(size_t)j * (size_t)(near_max + 1) + (size_t)(d - 1)] = (d < 256) ? cnt[d] : (unsigned)len;
+        // segment table of the near part: seg[q] = first synapse with key >= q, q = (d - 1) W + w for d = 1 .. ev_near_d,
+        // and seg[K] = start of the far part (delays are >= 1: the bins 0 .. W - 1 are empty)
+        const int K = p.ev_near_d * (int)W;
+        for (int q = (int)lane; q <= K; q += 32) seg[(size_t)j * (size_t)(K + 1) + (size_t)q] = (q + (int)W < nb) ? cnt[q + (int)W] : (unsigned)len;
         __syncwarp();
         for (int e = (int)lane; e < len; e += 32) {
-            const unsigned d = delay[rb + e];
-            const int64_t o = rb - s0 + (int64_t)atomicAdd(&cnt[d], 1u);
-            tgt_out[o] = tgt_rec[rb + e];
+            const unsigned d = p.delay[rb + e];
+            const uint32_t t = p.tgt_rec[rb + e];
+            const int64_t o = rb - s0 + (int64_t)atomicAdd(&cnt[d * W + ev_window(p, t & 0x3FFFFFFFu)], 1u);
+            tgt_out[o] = t;
             delay_out[o] = (uint8_t)d;
-            if (kHalf) static_cast<__half*>(w_out)[o] = static_cast<const __half*>(w)[rb + e];
-            else       static_cast<float*>(w_out)[o] = static_cast<const float*>(w)[rb + e];
+            if (kHalf) static_cast<__half*>(w_out)[o] = static_cast<const __half*>(p.w)[rb + e];
+            else       static_cast<float*>(w_out)[o] = static_cast<const float*>(p.w)[rb + e];
         }
         const int padded = (len + kRowAlign - 1) / kRowAlign * kRowAlign;      // keep the row padding inert
         for (int e = len + (int)lane; e < padded; e += 32) {
@@ -1002,174 +1034,327 @@ __global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const int64_t* __
     }
 }
 
-// Push `len` synapses starting at `rb` (any alignment), one synapse per lane and pass.
-// kFixed: all of them land in slot `slot_fixed` (a delay segment); else the slot follows the stored delay.
-template <bool kHalf, bool kFixed>
-__device__ __forceinline__ void deliver_scalar(const SimDev& p, const unsigned nlo, const unsigned slot_fixed,
-                                               const int64_t rb, const int len, const unsigned lane) {
+// Index of the list that takes a record arriving `ahead` steps after step n (ahead > ev_direct) at target tg, and its
+// capacity.  Lists are numbered near family first: ((slot * W + window) * P + part).
+__device__ __forceinline__ unsigned ev_list_of(const SimDev& p, const unsigned arrival, const unsigned ahead, const unsigned tg,
+                                               const unsigned part) {
+    const unsigned w = ev_window(p, tg);
+    if (ahead <= (unsigned)p.ev_near_lim)
+        return (((arrival & (unsigned)(p.ev_Dn - 1)) * (unsigned)p.ev_W + w) * (unsigned)p.ev_P) + part;
+    return (unsigned)p.ev_n_near + (((arrival & (unsigned)(p.ev_D - 1)) * (unsigned)p.ev_W + w) * (unsigned)p.ev_P) + part;
+}
+__device__ __forceinline__ uint2* ev_records(const SimDev& p, const unsigned list) {
+    return list < (unsigned)p.ev_n_near ? p.ev_rec + (size_t)list * p.ev_cap_near
+                                        : p.ev_rec + (size_t)p.ev_n_near * p.ev_cap_near + (size_t)(list - (unsigned)p.ev_n_near) * p.ev_cap_far;
+}
+__device__ __forceinline__ unsigned ev_capacity(const SimDev& p, const unsigned list) {
+    return list < (unsigned)p.ev_n_near ? p.ev_cap_near : p.ev_cap_far;
+}
+constexpr int kEvCntStride = 8;      // one list cursor per 32-byte sector
+
+// Turn `len` synapses starting at `rb` into records: the lanes take 32 consecutive synapses per pass, four passes of
+// loads in flight; the lanes of a pass whose records go to the same list (a run of the sorted row) reserve their
+// positions with ONE atomic on the list's cursor.  n = step of the spike, nto = its transfer step (R29).
+template <bool kHalf>
+__device__ __forceinline__ void bin_span(const SimDev& p, const unsigned n_lo, const unsigned nto_lo, const int64_t rb,
+                                         const int len, const unsigned lane, const unsigned part, unsigned& spilled) {
     const size_t Np = (size_t)p.Npad;
     const unsigned Dm = (unsigned)(p.D - 1);
-    for (int e = (int)lane; e < len; e += 32) {
-        const unsigned t = __ldg(p.tgt_rec + rb + e);
-        float wf;
-        if (kHalf) wf = __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e));
-        else       wf = __ldg(static_cast<const float*>(p.w) + rb + e);
-        const unsigned sl = kFixed ? slot_fixed : ((nlo + (unsigned)__ldg(p.delay + rb + e)) & Dm);
-        const int wq = __float2int_rn(__fmul_rn(wf, p.wscale));
-        red_add_s32(p.ring + ((size_t)sl * 4 + (t >> 30)) * Np + (t & 0x3FFFFFFFu), wq);
+    const unsigned shift = nto_lo - n_lo;                // steps until the end of the spike's time bin
+    constexpr int kRounds = 4;                           // passes of 32 synapses in flight: loads first, then the cursor
+    for (int base = 0; base < len; base += 32 * kRounds) {   // atomics of all passes, then the stores
+        unsigned tr[kRounds], dl[kRounds], list[kRounds], pos[kRounds], peers[kRounds];
+        float wf[kRounds];
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const int e = base + r * 32 + (int)lane;
+            tr[r] = 0u; dl[r] = 0u; wf[r] = 0.0f;
+            if (e < len) {
+                tr[r] = __ldg(p.tgt_rec + rb + e);
+                dl[r] = __ldg(p.delay + rb + e);
+                if (kHalf) wf[r] = __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e));
+                else       wf[r] = __ldg(static_cast<const float*>(p.w) + rb + e);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            list[r] = 0xFFFFFFFFu; pos[r] = 0u; peers[r] = 0u;
+            if (base + r * 32 >= len) continue;          // warp-uniform
+            const bool valid = base + r * 32 + (int)lane < len;
+            const unsigned ahead = shift + dl[r];
+            if (valid && ahead > (unsigned)p.ev_direct) list[r] = ev_list_of(p, nto_lo + dl[r], ahead, tr[r] & 0x3FFFFFFFu, part);
+            peers[r] = __match_any_sync(0xffffffffu, list[r]);
+            if (lane == (unsigned)__ffs(peers[r]) - 1u && list[r] != 0xFFFFFFFFu)
+                pos[r] = atomicAdd(p.ev_cnt + (size_t)list[r] * kEvCntStride, (unsigned)__popc(peers[r]));
+        }
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            if (base + r * 32 >= len) continue;          // warp-uniform
+            const unsigned at = __shfl_sync(0xffffffffu, pos[r], __ffs(peers[r]) - 1) + (unsigned)__popc(peers[r] & ((1u << lane) - 1u));
+            if (base + r * 32 + (int)lane >= len) continue;
+            const int wq = __float2int_rn(__fmul_rn(wf[r], p.wscale));
+            if (list[r] != 0xFFFFFFFFu && at < ev_capacity(p, list[r])) {
+                ev_records(p, list[r])[at] = make_uint2(tr[r], (unsigned)wq);
+            } else {                                     // next step's arrivals, or a full list: straight into the ring
+                red_add_s32(p.ring + ((size_t)((nto_lo + dl[r]) & Dm) * 4 + (tr[r] >> 30)) * Np + (tr[r] & 0x3FFFFFFFu), wq);
+                if (list[r] != 0xFFFFFFFFu) ++spilled;
+            }
+        }
     }
 }
 
-// Spike list of step m in the two-kernel modes: raster positions [begin, end).  `n` = current step
-// (its own entry is not in the step log yet: the count comes from the step counter).
-__device__ __forceinline__ void spike_range(const SimDev& p, const unsigned long long n, const unsigned long long counts,
-                                            const long long m, unsigned long long& begin, unsigned long long& end) {
-    begin = end = 0ull;
-    if (m < 0) return;
-    if ((unsigned long long)m == n) { begin = p.ctl->spike_begin; end = begin + (counts >> 32); return; }
-    begin = (m == 0) ? 0ull : p.step_end[(unsigned long long)(m - 1) & p.step_log_mask];
-    end = p.step_end[(unsigned long long)m & p.step_log_mask];
+// The near part of one work item: the synapses [c0, c1) (relative to the row start rb0) of row j with delay <= ev_near_d.
+// The row is sorted by (delay, window) and seg[] holds where every (delay, window) run starts, so the lanes reserve the
+// list positions of ALL runs of the item at once (one atomic per run, issued together: one round trip), leave
+// "list position - synapse index" per run in a table of the warp, and then copy the synapses as one flat range:
+// no atomic and no vote inside the copy loop, whose loads are all independent.
+constexpr int kEvKeysMax = 128;      // (delay, window) runs of the near part: ev_near_d <= 29 delays x W <= 4 windows
+template <bool kHalf>
+__device__ __forceinline__ void bin_near(const SimDev& p, const unsigned n_lo, const unsigned nto_lo, const int j, const int64_t rb0,
+                                         const int c0, const int c1, const unsigned lane, const unsigned part,
+                                         int* tab_off, unsigned* tab_list, unsigned& spilled) {
+    const unsigned W = (unsigned)p.ev_W;
+    const int K = p.ev_near_d * (int)W;
+    const uint32_t* sg = p.seg + (size_t)j * (size_t)(K + 1);
+    const unsigned shift = nto_lo - n_lo;
+    for (int q = (int)lane; q < K; q += 32) {
+        const int s0 = max((int)__ldg(sg + q), c0), s1 = min((int)__ldg(sg + q + 1), c1);
+        unsigned list = 0xFFFFFFFFu;
+        int off = 0;
+        if (s1 > s0) {
+            const unsigned d = (unsigned)q / W + 1u, w = (unsigned)q % W;
+            if (shift + d > (unsigned)p.ev_direct) {
+                list = (((nto_lo + d) & (unsigned)(p.ev_Dn - 1)) * W + w) * (unsigned)p.ev_P + part;
+                off = (int)atomicAdd(p.ev_cnt + (size_t)list * kEvCntStride, (unsigned)(s1 - s0)) - s0;
+            }
+        }
+        tab_off[q] = off;
+        tab_list[q] = list;
+    }
+    __syncwarp();
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    constexpr int kRounds = 4;
+    for (int base = c0; base < c1; base += 32 * kRounds) {
+        unsigned tr[kRounds], dl[kRounds];
+        float wf[kRounds];
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const int e = base + r * 32 + (int)lane;
+            tr[r] = 0u; dl[r] = 1u; wf[r] = 0.0f;
+            if (e < c1) {
+                tr[r] = __ldg(p.tgt_rec + rb0 + e);
+                dl[r] = __ldg(p.delay + rb0 + e);
+                if (kHalf) wf[r] = __half2float(__ldg(static_cast<const __half*>(p.w) + rb0 + e));
+                else       wf[r] = __ldg(static_cast<const float*>(p.w) + rb0 + e);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const int e = base + r * 32 + (int)lane;
+            if (e >= c1) continue;
+            const unsigned tg = tr[r] & 0x3FFFFFFFu;
+            const unsigned q = (dl[r] - 1u) * W + ev_window(p, tg);
+            const unsigned list = tab_list[q];
+            const unsigned pos = (unsigned)(tab_off[q] + e);
+            const int wq = __float2int_rn(__fmul_rn(wf[r], p.wscale));
+            if (list != 0xFFFFFFFFu && pos < p.ev_cap_near) {
+                p.ev_rec[(size_t)list * p.ev_cap_near + pos] = make_uint2(tr[r], (unsigned)wq);
+            } else {                                     // a full list, or next step's arrivals: straight into the ring
+                red_add_s32(p.ring + ((size_t)((nto_lo + dl[r]) & Dm) * 4 + (tr[r] >> 30)) * Np + tg, wq);
+                if (list != 0xFFFFFFFFu) ++spilled;
+            }
+        }
+    }
+    __syncwarp();
 }
 
-template <bool kHalf>
-__global__ void __launch_bounds__(256) k_deliver_deferred(const __grid_constant__ SimDev p) {
-    __shared__ unsigned long long s_begin[32];
-    __shared__ unsigned s_cum[33];                  // s_cum[d] = near items of the delays < d + 1 (exclusive prefix)
-    __shared__ unsigned s_pref[8][32];              // per warp: first flat synapse index of each of its 32 items
-    __shared__ long long s_rb[8][32];               // per warp: first synapse of each item
-    const unsigned long long n = p.ctl->step;
-    const unsigned long long counts = p.ctl->step_counts[n & 1ull];
-    const unsigned n_work = (unsigned)counts;       // far-part chunks of this step's spikes
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
-    const int S = p.near_max + 1;
-    if (threadIdx.x < 32) {
-        unsigned long long b = 0ull, e = 0ull;
-        if ((int)lane < p.near_max) spike_range(p, n, counts, (long long)n - (long long)lane, b, e);   // d = lane + 1
-        const unsigned c = (unsigned)(e - b);
-        unsigned inc = c;
+// How many synapses carry each delay (db_create: sizes the arrival lists); padding entries count as delay 1.
+__global__ void __launch_bounds__(256) k_delay_hist(const uint8_t* __restrict__ delay, const int64_t n, unsigned long long* __restrict__ hist) {
+    __shared__ unsigned s_h[256];
+    s_h[threadIdx.x] = 0u;
+    __syncthreads();
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x * 16;
+    for (int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 16; e < n; e += stride) {
+        if (e + 16 <= n) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(delay + e));
+            const unsigned w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
-            if (lane >= (unsigned)d) inc += o;
+            for (int k = 0; k < 16; ++k) atomicAdd(&s_h[(w[k >> 2] >> ((k & 3) * 8)) & 0xFFu], 1u);
+        } else {
+            for (int64_t f = e; f < n; ++f) atomicAdd(&s_h[delay[f]], 1u);
         }
-        s_begin[lane] = b;
-        s_cum[lane + 1] = inc;
-        if (lane == 0) s_cum[0] = 0u;
     }
     __syncthreads();
-    // ---- far part of the rows that fired in this step (delay > near_max): pushed now, slot by stored delay
-    for (unsigned q = warp; q < n_work; q += n_warps) {
-        const int2 wk = p.work[q];
-        const int j = wk.x;
-        const int near_end = (int)__ldg(p.seg + (size_t)j * S + p.near_max);
-        const int off = near_end + wk.y * kChunk;
-        const int len = min(kChunk, __ldg(p.row_len + j) - off);
-        deliver_scalar<kHalf, false>(p, (unsigned)n, 0u, __ldg(p.row_begin + j) + off, len, lane);
-    }
-    // ---- near part: segment d of every row that fired in step n + 1 - d arrives in step n + 1.
-    // An item = (delay d, one spike of step n + 1 - d).  A warp takes 32 items at a time: every lane
-    // fetches the descriptor of one item (spike id -> segment bounds -> row start: all 32 chains in
-    // flight together), then the lanes walk the synapses of the 32 segments as ONE flat range, so that
-    // the loads of a pass are independent whatever the segment lengths are.
-    const unsigned total = s_cum[32];
-    const unsigned slot = (unsigned)(n + 1ull) & (unsigned)(p.D - 1);
-    const size_t Np = (size_t)p.Npad;
-    int32_t* const ring_slot = p.ring + (size_t)slot * 4 * Np;
-    unsigned* const w_pref = s_pref[threadIdx.x >> 5];
-    long long* const w_rb = s_rb[threadIdx.x >> 5];
-    for (unsigned base = warp * 32u; base < total; base += n_warps * 32u) {
-        const unsigned q = base + lane;
-        int len = 0;
-        long long rb = 0;
-        if (q < total) {
-            unsigned lo = 0u, hi = (unsigned)p.near_max;                     // largest dm1 with s_cum[dm1] <= q
-            while (hi - lo > 1u) { const unsigned mid = (lo + hi) >> 1; if (s_cum[mid] <= q) lo = mid; else hi = mid; }
-            const unsigned long long pos = s_begin[lo] + (unsigned long long)(q - s_cum[lo]);
-            const int j = p.spike_ids[pos & p.spike_mask];
-            const uint32_t* sg = p.seg + (size_t)j * S + lo;
-            const int o0 = (int)__ldg(sg), o1 = (int)__ldg(sg + 1);
-            len = o1 - o0;
-            rb = (long long)__ldg(p.row_begin + j) + o0;
-        }
-        unsigned inc = (unsigned)len;
+    if (s_h[threadIdx.x]) atomicAdd(hist + threadIdx.x, (unsigned long long)s_h[threadIdx.x]);
+}
+
+constexpr int kEvChunk = 2048;       // records per apply work unit (one block pass: 256 threads x 8)
+constexpr int kEvMaxLists = 2048;    // lists of one arrival step: 2 families x W <= 4 x P <= 256
+constexpr int kEvMapMax = 6144;      // chunks of one arrival step whose list is looked up in a table (else: binary search)
+
+// The delivery kernel of step n in list mode.  It touches nothing the NEXT update kernel (B_n, A_(n+1): reads ring slot
+// n) reads -- ring slot n + 1 and later, the lists, the work list of step n -- so it runs BESIDE that kernel on a second
+// branch of the step graph (db_api.cu) and has to be done before the update kernel after it (B_(n+1)) starts:
+//   1. the records that arrive in step n + 1 (written by the delivery kernels of the earlier steps) are streamed into
+//      ring slot n + 1, window by window: the only slot that takes reductions here;
+//   2. the rows that fired in step n: their synapses that arrive in step n + 1 are reduced into that slot straight from
+//      the CSR, the later ones become records in the lists of their arrival steps.
+// It takes n from the cell the update kernel left for it (Ctl::step moves on meanwhile).
+template <bool kHalf>
+__global__ void __maxnreg__(56) k_deliver_lists(const __grid_constant__ SimDev p, const unsigned parity) {
+    __shared__ unsigned s_count[kEvMaxLists], s_first[kEvMaxLists + 1];
+    __shared__ unsigned short s_map[kEvMapMax];
+    __shared__ unsigned s_warp[8];
+    __shared__ int s_tab_off[8][kEvKeysMax];
+    __shared__ unsigned s_tab_list[8][kEvKeysMax];
+    __shared__ unsigned s_last;
+    const unsigned long long n = p.ctl->work_step[parity];
+    const unsigned long long counts = p.ctl->step_counts[n & 3ull];
+    const unsigned n_work = (unsigned)counts;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned m = (unsigned)n + (unsigned)p.ev_direct;
+    const unsigned fams = p.ev_n_far ? 2u : 1u, P = (unsigned)p.ev_P;
+    const unsigned n_lists = (unsigned)p.ev_W * fams * P;
+    auto list_of = [&](const unsigned k) {
+        const unsigned part = k % P, fam = (k / P) % fams, w = k / (P * fams);
+        const unsigned slot = fam ? (m & (unsigned)(p.ev_D - 1)) : (m & (unsigned)(p.ev_Dn - 1));
+        return (fam ? (unsigned)p.ev_n_near : 0u) + ((slot * (unsigned)p.ev_W + w) * P) + part;
+    };
+    unsigned spilled = 0u;
+    {
+        // ---- 1. the lists of step m, window-major (so that the blocks sweep the slot window by window): entry k of the
+        // table = (window, family, part); s_first[k] = first 2048-record chunk of list k (block-wide exclusive scan)
+        {
+            const unsigned per = (n_lists + 255u) / 256u, k0 = threadIdx.x * per;
+            unsigned sum = 0u;
+            for (unsigned k = k0; k < min(k0 + per, n_lists); ++k) {
+                const unsigned list = list_of(k);
+                const unsigned c = min(ld_cg_u32(p.ev_cnt + (size_t)list * kEvCntStride), ev_capacity(p, list));
+                s_count[k] = c;
+                s_first[k] = sum;                            // exclusive inside the thread's run
+                sum += (c + kEvChunk - 1u) / kEvChunk;
+            }
+            unsigned inc = sum;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
-            if (lane >= (unsigned)d) inc += o;
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= (unsigned)d) inc += o;
+            }
+            if (lane == 31u) s_warp[threadIdx.x >> 5] = inc;
+            __syncthreads();
+            unsigned before = inc - sum;
+            for (unsigned w2 = 0; w2 < (threadIdx.x >> 5); ++w2) before += s_warp[w2];
+            for (unsigned k = k0; k < min(k0 + per, n_lists); ++k) {
+                const unsigned f = s_first[k] + before, nc = (s_count[k] + kEvChunk - 1u) / kEvChunk;
+                s_first[k] = f;
+                for (unsigned c = f; c < min(f + nc, (unsigned)kEvMapMax); ++c) s_map[c] = (unsigned short)k;
+            }
+            if (threadIdx.x == 255u) s_first[n_lists] = before + sum;
+            __syncthreads();
         }
-        const unsigned flat = __shfl_sync(0xffffffffu, inc, 31);
-        w_pref[lane] = inc - (unsigned)len;
-        w_rb[lane] = rb;
-        __syncwarp();
-        for (unsigned s0 = 0u; s0 < flat; s0 += 128u) {                      // four independent passes in flight
-            unsigned t[4];
-            float wf[4];
+        const unsigned n_chunks = s_first[n_lists];
+        const size_t Np = (size_t)p.Npad;
+        int32_t* const ring_slot = p.ring + (size_t)(m & (unsigned)(p.D - 1)) * 4 * Np;
+        auto chunk_range = [&](const unsigned c, const uint2*& rec, unsigned& r0, unsigned& r1) {
+            unsigned k;
+            if (c < (unsigned)kEvMapMax) k = s_map[c];
+            else {                                           // largest k with s_first[k] <= c
+                unsigned hi = n_lists;
+                k = 0u;
+                while (hi - k > 1u) { const unsigned mid = (k + hi) >> 1; if (s_first[mid] <= c) k = mid; else hi = mid; }
+            }
+            r0 = (c - s_first[k]) * kEvChunk; r1 = min(r0 + (unsigned)kEvChunk, s_count[k]);
+            rec = ev_records(p, list_of(k));
+        };
+        auto load_chunk = [&](const uint2* rec, const unsigned r0, const unsigned r1, uint4 (&v)[4]) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {                    // two records per 128-bit load, four loads in flight
+                const unsigned r = r0 + ((unsigned)u * 256u + threadIdx.x) * 2u;
+                v[u] = make_uint4(0u, 0u, 0u, 0u);
+                if (r + 1u < r1) v[u] = ld_cg_u4(reinterpret_cast<const uint4*>(rec + r));
+                else if (r < r1) { const uint2 a = rec[r]; v[u] = make_uint4(a.x, a.y, 0u, 0u); }
+            }
+        };
+        // the records of the next chunk are requested before the reductions of this one are issued
+        const uint2* rec = nullptr;
+        unsigned r0 = 0u, r1 = 0u;
+        uint4 v[4], vn[4];
+        unsigned c = blockIdx.x;
+        if (c < n_chunks) { chunk_range(c, rec, r0, r1); load_chunk(rec, r0, r1, v); }
+        while (c < n_chunks) {
+            const unsigned cn = c + gridDim.x;
+            const uint2* recn = nullptr;
+            unsigned r0n = 0u, r1n = 0u;
+            if (cn < n_chunks) { chunk_range(cn, recn, r0n, r1n); load_chunk(recn, r0n, r1n, vn); }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const unsigned sx = s0 + (unsigned)u * 32u + lane;
-                t[u] = 0u; wf[u] = 0.0f;
-                if (sx < flat) {
-                    unsigned k = 0u;                                         // largest k with w_pref[k] <= sx
-#pragma unroll
-                    for (unsigned step = 16u; step; step >>= 1) if (w_pref[k + step] <= sx) k += step;
-                    const long long e = w_rb[k] + (long long)(sx - w_pref[k]);
-                    t[u] = __ldg(p.tgt_rec + e);
-                    if (kHalf) wf[u] = __half2float(__ldg(static_cast<const __half*>(p.w) + e));
-                    else       wf[u] = __ldg(static_cast<const float*>(p.w) + e);
-                }
+                const unsigned r = r0 + ((unsigned)u * 256u + threadIdx.x) * 2u;
+                if (r < r1) red_add_s32(ring_slot + (size_t)(v[u].x >> 30) * Np + (v[u].x & 0x3FFFFFFFu), (int)v[u].y);
+                if (r + 1u < r1) red_add_s32(ring_slot + (size_t)(v[u].z >> 30) * Np + (v[u].z & 0x3FFFFFFFu), (int)v[u].w);
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (s0 + (unsigned)u * 32u + lane < flat)
-                    red_add_s32(ring_slot + (size_t)(t[u] >> 30) * Np + (t[u] & 0x3FFFFFFFu), __float2int_rn(__fmul_rn(wf[u], p.wscale)));
+            for (int u = 0; u < 4; ++u) v[u] = vn[u];
+            r0 = r0n; r1 = r1n; c = cn;
         }
-        __syncwarp();
     }
+    {
+        // ---- 2. the rows that fired in step n
+        const unsigned bwarp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+        const unsigned n_bwarps = (gridDim.x * blockDim.x) >> 5;
+        const unsigned nto = (unsigned)transfer_step(p, n);
+        const unsigned part = bwarp & (unsigned)(p.ev_P - 1);   // many cursors per slot: same-address atomics serialise in L2
+        int* const tab_off = s_tab_off[threadIdx.x >> 5];
+        unsigned* const tab_list = s_tab_list[threadIdx.x >> 5];
+        const int K = p.ev_near_d * p.ev_W;
+        const int2* const work = p.work + (size_t)(n & 1ull) * p.work_half;
+        for (unsigned q = bwarp; q < n_work; q += n_bwarps) {
+            const int2 wk = work[q];
+            const int64_t rb0 = __ldg(p.row_begin + wk.x);
+            const int c0 = wk.y * kChunk, c1 = min(c0 + kChunk, __ldg(p.row_len + wk.x));
+            const int near_end = (int)__ldg(p.seg + (size_t)wk.x * (size_t)(K + 1) + (size_t)K);
+            if (c0 < near_end) bin_near<kHalf>(p, (unsigned)n, nto, wk.x, rb0, c0, min(c1, near_end), lane, part, tab_off, tab_list, spilled);
+            if (c1 > near_end) {                             // far part: runs of about one synapse, positions by vote + atomic
+                const int f0 = max(c0, near_end);
+                bin_span<kHalf>(p, (unsigned)n, nto, rb0 + f0, c1 - f0, lane, part, spilled);
+            }
+        }
+    }
+    spilled = __reduce_add_sync(0xffffffffu, spilled);
+    if (lane == 0 && spilled) atomicAdd(&p.ctl->ev_spilled, (unsigned long long)spilled);
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        const unsigned ticket = atomicAdd(&p.ctl->done_blocks, 1u);
-        if (ticket == gridDim.x - 1) {            // every block has read n / counts / the step log: safe to advance
-            p.ctl->done_blocks = 0u;
-            finalize_step(p, n, counts);
-        }
+        s_last = (atomicAdd(&p.ctl->done_lists, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last) {                                 // every block has read the cursors of step m: they start again at zero
+        for (unsigned k = threadIdx.x; k < n_lists; k += blockDim.x) p.ev_cnt[(size_t)list_of(k) * kEvCntStride] = 0u;
+        if (threadIdx.x == 0) p.ctl->done_lists = 0u;
     }
 }
 
-// Read-back of the ring in deferred mode: the arrivals still to come are the ring's content PLUS the
-// near segments not pushed yet -- spikes of step m (n - near_max < m < n), delays n - m < d <= near_max,
-// arriving in step m + d.  Adds them for the targets [first, first + count) into `out`, which has the
-// layout of DB_FIELD_RING: out[(slot * count + i) * 4 + receptor], slot = arrival step mod D_api.
-template <bool kHalf>
-__global__ void __launch_bounds__(256) k_pending_ring(const __grid_constant__ SimDev p, int32_t* __restrict__ out,
-                                                      const int first, const int count, const int D_api) {
+// Read-back of the ring in list mode: the arrivals still to come are the ring's content PLUS the records waiting in
+// the lists.  Adds them for the targets [first, first + count) into `out`, which has the layout of DB_FIELD_RING:
+// out[(slot * count + i) * 4 + receptor], slot = arrival step mod D_api.  One block per list at a time.
+__global__ void __launch_bounds__(256) k_lists_to_ring(const __grid_constant__ SimDev p, int32_t* __restrict__ out,
+                                                       const int first, const int count, const int D_api) {
     const unsigned long long n = p.ctl->step;
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
-    const int S = p.near_max + 1;
-    for (int age = 1; age < p.near_max; ++age) {              // m = n - age: delays age + 1 .. near_max are pending
-        const long long m = (long long)n - age;
-        unsigned long long b, e;
-        spike_range(p, n, 0ull, m, b, e);
-        for (unsigned long long pos = b + warp; pos < e; pos += n_warps) {
-            const int j = p.spike_ids[pos & p.spike_mask];
-            const int64_t rb = __ldg(p.row_begin + j);
-            const int o0 = (int)__ldg(p.seg + (size_t)j * S + age);          // first synapse with delay >= age + 1
-            const int o1 = (int)__ldg(p.seg + (size_t)j * S + p.near_max);   // start of the far part
-            for (int s = o0 + (int)lane; s < o1; s += 32) {
-                const unsigned t = __ldg(p.tgt_rec + rb + s);
-                const int tg = (int)(t & 0x3FFFFFFFu) - first;
-                if (tg < 0 || tg >= count) continue;
-                float wf;
-                if (kHalf) wf = __half2float(__ldg(static_cast<const __half*>(p.w) + rb + s));
-                else       wf = __ldg(static_cast<const float*>(p.w) + rb + s);
-                const unsigned long long arrive = (unsigned long long)m + (unsigned long long)__ldg(p.delay + rb + s);
-                const size_t slot = (size_t)(arrive % (unsigned long long)D_api);
-                atomicAdd(out + (slot * (size_t)count + (size_t)tg) * 4 + (t >> 30), __float2int_rn(__fmul_rn(wf, p.wscale)));
-            }
+    const unsigned total = (unsigned)(p.ev_n_near + p.ev_n_far);
+    const unsigned per_slot = (unsigned)(p.ev_W * p.ev_P);
+    for (unsigned list = blockIdx.x; list < total; list += gridDim.x) {
+        const bool far = list >= (unsigned)p.ev_n_near;
+        const unsigned depth = far ? (unsigned)p.ev_D : (unsigned)p.ev_Dn;
+        const unsigned slot = (far ? list - (unsigned)p.ev_n_near : list) / per_slot;
+        // the one step in [n, n + depth) that maps to this slot
+        const unsigned long long arrive = n + (unsigned long long)((slot - (unsigned)n) & (depth - 1u));
+        const size_t api_slot = (size_t)(arrive % (unsigned long long)D_api);
+        const unsigned c = min(p.ev_cnt[(size_t)list * kEvCntStride], ev_capacity(p, list));
+        const uint2* rec = ev_records(p, list);
+        for (unsigned r = threadIdx.x; r < c; r += blockDim.x) {
+            const uint2 v = rec[r];
+            const int tg = (int)(v.x & 0x3FFFFFFFu) - first;
+            if (tg >= 0 && tg < count) atomicAdd(out + (api_slot * (size_t)count + (size_t)tg) * 4 + (v.x >> 30), (int)v.y);
         }
     }
 }
@@ -1185,25 +1370,39 @@ cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStr
 void run_shape(const SimDev& p, int n_sm, int* grid, int* threads, RunCfg* cfg);
 
 // Function attributes belong to the device context: called once per handle (finish_setup), on the handle's device.
+template <bool kOU>
+static const void* update_fn(int mode) {
+    switch (mode) {
+    case 1: return (const void*)k_update_stream<kOU, 1>;
+    case 2: return (const void*)k_update_stream<kOU, 2>;
+    case 3: return (const void*)k_update_stream<kOU, 3>;
+    default: return (const void*)k_update_stream<kOU, 0>;
+    }
+}
+
 cudaError_t prepare_kernels() {
-    cudaError_t e = cudaFuncSetAttribute(k_update_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_update_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+    cudaError_t e = cudaSuccess;
+    for (int mode = 0; mode < 4 && e == cudaSuccess; ++mode) {
+        e = cudaFuncSetAttribute(update_fn<false>(mode), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(update_fn<true>(mode), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStageBytes);
+    }
     return e;
 }
 
-cudaError_t launch_update(const SimDev& p, int n_sm, cudaStream_t st) {
+// mode: 0 = classic whole step; list mode: 1 = A only, 2 = B then A, 3 = B only (k_update_stream)
+cudaError_t launch_update(const SimDev& p, int n_sm, int mode, cudaStream_t st) {
     int grid = 0, threads = 0;
     RunCfg cfg{};
     run_shape(p, n_sm, &grid, &threads, &cfg);
-    if (p.ou_on) k_update_stream<true><<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);      // no service warp here
-    else         k_update_stream<false><<<grid, threads - 32, (size_t)kStageBytes, st>>>(p, cfg);
-    return cudaGetLastError();
+    void* args[] = {(void*)&p, (void*)&cfg};
+    return cudaLaunchKernel(p.ou_on ? update_fn<true>(mode) : update_fn<false>(mode), dim3(grid), dim3(threads - 32), args,
+                            (size_t)kStageBytes, st);                                               // no service warp here
 }
 
-cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
-    if (p.near_max > 0) {
-        if (p.w_fp16) k_deliver_deferred<true><<<grid, 256, 0, st>>>(p);
-        else          k_deliver_deferred<false><<<grid, 256, 0, st>>>(p);
+cudaError_t launch_deliver(const SimDev& p, int grid, unsigned parity, cudaStream_t st) {
+    if (p.ev_on) {
+        if (p.w_fp16) k_deliver_lists<true><<<grid, 256, 0, st>>>(p, parity);
+        else          k_deliver_lists<false><<<grid, 256, 0, st>>>(p, parity);
     } else {
         if (p.w_fp16) k_deliver<true><<<grid, 256, 0, st>>>(p);
         else          k_deliver<false><<<grid, 256, 0, st>>>(p);
@@ -1212,19 +1411,21 @@ cudaError_t launch_deliver(const SimDev& p, int grid, cudaStream_t st) {
 }
 
 cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
-                             uint8_t* delay_out, uint32_t* seg, int near_max, cudaStream_t st) {
+                             uint8_t* delay_out, uint32_t* seg, cudaStream_t st) {
     const int grid = (int)std::min<int64_t>((row1 - row0 + kSortWarps - 1) / kSortWarps, (int64_t)n_sm * 16);
     if (grid <= 0) return cudaSuccess;
-    if (p.w_fp16) k_sort_rows<true><<<grid, kSortWarps * 32, 0, st>>>(p.row_begin, p.row_len, p.tgt_rec, p.w, p.delay, row0, row1,
-                                                                     s0, tgt_out, w_out, delay_out, seg, near_max);
-    else          k_sort_rows<false><<<grid, kSortWarps * 32, 0, st>>>(p.row_begin, p.row_len, p.tgt_rec, p.w, p.delay, row0, row1,
-                                                                      s0, tgt_out, w_out, delay_out, seg, near_max);
+    if (p.w_fp16) k_sort_rows<true><<<grid, kSortWarps * 32, 0, st>>>(p, row0, row1, s0, tgt_out, w_out, delay_out, seg);
+    else          k_sort_rows<false><<<grid, kSortWarps * 32, 0, st>>>(p, row0, row1, s0, tgt_out, w_out, delay_out, seg);
     return cudaGetLastError();
 }
 
-cudaError_t launch_pending_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st) {
-    if (p.w_fp16) k_pending_ring<true><<<n_sm * 4, 256, 0, st>>>(p, out, first, count, D_api);
-    else          k_pending_ring<false><<<n_sm * 4, 256, 0, st>>>(p, out, first, count, D_api);
+cudaError_t launch_delay_hist(const uint8_t* delay, int64_t n, unsigned long long* hist, int n_sm, cudaStream_t st) {
+    k_delay_hist<<<n_sm * 8, 256, 0, st>>>(delay, n, hist);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lists_to_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st) {
+    k_lists_to_ring<<<n_sm * 4, 256, 0, st>>>(p, out, first, count, D_api);
     return cudaGetLastError();
 }
 

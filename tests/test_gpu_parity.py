@@ -134,7 +134,7 @@ def test_edge_cases(db, oracle_mod, mode, case):
         net = db_inputs.random_csr(N=2500, mean_outdeg=30, seed=7, n_regions=7, fp16=True)
         fp16 = True
         sim["window_steps"] = 7
-    elif case == "far":                       # delays beyond the 31 steps whose push the deferred mode defers
+    elif case == "far":                       # delays beyond the 29 steps the near arrival lists reach: the far family of lists
         sim["D"] = 128
         net = db_inputs.random_csr(N=1500, mean_outdeg=40, seed=9, max_delay=100, fp16=True)
         fp16 = True
@@ -221,7 +221,7 @@ def test_time_binned_spike_transfer(db, oracle_mod, mode, B):
     t = db_inputs.type_params(bg_weight=0.012)
     sim = db_inputs.sim_params(D=32, types=[t, dict(t)], spike_bin_steps=B)       # largest delay + b_t - 1 = 29 < D
     g, o = _pair(db, oracle_mod, sim, net, mode)
-    assert g.db_get_counters()["exec_mode"] == (1 if mode == 3 else mode)         # deferred falls back to two kernels
+    assert g.db_get_counters()["exec_mode"] == mode                               # the arrival lists carry the time bin too
     for upto in (1, B - 1, B, 3 * B, 3 * B + 3, 40 * B, 40 * B + 1, 100 * B):
         g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
         dv, dg = _compare_state(g, o)
