@@ -34,12 +34,15 @@ BG_DRIVE_FOR_CONFIG = {(2, 7): 0.00773, (3, 15): 0.0171, (4, 30): 0.0378}
 # gives 2.6 Hz there); swept on the GPU at N = 200,000: 0.66 -> 2.6, 0.74 -> 5.1, 0.82 -> 7.3, 0.90 -> 9.2 Hz.
 OU_SIGMA, OU_TAU_MS = 0.12, 10.0
 OU_MU_FOR_RATE = {7: 0.81}
+# the same at the paper's production step dt = 1 ms: swept on the GPU at N = 200,000: 0.70 -> 5.1, 0.75 -> 6.7, 0.81 -> 8.4 Hz
+OU_MU_FOR_RATE_DT1 = {7: 0.76}
 
 
 def ou_drive(sim: dict, rate_hz: int = 7) -> dict:
-    """Replace the Poisson drive of every type of `sim` by the OU current calibrated for `rate_hz`."""
+    """Replace the Poisson drive of every type of `sim` by the OU current calibrated for `rate_hz` at the step of `sim`."""
+    mu = (OU_MU_FOR_RATE_DT1 if sim["dt_ms"] >= 1.0 else OU_MU_FOR_RATE)[rate_hz]
     for t in sim["types"]:
-        t.update(bg_weight=0.0, bg_rate_hz=0.0, ou_mu=OU_MU_FOR_RATE[rate_hz], ou_sigma=OU_SIGMA, ou_tau_ms=OU_TAU_MS)
+        t.update(bg_weight=0.0, bg_rate_hz=0.0, ou_mu=mu, ou_sigma=OU_SIGMA, ou_tau_ms=OU_TAU_MS)
     return sim
 
 

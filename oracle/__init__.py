@@ -14,6 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "db_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB_OMP = os.path.join(_HERE, "liboracle_omp.so")      # same source with -fopenmp: the all-cores timing leg of bench.py
 _lib = None
 
 CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-Wall", "-shared", "-fPIC"]
@@ -22,7 +23,18 @@ CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-Wall",
 def build(force: bool = False) -> str:
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", *CXXFLAGS, "-fopenmp", "-o", _LIB_OMP, _SRC])
     return _LIB
+
+
+def use_all_cores(on: bool = True):
+    """Switch this process to the -fopenmp build of the same source (loops over neurons and over spikes shared among
+    the host cores, integer atomics in delivery: same results) or back.  Handles created before the switch stay valid
+    only with the library that made them: switch before creating simulators."""
+    global _lib
+    _lib = None
+    globals()["_ACTIVE"] = _LIB_OMP if on else _LIB
 
 
 class TypeParams(C.Structure):
@@ -59,7 +71,7 @@ def lib():
     global _lib
     if _lib is None:
         build()
-        L = C.CDLL(_LIB)
+        L = C.CDLL(globals().get("_ACTIVE", _LIB))
         L.orc_generate.restype = C.POINTER(Network)
         L.orc_generate.argtypes = [C.POINTER(NetSpec), C.c_uint64]
         L.orc_network_free.argtypes = [C.POINTER(Network)]

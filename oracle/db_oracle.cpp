@@ -579,6 +579,7 @@ struct Sim {
     uint64_t n_events = 0, n_bg = 0;
     int32_t overflow = 0;
     bool log_arrivals = false;            // pins only: what step 1 consumed, [n][i][u]
+    std::vector<uint8_t> spike_flag;      // scratch of one_step: neuron i was flagged in this step
     std::vector<int32_t> arrivals_log;
 
     void one_step() {
@@ -586,19 +587,30 @@ struct Sim {
         const real scale = (real)std::ldexp(1.0, -S);
         int32_t* slot = &ring[(size_t)(n % (uint64_t)D) * (size_t)N * 4];
         std::vector<int32_t> L;                           // SpikeList (Alg. 2 line 2)
+        // The loop body reads and writes neuron i's own state and ring cells only, so its iterations are independent:
+        // built with -fopenmp (the all-cores timing leg of bench.py, liboracle_omp.so) they are shared among the host
+        // cores -- same arithmetic, same results; the plain build runs them in order on one core.
+        spike_flag.assign((size_t)N, 0);
+        if (log_arrivals) arrivals_log.resize(arrivals_log.size() + (size_t)N * 4);
+        int32_t* const alog = log_arrivals ? &arrivals_log[arrivals_log.size() - (size_t)N * 4] : nullptr;
+        uint64_t bg_sum = 0;
+        int32_t ovf = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : bg_sum) reduction(| : ovf)
+#endif
         for (int64_t i = 0; i < N; ++i) {
             const TypeConst<real>& c = tc[ntype[(size_t)i]];
             // 1. arrivals due now; the slot is consumed
             int32_t a[4];
             for (int u = 0; u < 4; ++u) { a[u] = slot[i * 4 + u]; slot[i * 4 + u] = 0; }
-            if (log_arrivals) for (int u = 0; u < 4; ++u) arrivals_log.push_back(a[u]);
+            if (alog) for (int u = 0; u < 4; ++u) alog[i * 4 + u] = a[u];
             for (int u = 0; u < 4; ++u)
-                if (a[u] > (1 << 30) || a[u] < -(1 << 30)) overflow = 1;
+                if (a[u] > (1 << 30) || a[u] < -(1 << 30)) ovf |= 1;
             // 2. Poisson background into AMPA (R14); one Philox block serves 4 neurons
             uint32_t uu = draw(seed, STREAM_BG, (uint64_t)(i >> 2), n).w[i & 3];
             int k = poisson_count(uu, c.T, c.M);
             a[0] = (int32_t)((uint32_t)a[0] + (uint32_t)k * (uint32_t)c.wq_bg);
-            n_bg += (uint64_t)k;
+            bg_sum += (uint64_t)k;
             // 3. fixed point -> real
             real x[4];
             for (int u = 0; u < 4; ++u) x[u] = (real)a[u] * scale;
@@ -630,8 +642,11 @@ struct Sim {
             if (ref[(size_t)i] > 0) { vn = c.Vreset; ref[(size_t)i] -= 1; }
             else if (vn >= c.Vth) { spike = 1; vn = c.Vreset; ref[(size_t)i] = c.R; }
             V[(size_t)i] = vn;
-            if (spike) L.push_back((int32_t)i);
+            spike_flag[(size_t)i] = (uint8_t)spike;
         }
+        n_bg += bg_sum;
+        overflow |= ovf;
+        for (int64_t i = 0; i < N; ++i) if (spike_flag[(size_t)i]) L.push_back((int32_t)i);
         // 8. record + region counts
         const size_t win = (size_t)(n / (uint64_t)window);
         if (region_count.size() < (win + 1) * (size_t)n_regions) region_count.resize((win + 1) * (size_t)n_regions, 0);
@@ -651,12 +666,23 @@ struct Sim {
         }
         if ((n + 1) % (uint64_t)bin == 0) {
             // push delivery along the destination lists (Alg. 2 lines 3-4), w A_j(t) of Eq.(3)
-            for (int32_t j : A) {
+            // (-fopenmp build: the spikes are shared among the cores and the additions are atomic; integer sums do not
+            // depend on their order, so the ring is the same)
+            const int64_t nA = (int64_t)A.size();
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 16)
+#endif
+            for (int64_t k = 0; k < nA; ++k) {
+                const int32_t j = A[(size_t)k];
                 for (int64_t s = row_ptr[(size_t)j]; s < row_ptr[(size_t)j + 1]; ++s) {
                     int32_t wq = (int32_t)std::lrintf(w[(size_t)s] * (float)std::ldexp(1.0, S));
                     size_t sl = (size_t)((n + delay[(size_t)s]) % (uint64_t)D);
                     int32_t* cell = &ring[(sl * (size_t)N + (size_t)tgt[(size_t)s]) * 4 + rec[(size_t)s]];
+#ifdef _OPENMP
+                    __atomic_fetch_add(reinterpret_cast<uint32_t*>(cell), (uint32_t)wq, __ATOMIC_RELAXED);   // wraps the same way
+#else
                     *cell = (int32_t)((uint32_t)*cell + (uint32_t)wq);      // two's-complement wrap
+#endif
                 }
             }
             A.clear();

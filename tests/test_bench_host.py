@@ -71,3 +71,48 @@ def test_single_process_reduction_is_identity():
     import bench
     ms, sums = bench.reduce_over_ranks(None, "cpu", 3.5, [1, 2])
     assert ms == 3.5 and sums == [1.0, 2.0]
+
+
+def test_all_cores_build_of_the_oracle_gives_the_oracles_results(oracle_mod):
+    # bench.py's cpu_baseline times the oracle on one core and on all of them (same source, -fopenmp: parallel for over
+    # neurons and over spikes, integer atomics): the two builds must agree bit for bit, or the second figure is not the oracle's
+    import numpy as np
+    import db_inputs
+    cfg = db_inputs.config(0, scale=0.5)
+    net = oracle_mod.generate(cfg["net"], 3)
+    try:
+        a = oracle_mod.OracleSim(cfg["sim"], net, 2)
+        a.step(400)
+        ra = (a.spikes(), a.ring(), a.state(), a.counters(), a.region_counts())
+        a.close()
+        oracle_mod.use_all_cores(True)
+        b = oracle_mod.OracleSim(cfg["sim"], net, 2)
+        b.step(400)
+        rb = (b.spikes(), b.ring(), b.state(), b.counters(), b.region_counts())
+        b.close()
+    finally:
+        oracle_mod.use_all_cores(False)
+    assert len(ra[0][1]) > 500 and ra[3] == rb[3]
+    assert np.array_equal(ra[0][0], rb[0][0]) and np.array_equal(ra[0][1], rb[0][1])
+    assert np.array_equal(ra[1], rb[1]) and np.array_equal(ra[4], rb[4])
+    for x, y in zip(ra[2], rb[2]):
+        assert np.array_equal(x, y)
+
+
+def test_cpu_baseline_reports_one_core_all_cores_and_the_host():
+    sys.path.insert(0, ROOT)
+    import argparse
+    import bench
+    args = argparse.Namespace(rate=7, ref_scale=0.01, ref_warm_steps=50)
+    c = bench.cpu_baseline(args, steps_one=40, steps_all=40)
+    assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0
+    assert c["all_cores"]["cores"] == os.cpu_count() == c["nproc"] and c["all_cores"]["value"] > 0
+    assert c["cpu_model"] and "linear" in c["extrapolation"] and "no code" in c["external_reference"]
+
+
+def test_ncu_traffic_is_tied_to_the_kernel_sources():
+    sys.path.insert(0, ROOT)
+    import bench
+    v, why = bench._ncu_traffic("no such kernel")
+    assert v is None and isinstance(why, str)
+    assert len(bench._csrc_sha16()) == 16
