@@ -41,7 +41,8 @@ class TypeParams(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext")] + [
         ("G", C.c_double * 4), ("E", C.c_double * 4), ("tau_ms", C.c_double * 4),
         ("bg_rate_hz", C.c_double), ("bg_weight", C.c_double),
-        ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double)]
+        ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double),
+        ("iext_gamma_shape", C.c_double), ("iext_gamma_scale", C.c_double)]
 
 
 class SimParams(C.Structure):
@@ -100,6 +101,10 @@ def lib():
         L.orc_sim_set_ring.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_sim_get_iou.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_sim_set_iou.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_sim_get_iext.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_gamma_ppf.restype = C.c_double
+        L.orc_gamma_ppf.argtypes = [C.c_double] * 3
+        L.orc_gamma_table.argtypes = [C.c_double, C.c_double, C.c_void_p]
         L.orc_normal_table.argtypes = [C.c_void_p]
         L.orc_sim_region_counts.restype = C.c_int64
         L.orc_sim_region_counts.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
@@ -258,7 +263,7 @@ def _sim_params(d: dict) -> SimParams:
         q = p.type[i]
         for k in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext", "bg_rate_hz", "bg_weight"):
             setattr(q, k, float(t[k]))
-        for k in ("ou_mu", "ou_sigma", "ou_tau_ms"):          # OU background current, off by default
+        for k in ("ou_mu", "ou_sigma", "ou_tau_ms", "iext_gamma_shape", "iext_gamma_scale"):   # off by default
             setattr(q, k, float(t.get(k, 0.0)))
         for k in ("G", "E", "tau_ms"):
             for u in range(4):
@@ -334,6 +339,12 @@ class OracleSim:
         lib().orc_sim_get_iou(self.h, _p(out))
         return out
 
+    def iext(self):
+        """External current of every neuron (R31): a parameter drawn once at creation."""
+        out = np.zeros(self.N, np.float64)
+        lib().orc_sim_get_iext(self.h, _p(out))
+        return out
+
     def set_iou(self, v):
         v = np.ascontiguousarray(v, np.float64)
         assert v.shape == (self.N,)
@@ -368,6 +379,13 @@ class OracleSim:
         a = np.zeros(n, np.int32)
         lib().orc_sim_get_arrivals(self.h, _p(a))
         return a.reshape(-1, self.N, 4)
+
+
+def gamma_table(shape: float, scale: float) -> np.ndarray:
+    """The 65536 Gamma(shape, scale) quantiles (fp32) the per-neuron external currents are drawn from."""
+    tab = np.zeros(65536, np.float32)
+    lib().orc_gamma_table(float(shape), float(scale), _p(tab))
+    return tab
 
 
 def normal_table() -> np.ndarray:

@@ -80,7 +80,8 @@ enum : uint32_t {
     STREAM_REGION = 5, // region sizes and region matrix (host-side normals)
     STREAM_INTER = 6,  // source-region choice of an inter-region input
     STREAM_DEG = 7,    // out-degree of a neuron (out-degree mode)
-    STREAM_OU = 8      // Gaussian increments of the OU background current
+    STREAM_OU = 8,     // Gaussian increments of the OU background current
+    STREAM_IEXT = 9    // per-neuron external current (Gamma quantile table)
 };
 
 u32x4 draw(uint64_t seed, uint32_t stream, uint64_t a, uint64_t b) {
@@ -162,6 +163,44 @@ double norm_ppf(double p) {                      // bisection on the CDF
     return 0.5 * (lo + hi);
 }
 
+// Regularised lower incomplete gamma function P(a, x) = gamma(a, x) / Gamma(a): power series for x < a + 1, else one minus
+// the continued fraction of Q(a, x) (modified Lentz); a > 0, x >= 0.
+double gamma_p(double a, double x) {
+    if (x <= 0.0) return 0.0;
+    const double lg = std::lgamma(a);
+    if (x < a + 1.0) {
+        double ap = a, sum = 1.0 / a, del = sum;
+        for (int n = 0; n < 100000; ++n) {
+            ap += 1.0; del *= x / ap; sum += del;
+            if (std::fabs(del) < std::fabs(sum) * 1e-17) break;
+        }
+        return sum * std::exp(-x + a * std::log(x) - lg);
+    }
+    const double tiny = 1e-300;
+    double b = x + 1.0 - a, c = 1.0 / tiny, d = 1.0 / b, h = d;
+    for (int i = 1; i < 100000; ++i) {
+        const double an = -(double)i * ((double)i - a);
+        b += 2.0;
+        d = an * d + b; if (std::fabs(d) < tiny) d = tiny;
+        c = b + an / c; if (std::fabs(c) < tiny) c = tiny;
+        d = 1.0 / d;
+        const double del = d * c;
+        h *= del;
+        if (std::fabs(del - 1.0) < 1e-16) break;
+    }
+    return 1.0 - std::exp(-x + a * std::log(x) - lg) * h;
+}
+// Quantile of the Gamma(shape k, scale theta) distribution: bisection on P(k, x / theta) = p.
+double gamma_ppf(double p, double k, double theta) {
+    double lo = 0.0, hi = k + 10.0;
+    while (gamma_p(k, hi) < p) hi *= 2.0;
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (gamma_p(k, mid) < p) lo = mid; else hi = mid;
+    }
+    return theta * 0.5 * (lo + hi);
+}
+
 // IEEE binary16 round-to-nearest-even of a float, returned as float.
 float round_to_half(float f) {
     uint32_t x; std::memcpy(&x, &f, 4);
@@ -202,6 +241,10 @@ struct orc_type_params {
     // Ext. Table 2), read per R3: I += (mu - I) dt/tau + sigma sqrt(2 dt/tau) xi, xi ~ N(0,1).
     // ou_tau_ms = 0 switches it off.
     double ou_mu, ou_sigma, ou_tau_ms;
+    // External current per neuron ("independently sampled following a Gamma distribution"; property table
+    // P:L821), reading R31: I_ext,i = Iext + Gamma(shape, scale) drawn once per neuron through a 65,536-point quantile table
+    // indexed by the top 16 bits of a Philox word (stream 9, counter = neuron).  iext_gamma_shape = 0: every neuron gets Iext.
+    double iext_gamma_shape, iext_gamma_scale;
 };
 
 struct orc_sim_params {
@@ -246,6 +289,10 @@ int32_t orc_poisson_thresholds(double lambda, uint32_t* T) { return poisson_thre
 int32_t orc_poisson_count(uint32_t u, const uint32_t* T, int32_t M) { return poisson_count(u, T, M); }
 uint32_t orc_prp(uint32_t x, uint32_t M, const uint32_t* key4) { return prp(x, M, key4); }
 double orc_norm_ppf(double p) { return norm_ppf(p); }
+double orc_gamma_ppf(double p, double k, double theta) { return gamma_ppf(p, k, theta); }
+void orc_gamma_table(double k, double theta, float* tab /*[65536]*/) {
+    for (int q = 0; q < 65536; ++q) tab[q] = (float)gamma_ppf(((double)q + 0.5) / 65536.0, k, theta);
+}
 float orc_round_to_half(float f) { return round_to_half(f); }
 
 // =============================================================================
@@ -550,6 +597,7 @@ struct TypeConst {
     int32_t wq_bg;
     uint32_t T[POISSON_MAX]; int M;
     bool ou = false;        // OU background current on
+    double ix_shape = 0, ix_scale = 0;   // Gamma law of the per-neuron external current (0: constant)
     real ou_mu = 0, ou_a = 0, ou_s = 0;   // mean, dt/tau, sigma sqrt(2 dt/tau): formed in double, rounded once
 };
 
@@ -570,6 +618,7 @@ struct Sim {
     // state
     std::vector<real> V, g;           // g[4*i+u]
     std::vector<real> Iou;            // OU background current (R3)
+    std::vector<real> Iext;           // external current of every neuron (R31): a parameter, drawn once
     std::vector<float> ntab;          // 65536 standard-normal quantiles, Phi^-1((q + 0.5) / 65536), as fp32
     std::vector<int32_t> ref;
     std::vector<int32_t> ring;        // ring[(slot*N + i)*4 + u]
@@ -621,7 +670,7 @@ struct Sim {
             real t1 = (c.G[1] * gi[1]) * (c.E[1] - v);
             real t2 = (c.G[2] * gi[2]) * (c.E[2] - v);
             real t3 = (c.G[3] * gi[3]) * (c.E[3] - v);
-            real I = (((t0 + t1) + t2) + t3) + c.Iext;
+            real I = (((t0 + t1) + t2) + t3) + Iext[(size_t)i];
             // 4b. OU background current (SI Eq.(4); R3): the membrane step sees I_ou(t), then
             //     I_ou(t+dt) = I_ou + ((mu - I_ou) dt/tau + sigma sqrt(2 dt/tau) xi); one Philox block serves 4
             //     neurons, xi = table[top 16 bits of the word]
@@ -718,6 +767,7 @@ Sim<real>* sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
         c.R = (int32_t)std::lrint(q.Tref_ms / p->dt_ms);
         c.wq_bg = (int32_t)std::lrint(q.bg_weight * std::ldexp(1.0, p->S));
         c.M = poisson_thresholds(q.bg_rate_hz * p->dt_ms * 1e-3, c.T);
+        c.ix_shape = q.iext_gamma_shape; c.ix_scale = q.iext_gamma_scale;
         if (q.ou_tau_ms > 0) {
             c.ou = true;
             c.ou_mu = (real)q.ou_mu;
@@ -730,6 +780,22 @@ Sim<real>* sim_create(const orc_sim_params* p, int64_t N, const uint8_t* ntype,
     for (int q = 0; q < 65536; ++q) s->ntab[(size_t)q] = (float)norm_ppf(((double)q + 0.5) / 65536.0);
     s->Iou.resize((size_t)N);
     for (int64_t i = 0; i < N; ++i) s->Iou[(size_t)i] = s->tc[ntype[i]].ou ? s->tc[ntype[i]].ou_mu : (real)0;
+    // per-neuron external current (R31): Iext + table[top 16 bits of Philox(stream 9, neuron)], one fp32 addition
+    s->Iext.resize((size_t)N);
+    {
+        std::vector<std::vector<float>> gtab(s->tc.size());
+        for (size_t t = 0; t < s->tc.size(); ++t)
+            if (s->tc[t].ix_shape > 0) {
+                gtab[t].resize(65536);
+                for (int q = 0; q < 65536; ++q) gtab[t][(size_t)q] = (float)gamma_ppf(((double)q + 0.5) / 65536.0, s->tc[t].ix_shape, s->tc[t].ix_scale);
+            }
+        for (int64_t i = 0; i < N; ++i) {
+            const size_t t = ntype[i];
+            real v = s->tc[t].Iext;
+            if (s->tc[t].ix_shape > 0) v = v + (real)gtab[t][draw(seed, STREAM_IEXT, (uint64_t)i, 0).w[0] >> 16];
+            s->Iext[(size_t)i] = v;
+        }
+    }
     s->V.resize((size_t)N); s->g.assign((size_t)N * 4, (real)0); s->ref.assign((size_t)N, 0);
     s->ring.assign((size_t)p->D * (size_t)N * 4, 0);
     for (int64_t i = 0; i < N; ++i) {
@@ -762,6 +828,11 @@ void orc_sim_get_iou(void* hv, double* out) {
     Handle* h = (Handle*)hv;
     const int64_t N = h->fp64 ? h->d->N : h->f->N;
     for (int64_t i = 0; i < N; ++i) out[i] = h->fp64 ? h->d->Iou[(size_t)i] : (double)h->f->Iou[(size_t)i];
+}
+void orc_sim_get_iext(void* hv, double* out) {
+    Handle* h = (Handle*)hv;
+    const int64_t N = h->fp64 ? h->d->N : h->f->N;
+    for (int64_t i = 0; i < N; ++i) out[i] = h->fp64 ? h->d->Iext[(size_t)i] : (double)h->f->Iext[(size_t)i];
 }
 void orc_sim_set_iou(void* hv, const double* in) {
     Handle* h = (Handle*)hv;
