@@ -259,16 +259,20 @@ def reduce_over_ranks(dist, device, ms: float, sums: list):
 
 
 # --------------------------------------------------------------------------------------------- CUDA arm
-def _make_cfg(idx, rate, scale=1.0, drive="poisson", spike_bin=1, dt_ms=0.1):
+def _make_cfg(idx, rate, scale=1.0, drive="poisson", spike_bin=1, dt_ms=0.1, iext_gamma=False):
     cfg = db_inputs.config(idx, rate_hz=(rate if idx == 1 else None), scale=scale)
     cfg["sim"]["dt_ms"] = dt_ms
+    if iext_gamma:                              # per-neuron external currents (R31): zero-mean Gamma(4, 0.01) spread
+        for t in cfg["sim"]["types"]:
+            t.update(Iext=-0.04, iext_gamma_shape=4.0, iext_gamma_scale=0.01)
     if drive == "ou":                           # the paper's production drive instead of Poisson
         db_inputs.ou_drive(cfg["sim"], rate)
     cfg["sim"]["spike_bin_steps"] = spike_bin
     return cfg
 
 
-def measure(db, torch, cfg, exec_mode, n_sim, steps, warmup, profile_steps, local, seed_off=0, barrier=None, drive="poisson"):
+def measure(db, torch, cfg, exec_mode, n_sim, steps, warmup, profile_steps, local, seed_off=0, barrier=None, drive="poisson",
+            extra_bytes=0):
     """Creates the simulation, runs `warmup` untimed and `steps` timed db_step(n_sim) calls (CUDA events on the stream
     the library launches on, one per call) and, in the two-kernel modes, `profile_steps` steps with events around
     every kernel.  Returns (sim, record); the caller destroys sim."""
@@ -303,7 +307,7 @@ def measure(db, torch, cfg, exec_mode, n_sim, steps, warmup, profile_steps, loca
     events, spikes = c1["events"] - c0["events"], c1["spikes"] - c0["spikes"]
     used = c1["exec_mode"]
     peak, peak_src = _peaks()
-    upd_per = UPDATE_BYTES_PER_NEURON_STEP + (8 if drive == "ou" else 0)      # + read and write of I_ou
+    upd_per = UPDATE_BYTES_PER_NEURON_STEP + (8 if drive == "ou" else 0) + extra_bytes      # + read and write of I_ou (+ read of I_ext)
     ev_bytes = DELIVER_BYTES_PER_EVENT[fp16]
     secs = ms * 1e-3
     bio_s = steps * n_sim * cfg["sim"]["dt_ms"] * 1e-3
@@ -499,10 +503,10 @@ def run_ours(args):
     rates, configs, variants = {}, {}, {}
     if rank == 0 and world == 1 and not args.no_sweep and args.config == 1 and args.scale == 1.0 and args.drive == "poisson" \
             and args.dt == 0 and args.spike_bin == 1:
-        def sub(cfg_s, n_sim_s, steps_s, warm_s, prof_s, drive="poisson"):
+        def sub(cfg_s, n_sim_s, steps_s, warm_s, prof_s, drive="poisson", extra_bytes=0):
             torch.cuda.empty_cache()
             t0 = time.perf_counter()
-            sm, r = measure(db, torch, cfg_s, db.EXEC_AUTO, n_sim_s, steps_s, warm_s, prof_s, local, drive=drive)
+            sm, r = measure(db, torch, cfg_s, db.EXEC_AUTO, n_sim_s, steps_s, warm_s, prof_s, local, drive=drive, extra_bytes=extra_bytes)
             sm.db_destroy()
             del sm
             r = _public(r)
@@ -515,6 +519,8 @@ def run_ours(args):
         # the paper's production mode: dt = 1 ms (b_t = dt), OU drive; RTF comparable in kind with BASELINE.md 1a
         variants["dt_1ms_ou"] = sub(_make_cfg(1, 7, drive="ou", dt_ms=1.0), 1000, 5, 3, 0, drive="ou")
         variants["dt_0.1ms_ou_bin10"] = sub(_make_cfg(1, 7, drive="ou", spike_bin=10), 1000, 5, 3, 0, drive="ou")
+        # per-neuron external currents from a Gamma law (R31): one more fp32 plane read by the update (62 B per neuron-step)
+        variants["iext_gamma_plane"] = sub(_make_cfg(1, 7, iext_gamma=True), 1000, 5, 3, 0, extra_bytes=4)
         for idx, (n_s, st_s, wm_s) in {2: (500, 2, 3), 4: (500, 2, 3), 3: (150, 2, 4)}.items():
             if idx == 3 and args.skip_config3:
                 configs["3"] = "skipped (--skip-config3)"

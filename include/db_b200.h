@@ -67,6 +67,12 @@ typedef struct db_type_params {
      * 0.12, tau 10), read per R3: I += (mu - I) dt/tau + sigma sqrt(2 dt/tau) xi, xi ~ N(0,1) from a
      * 65536-point quantile table; enters the membrane equation as a current.  ou_tau_ms = 0: off. */
     double ou_mu, ou_sigma, ou_tau_ms;
+    /* External current per neuron ("I_ext,i are parameters, independently sampled following a Gamma
+     * distribution"; property table; reading R31): I_ext,i = Iext + Gamma(shape, scale), drawn once per neuron at
+     * creation through a 65,536-point quantile table (top 16 bits of a Philox word keyed by dyn_seed, stream 9, neuron).
+     * iext_gamma_shape = 0: every neuron of the type gets Iext.  When any type uses it the currents are an extra fp32
+     * plane the update streams (+4 B per neuron-step); readable and writable as DB_FIELD_IEXT. */
+    double iext_gamma_shape, iext_gamma_scale;
 } db_type_params;
 
 /* Balloon-Windkessel BOLD read-out per region (Extended Data Table 4; reading R30): one explicit Euler
@@ -194,6 +200,7 @@ typedef struct db_phase_times {
 #define DB_FIELD_RING   7  /* int32  [D][count][4] fixed-point arrivals, slot = step mod D */
 #define DB_FIELD_OUTDEG 8  /* int32  [count], out-degree = length of the neuron's destination list (read only) */
 #define DB_FIELD_IOU    9  /* float  [count], OU background current (zeros when no type uses it) */
+#define DB_FIELD_IEXT  10  /* float  [count], external current of every neuron (R31); writable only when the plane exists */
 
 /* a0: generate the network on the device from `spec` (seed keys every draw of
  * the generator), build the CSR and initialise the state (V0 keyed by

@@ -17,7 +17,7 @@ from . import build as _build
 DB_OK, DB_EINVAL, DB_ENOMEM, DB_ECUDA, DB_ERANGE, DB_ESTATE = 0, -1, -2, -3, -4, -5
 EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 (FIELD_V, FIELD_G_AMPA, FIELD_G_NMDA, FIELD_G_GABAA, FIELD_G_GABAB, FIELD_REF, FIELD_TYPE, FIELD_RING,
- FIELD_OUTDEG, FIELD_IOU) = range(10)
+ FIELD_OUTDEG, FIELD_IOU, FIELD_IEXT) = range(11)
 
 EXPORTS = [
     "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_step_profiled", "db_read_spikes",
@@ -36,7 +36,8 @@ class TypeParams(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext")] + [
         ("G", C.c_double * 4), ("E", C.c_double * 4), ("tau_ms", C.c_double * 4),
         ("bg_rate_hz", C.c_double), ("bg_weight", C.c_double),
-        ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double)]
+        ("ou_mu", C.c_double), ("ou_sigma", C.c_double), ("ou_tau_ms", C.c_double),
+        ("iext_gamma_shape", C.c_double), ("iext_gamma_scale", C.c_double)]
 
 
 BOLD_KEYS = ("kappa", "gamma", "tau", "alpha", "rho", "V0", "k1", "k2", "k3", "z_scale")
@@ -149,7 +150,7 @@ def _fill_sim_params(p: SimParams, d: dict, dyn_seed: int, exec_mode: int, raste
         q = p.type[i]
         for k in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext", "bg_rate_hz", "bg_weight"):
             setattr(q, k, float(t[k]))
-        for k in ("ou_mu", "ou_sigma", "ou_tau_ms"):          # OU background current, off by default
+        for k in ("ou_mu", "ou_sigma", "ou_tau_ms", "iext_gamma_shape", "iext_gamma_scale"):   # off by default
             setattr(q, k, float(t.get(k, 0.0)))
         for k in ("G", "E", "tau_ms"):
             for u in range(4):

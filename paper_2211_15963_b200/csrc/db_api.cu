@@ -34,6 +34,7 @@ struct db_sim {
     uint64_t spike_cap = 0, work_cap = 0;
     std::vector<int64_t> region_start;
     uint8_t* ntype_dev = nullptr;
+    float* iext_tab_dev = nullptr;  // [kMaxTypes][65536] Gamma quantiles of the per-neuron external currents (R31)
     int exec_mode = DB_EXEC_KERNELS;
     int deliver_grid = 0;
     bool heavy = false;             // some row is longer than kInlineMax
@@ -130,6 +131,9 @@ int32_t make_type_consts(db_sim* sim, const db_sim_params& sp, TypeConst* tc) {
         if (!saturated) return fail(sim, DB_EINVAL, "bg_rate_hz * dt too large for the Poisson table");
         c.M = M;
         if (!(q.ou_tau_ms >= 0) || !(q.ou_sigma >= 0)) return fail(sim, DB_EINVAL, "OU parameters out of range");
+        if (!(q.iext_gamma_shape >= 0) || (q.iext_gamma_shape > 0 && !(q.iext_gamma_scale > 0)))
+            return fail(sim, DB_EINVAL, "iext_gamma_shape must be >= 0 and iext_gamma_scale > 0 with it");
+        c.ix_on = q.iext_gamma_shape > 0 ? 1 : 0;
         if (q.ou_tau_ms > 0) {          // OU background current (R3): constants formed in double, rounded once
             c.ou = 1;
             c.ou_mu = (float)q.ou_mu;
@@ -224,6 +228,20 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
         CK(cudaMemcpyAsync(ntab, tab.data(), 65536 * sizeof(float), cudaMemcpyHostToDevice, sim->stream));
         CK(cudaStreamSynchronize(sim->stream));
         d.ntab = ntab;
+    }
+    bool ix_any = false;
+    for (int t = 0; t < sp->n_types; ++t) ix_any |= d.tc[t].ix_on != 0;
+    if (ix_any) {                       // per-neuron external currents (R31): the plane and the Gamma quantile tables of the types
+        if ((rc = alloc_zero(sim, &d.iext, Np))) return rc;
+        if ((rc = alloc_zero(sim, &sim->iext_tab_dev, (size_t)kMaxTypes * 65536))) return rc;
+        std::vector<float> tab(65536);
+        for (int t = 0; t < sp->n_types; ++t) {
+            if (!d.tc[t].ix_on) continue;
+            for (int q = 0; q < 65536; ++q)
+                tab[(size_t)q] = (float)gamma_quantile(((double)q + 0.5) / 65536.0, sp->type[t].iext_gamma_shape, sp->type[t].iext_gamma_scale);
+            CK(cudaMemcpyAsync(sim->iext_tab_dev + (size_t)t * 65536, tab.data(), 65536 * sizeof(float), cudaMemcpyHostToDevice, sim->stream));
+            CK(cudaStreamSynchronize(sim->stream));
+        }
     }
     if ((rc = alloc_zero(sim, &d.ring, (size_t)d.D * 4 * Np))) return rc;
     uint64_t cap = sp->raster_capacity ? sp->raster_capacity : (1ull << 24);
@@ -380,7 +398,7 @@ int32_t finish_setup(db_sim* sim, uint64_t work_cap, uint64_t heavy_chunks) {
     d.work_half = sim->work_cap;
     if ((rc = alloc_zero(sim, &d.work, 2 * (size_t)sim->work_cap))) return rc;
     sim->heavy = heavy_chunks > 0;
-    CK(launch_init_state(d, sim->ntype_dev, sim->stream));
+    CK(launch_init_state(d, sim->ntype_dev, sim->iext_tab_dev, sim->stream));
     sim->deliver_grid = sim->n_sm * 8;
     sim->update_sm = sim->n_sm;
     int coop = 0;
@@ -841,6 +859,14 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
         if (d.ou_on) CK(cudaMemcpy(dst, d.Iou + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
         else std::memset(dst, 0, (size_t)count * 4);
         break;
+    case DB_FIELD_IEXT:
+        if (d.iext) CK(cudaMemcpy(dst, d.iext + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
+        else {                          // no plane: every neuron carries the constant of its type
+            std::vector<uint16_t> t((size_t)count);
+            CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));
+            for (int64_t i = 0; i < count; ++i) static_cast<float*>(dst)[i] = d.tc[t[(size_t)i] >> 12].Iext;
+        }
+        break;
     case DB_FIELD_RING: {
         // API slot j holds the arrivals of the step t in [n, n + D) with t mod D == j; device slot = t mod d.D
         Ctl c;
@@ -892,6 +918,9 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
     case DB_FIELD_IOU:
         if (!d.ou_on) return fail(sim, DB_ESTATE, "no neuron type uses the OU background current");
         CK(cudaMemcpy(d.Iou + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
+    case DB_FIELD_IEXT:
+        if (!d.iext) return fail(sim, DB_ESTATE, "no neuron type draws its external current per neuron (iext_gamma_shape = 0)");
+        CK(cudaMemcpy(d.iext + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
     case DB_FIELD_REF: {
         std::vector<uint16_t> t((size_t)count);
         CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));

@@ -17,7 +17,7 @@ constexpr int kRefMask = 0x0FFF;     // rt = type << 12 | refractory steps left
 
 // Philox streams
 constexpr uint32_t kStreamV0 = 1, kStreamBG = 2, kStreamSRC = 3, kStreamSYN = 4,
-                   kStreamREGION = 5, kStreamINTER = 6, kStreamDEG = 7, kStreamOU = 8;
+                   kStreamREGION = 5, kStreamINTER = 6, kStreamDEG = 7, kStreamOU = 8, kStreamIEXT = 9;
 
 struct TypeConst {                   // per neuron type, rounded once on the host
     float neg_gL, VL, Vth, Vreset, kappa, Iext;
@@ -28,6 +28,7 @@ struct TypeConst {                   // per neuron type, rounded once on the hos
     uint32_t T[kPoissonMax];
     float ou_mu, ou_a, ou_s;         // OU background: mean, dt / tau, sigma sqrt(2 dt / tau) (0 when off)
     int32_t ou;                      // OU background on for this type
+    int32_t ix_on;                   // external current of the type's neurons has a Gamma part (R31)
 };
 
 struct alignas(128) Ctl {            // device-resident control block
@@ -67,6 +68,7 @@ struct SimDev {                      // passed by value to every kernel
     float* Iou;                      // [Npad] OU background current (allocated only if some type uses it)
     const float* ntab;               // [65536] standard-normal quantiles (same condition)
     int32_t ou_on;
+    float* iext;                     // [Npad] external current per neuron (R31; allocated only if some type draws it from a Gamma law)
     int32_t bg_on;                   // some type has a Poisson background (else its Philox draw is skipped)
     int32_t bin_steps;               // time bin b_t for transferring spikes, in steps (>= 1; R29)
     int32_t* ring;                   // [D][4][Npad] fixed-point arrivals

@@ -43,6 +43,57 @@ double std_normal_quantile(double p) {
     return z;
 }
 
+// Quantile of the Gamma(shape k, scale theta) law (per-neuron external currents, R31).  The regularised incomplete gamma
+// function comes from Kummer's series for the lower part and from the even part of Legendre's continued fraction,
+// summed by its forward (Wallis) recurrence, for the upper part; the root is found by a bracketed Newton iteration on
+// whichever tail is the smaller one, started from the Wilson-Hilferty approximation.
+static void gamma_tails(double a, double x, double* P, double* Q) {
+    if (x <= 0.0) { *P = 0.0; *Q = 1.0; return; }
+    const double front = std::exp(a * std::log(x) - x - std::lgamma(a));
+    if (x < a + 1.0) {
+        double term = 1.0 / a, sum = term;
+        for (int n = 1; n < 200000; ++n) {
+            term *= x / (a + (double)n);
+            sum += term;
+            if (term < sum * 1e-17) break;
+        }
+        *P = front * sum; *Q = 1.0 - *P;
+        return;
+    }
+    // Q = front / (x + 1 - a - 1 (1 - a) / (x + 3 - a - 2 (2 - a) / (x + 5 - a - ...))): convergents A_n / B_n
+    double A0 = 1.0, B0 = 0.0, A1 = 0.0, B1 = 1.0, prev = 0.0;      // A_{-1}, B_{-1}, A_0 = b_0 = 0, B_0 = 1
+    for (int n = 1; n < 200000; ++n) {
+        const double an = (n == 1) ? 1.0 : -((double)(n - 1)) * ((double)(n - 1) - a);
+        const double bn = x + (double)(2 * n - 1) - a;
+        const double A2 = bn * A1 + an * A0, B2 = bn * B1 + an * B0;
+        A0 = A1; B0 = B1; A1 = A2; B1 = B2;
+        if (std::fabs(B1) > 1e200) { A0 *= 1e-200; B0 *= 1e-200; A1 *= 1e-200; B1 *= 1e-200; }
+        const double cur = A1 / B1;
+        if (n > 1 && std::fabs(cur - prev) <= 1e-17 * std::fabs(cur)) { prev = cur; break; }
+        prev = cur;
+    }
+    *Q = front * prev; *P = 1.0 - *Q;
+}
+
+double gamma_quantile(double p, double k, double theta) {
+    const double z = std_normal_quantile(p), c = 1.0 / (9.0 * k);
+    double x = k * std::pow(std::max(1.0 - c + z * std::sqrt(c), 1e-3), 3.0);
+    double lo = 0.0, hi = std::max(4.0 * x, k + 20.0);
+    for (;;) { double P, Q; gamma_tails(k, hi, &P, &Q); if (P >= p) break; hi *= 2.0; }
+    for (int it = 0; it < 400; ++it) {
+        double P, Q;
+        gamma_tails(k, x, &P, &Q);
+        const double f = (p <= 0.5) ? (P - p) : ((1.0 - p) - Q);      // the smaller tail carries the precision
+        if (f > 0.0) hi = x; else lo = x;
+        const double pdf = std::exp((k - 1.0) * std::log(x) - x - std::lgamma(k));
+        double xn = (pdf > 0.0) ? x - f / pdf : 0.5 * (lo + hi);
+        if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);
+        if (xn == x || hi - lo <= 1e-17 * hi) break;
+        x = xn;
+    }
+    return theta * x;
+}
+
 namespace {
 
 double normal_from_words(uint32_t u0, uint32_t u1) {     // Box-Muller, double

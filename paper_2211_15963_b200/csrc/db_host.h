@@ -10,7 +10,7 @@
 namespace dbk {
 
 // ---- db_step.cu ------------------------------------------------------------
-cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st);
+cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, const float* iext_tab_dev /*[types][65536] or NULL*/, cudaStream_t st);
 cudaError_t prepare_kernels();                                            // per handle, on its device: opt-in shared-memory sizes
 cudaError_t launch_update(const SimDev& p, int n_sm, int mode, cudaStream_t st);   // mode: see k_update_stream
 cudaError_t launch_deliver(const SimDev& p, int grid, unsigned parity, cudaStream_t st);   // parity = step & 1 (list mode: which work-list half)
@@ -45,6 +45,7 @@ struct GenHostTables {                 // distribution tables formed on the host
 };
 
 double std_normal_quantile(double p);   // inverse normal CDF (Newton on erfc), double precision
+double gamma_quantile(double p, double shape, double scale);   // inverse Gamma CDF, double precision
 
 bool gen_host_tables(const db_network_spec& spec, uint64_t seed, GenHostTables* out, std::string* err);
 

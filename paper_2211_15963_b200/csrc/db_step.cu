@@ -356,7 +356,8 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
                                                  const int i0, int32_t* slot, const int next_off,
                                                  const uint4 v_bits, const uint2 rt_bits, const uint4 rnd,
                                                  unsigned& bg_acc, float4* iou = nullptr,
-                                                 const float4 xi_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f)) {
+                                                 const float4 xi_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f),
+                                                 const float4 ix = make_float4(0.0f, 0.0f, 0.0f, 0.0f)) {
     const size_t Np = (size_t)p.Npad;
     const int tp[4] = {tp0, tp1, tp2, tp3};
     const uint32_t rw[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
@@ -425,7 +426,9 @@ __device__ __forceinline__ unsigned neuron_group(const SimDev& p, const TypeSmem
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const float4 m0 = s_tc[tp[q]].m0, m1 = s_tc[tp[q]].m1;
-            float Iq = __fadd_rn(I[q], m0.w);
+            // external current: the neuron's own (R31, when the plane exists) or the constant of its type
+            const float ie = p.iext ? ((q == 0) ? ix.x : (q == 1) ? ix.y : (q == 2) ? ix.z : ix.w) : m0.w;
+            float Iq = __fadd_rn(I[q], ie);
             if (kOU) {                 // OU background current (R3): the membrane step sees I_ou(t); then
                 const float4 m3 = s_tc[tp[q]].m3;   // I_ou += (mu - I_ou) dt/tau + sigma sqrt(2 dt/tau) xi
                 if (__float_as_int(m3.w)) {
@@ -491,6 +494,8 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
         rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
                              __ldg(p.ntab + (wo.w >> 16)));
     }
+    float4 ix = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (kA && p.iext) ix = ld_cg_f4(p.iext + i0);   // per-neuron external currents (R31): one more plane, read only
     cp_async_wait_all();
     const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
     const uint2 rt_bits = lds64(sg.srt);
@@ -502,9 +507,9 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
     unsigned spike_bits;
     if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou, ix);
     else                                // a type boundary inside the group (rare)
-        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+        spike_bits = neuron_group<kB, kA, false, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou, ix);
     if (ou) st_cg_f4(p.Iou + i0, iou);
     cp_async_commit();
     if (!kA) return;
@@ -902,6 +907,8 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
             rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
                                  __ldg(p.ntab + (wo.w >> 16)));
         }
+        float4 ix = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (kA && p.iext) ix = ld_cg_f4(p.iext + i0);   // per-neuron external currents (R31)
         cp_async_wait_all();
         const uint4 v_bits = lds128(sg.sbase + 4u * kPlaneStride);
         const uint2 rt_bits = lds64(sg.srt);
@@ -913,9 +920,9 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int tp2 = (int)((rt_bits.y >> 12) & 0xFu), tp3 = (int)(rt_bits.y >> 28);
         unsigned spike_bits;
         if (tp0 == tp1 && tp0 == tp2 && tp0 == tp3)
-            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp0, tp0, tp0, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou, ix);
         else                            // a type boundary inside the group (rare)
-            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou);
+            spike_bits = neuron_group<kB, kA, kClassic, kOU>(p, s_tc, s_T, sg, tp0, tp1, tp2, tp3, i0, slot0 + i0, next_off, v_bits, rt_bits, rnd, bg_acc, &iou, rnd_ou, ix);
         if (kOU && kA) st_cg_f4(p.Iou + i0, iou);
         cp_async_commit();
         if (kA && __ballot_sync(0xffffffffu, spike_bits != 0)) emit_global(p, n, sb, i0, lane, spike_bits);
@@ -941,7 +948,7 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
 // State initialisation: V0 = Vreset + (Vth - Vreset) * U, U = (u >> 8) * 2^-24
 // keyed by (dyn_seed, STREAM_V0, i); g = 0, ref = 0.
 // ---------------------------------------------------------------------------
-__global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __restrict__ ntype) {
+__global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __restrict__ ntype, const float* __restrict__ iext_tab) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.Npad) return;
     const int tp = (i < p.N) ? ntype[i] : 0;
@@ -952,6 +959,14 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
     for (int u = 0; u < 4; ++u) p.g[(size_t)u * p.Npad + i] = 0.0f;
     p.rt[i] = (uint16_t)(tp << 12);
     if (p.ou_on) p.Iou[i] = (i < p.N && c.ou) ? c.ou_mu : 0.0f;   // the OU current starts at its mean
+    if (p.iext) {                      // external current of the neuron (R31): Iext + Gamma quantile at the top 16 bits of a Philox word
+        float v = 0.0f;
+        if (i < p.N) {
+            v = c.Iext;
+            if (c.ix_on) v = __fadd_rn(v, iext_tab[(size_t)tp * 65536u + (philox4x32_10(make_uint4((uint32_t)i, kStreamIEXT << 24, 0u, 0u), p.seed_lo, p.seed_hi).x >> 16)]);
+        }
+        p.iext[i] = v;
+    }
 }
 
 // ===========================================================================
@@ -1362,8 +1377,8 @@ __global__ void __launch_bounds__(256) k_lists_to_ring(const __grid_constant__ S
 // ---------------------------------------------------------------------------
 // host-side launchers (called from db_api.cu)
 // ---------------------------------------------------------------------------
-cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, cudaStream_t st) {
-    k_init_state<<<(p.Npad + 255) / 256, 256, 0, st>>>(p, ntype_dev);
+cudaError_t launch_init_state(const SimDev& p, const uint8_t* ntype_dev, const float* iext_tab_dev, cudaStream_t st) {
+    k_init_state<<<(p.Npad + 255) / 256, 256, 0, st>>>(p, ntype_dev, iext_tab_dev);
     return cudaGetLastError();
 }
 

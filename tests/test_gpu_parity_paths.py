@@ -214,3 +214,31 @@ def test_deferred_mode_ring_write_after_the_first_step_is_refused(db):
         g.db_write_state(7, r)
     assert e.value.code == db.binding.DB_ESTATE
     g.db_write_state(0, np.full(600, -60.0, np.float32))            # the other fields stay writable
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_per_neuron_external_current_from_a_gamma_law(db, oracle_mod, mode):
+    # SURVEY 8(f) row 1, remainder: I_ext,i "independently sampled following a Gamma distribution" (R31) on
+    # one type, the constant of the type on the other; the plane is one more stream of the update (read only)
+    exc, inh = _distinct_types()
+    exc.update(Iext=0.05, iext_gamma_shape=2.5, iext_gamma_scale=0.06)
+    sim = db_inputs.sim_params(types=[exc, inh])
+    N = 7000 + 21
+    net = db_inputs.random_csr(N=N, mean_outdeg=25, seed=33, n_regions=2)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    Ig, Io = g.db_read_state(db.FIELD_IEXT), o.iext().astype(np.float32)
+    assert np.array_equal(Ig, Io)                                     # same table, same Philox words, one fp32 addition
+    assert np.all(Ig[net["ntype"] == 1] == np.float32(-0.05)) and Ig[net["ntype"] == 0].std() > 0.05
+    for upto in (1, 2, 80, 400):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        n = _check(g, o, upto)
+    assert n > 300
+    assert np.array_equal(g.db_read_state(db.FIELD_IEXT), Io)         # a parameter: the step loop does not touch it
+    # the plane can be rewritten (e.g. by an assimilation loop): the dynamics follow the written values
+    g.db_write_state(db.FIELD_IEXT, np.full(N, 0.05, np.float32))
+    h = db.Sim.db_create_from_csr(db_inputs.sim_params(types=[dict(exc, iext_gamma_shape=0.0), inh]), net, exec_mode=mode)
+    assert np.all(h.db_read_state(db.FIELD_IEXT)[net["ntype"] == 0] == np.float32(0.05))      # no plane: the constants
+    with pytest.raises(db.DbError) as e:
+        h.db_write_state(db.FIELD_IEXT, Io)
+    assert e.value.code == db.binding.DB_ESTATE
