@@ -144,6 +144,11 @@ typedef struct db_network_spec {
     double   w_mu, w_sigma, w_scale, inh_mult, slow_frac;     /* weights (R11), NMDA / GABA_B share (R12) */
     int32_t  delay_intra_min, delay_intra_max, delay_inter_min, delay_inter_max;  /* steps, 1..255 */
     int32_t  weight_fp16;        /* store weights as binary16 (config 3) instead of fp32 */
+    int64_t  own_first, own_count; /* region-sharded simulation (SI Eq.(6); layout P:L494): the handle owns
+                                    the neurons [own_first, own_first + own_count) of the N-neuron network -- their state, their
+                                    ring, and the synapses ONTO them from every source; own_first a multiple of 1024;
+                                    own_count = 0: the whole network.  DB_MODE_FIXED_INDEGREE only.  Ids in the raster, in
+                                    db_read_state / db_write_state and in db_deliver_external are global */
     db_sim_params sim;
     const db_runtime* runtime;   /* may be NULL */
 } db_network_spec;
@@ -160,6 +165,7 @@ typedef struct db_csr_view {
     const uint8_t* delay;        /* [E] delay in steps, 1 <= delay < D */
     const uint8_t* rec;          /* [E] receptor 0..3 */
     int32_t weight_fp16;         /* store on the device as binary16 (w must already be representable) */
+    int64_t own_first, own_count; /* as in db_network_spec: keep only the synapses onto [own_first, own_first + own_count); 0, 0 = all */
 } db_csr_view;
 
 /* Library-allocated host copy of the network (db_export_csr); release with db_free_csr. */
@@ -215,6 +221,14 @@ int32_t db_destroy(db_sim* sim);
 
 /* a1-a4 for n_steps consecutive time steps; asynchronous on the stream. */
 int32_t db_step(db_sim* sim, uint32_t n_steps);
+
+/* Region-sharded simulation, second sum of SI Eq.(6): the neurons `ids` [n] (global ids, HOST pointer; neurons
+ * this handle does NOT own) fired in time step `step`; their synapses onto the handle's neurons are pushed into its ring
+ * (arrival = end of the spike's time bin + delay).  To be called before the handle steps past `step` + the smallest
+ * delay of the network: DB_ERANGE otherwise (the arrival step would already be consumed), DB_EINVAL for an id out of
+ * range or owned by the handle.  Two handles that exchange their db_read_spikes output every d_min steps reproduce the
+ * single-handle simulation bit for bit (tests).  Asynchronous on the stream like db_step. */
+int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n);
 
 /* Same in DB_EXEC_KERNELS mode with CUDA events around every kernel; blocks
  * until done.  For per-kernel roofline measurement. */

@@ -20,7 +20,7 @@ EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
  FIELD_OUTDEG, FIELD_IOU, FIELD_IEXT) = range(11)
 
 EXPORTS = [
-    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_step_profiled", "db_read_spikes",
+    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_deliver_external", "db_step_profiled", "db_read_spikes",
     "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_export_csr",
     "db_free_csr", "db_get_counters", "db_synchronize", "db_last_error",
 ]
@@ -70,14 +70,16 @@ class NetworkSpec(C.Structure):
                 ("outdeg_sigma", C.c_double), ("outdeg_cap", C.c_int32), ("w_mu", C.c_double), ("w_sigma", C.c_double),
                 ("w_scale", C.c_double), ("inh_mult", C.c_double), ("slow_frac", C.c_double),
                 ("delay_intra_min", C.c_int32), ("delay_intra_max", C.c_int32), ("delay_inter_min", C.c_int32),
-                ("delay_inter_max", C.c_int32), ("weight_fp16", C.c_int32), ("sim", SimParams),
+                ("delay_inter_max", C.c_int32), ("weight_fp16", C.c_int32), ("own_first", C.c_int64), ("own_count", C.c_int64),
+                ("sim", SimParams),
                 ("runtime", C.POINTER(Runtime))]
 
 
 class CsrView(C.Structure):
     _fields_ = [("N", C.c_int64), ("E", C.c_int64), ("n_regions", C.c_int32), ("region_start", C.c_void_p),
                 ("ntype", C.c_void_p), ("row_ptr", C.c_void_p), ("tgt", C.c_void_p), ("w", C.c_void_p),
-                ("delay", C.c_void_p), ("rec", C.c_void_p), ("weight_fp16", C.c_int32)]
+                ("delay", C.c_void_p), ("rec", C.c_void_p), ("weight_fp16", C.c_int32), ("own_first", C.c_int64),
+                ("own_count", C.c_int64)]
 
 
 class CsrHost(C.Structure):
@@ -117,6 +119,7 @@ def load():
                                          C.POINTER(C.c_void_p)]
         L.db_destroy.argtypes = [C.c_void_p]
         L.db_step.argtypes = [C.c_void_p, C.c_uint32]
+        L.db_deliver_external.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64]
         L.db_step_profiled.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(PhaseTimes)]
         L.db_read_spikes.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_uint64,
                                      C.POINTER(C.c_uint64)]
@@ -227,7 +230,7 @@ class Sim:
     # -- construction --------------------------------------------------------
     @classmethod
     def db_create(cls, net: dict, sim: dict, seed: int, dyn_seed: int = 1, exec_mode: int = EXEC_AUTO,
-                  raster_capacity: int = 0, max_windows: int = 0, device: int = 0) -> "Sim":
+                  raster_capacity: int = 0, max_windows: int = 0, device: int = 0, own=None) -> "Sim":
         s = cls()
         s._rt = _TorchRuntime(device)
         spec = NetworkSpec()
@@ -237,16 +240,18 @@ class Sim:
                 setattr(spec, k, net[k])
         _fill_sim_params(spec.sim, sim, dyn_seed, exec_mode, raster_capacity, max_windows)
         spec.runtime = C.pointer(s._rt.rt)
+        if own is not None:                              # (first, count): the neurons this handle owns
+            spec.own_first, spec.own_count = int(own[0]), int(own[1])
         rc = s.L.db_create(C.byref(spec), int(seed), C.byref(s.h))
         if rc != DB_OK:
             raise DbError(rc, s.L.db_last_error(None).decode())
-        s._remember(net["N"], net["n_regions"], sim)
+        s._remember(net["N"], net["n_regions"], sim, own)
         return s
 
     @classmethod
     def db_create_from_csr(cls, sim: dict, net: dict, dyn_seed: int = 1, exec_mode: int = EXEC_AUTO,
                            raster_capacity: int = 0, max_windows: int = 0, fp16: bool = False,
-                           device: int = 0) -> "Sim":
+                           device: int = 0, own=None) -> "Sim":
         s = cls()
         s._rt = _TorchRuntime(device)
         sp = SimParams()
@@ -257,15 +262,16 @@ class Sim:
                 np.ascontiguousarray(net["ntype"], np.uint8), np.ascontiguousarray(net["row_ptr"], np.int64),
                 np.ascontiguousarray(net["tgt"], np.int32), np.ascontiguousarray(net["w"], np.float32),
                 np.ascontiguousarray(net["delay"], np.uint8), np.ascontiguousarray(net["rec"], np.uint8)]
-        v = CsrView(N, int(keep[2][-1]), R, *[_p(a) for a in keep], int(fp16))
+        v = CsrView(N, int(keep[2][-1]), R, *[_p(a) for a in keep], int(fp16), *(own if own is not None else (0, 0)))
         rc = s.L.db_create_from_csr(C.byref(sp), C.byref(v), C.byref(s._rt.rt), C.byref(s.h))
         if rc != DB_OK:
             raise DbError(rc, s.L.db_last_error(None).decode())
-        s._remember(N, R, sim)
+        s._remember(N, R, sim, own)
         return s
 
-    def _remember(self, N, R, sim):
+    def _remember(self, N, R, sim, own=None):
         self.N, self.R, self.D = int(N), int(R), int(sim["D"])
+        self.first, self.count = (int(own[0]), int(own[1])) if own is not None and own[1] else (0, int(N))
         self.dt_ms, self.window = float(sim["dt_ms"]), int(sim["window_steps"])
 
     def _ck(self, rc):
@@ -288,6 +294,10 @@ class Sim:
     # -- stepping ----------------------------------------------------------------
     def db_step(self, n_steps: int):
         self._ck(self.L.db_step(self.h, int(n_steps)))
+
+    def db_deliver_external(self, step: int, ids: np.ndarray):
+        ids = np.ascontiguousarray(ids, np.int32)
+        self._ck(self.L.db_deliver_external(self.h, int(step), _p(ids), len(ids)))
 
     def db_step_profiled(self, n_steps: int) -> dict:
         t = PhaseTimes()
@@ -315,8 +325,9 @@ class Sim:
         m = min(n.value, len(ids_out))
         return steps_out[:m], ids_out[:m]
 
-    def db_read_state(self, field: int, first: int = 0, count: int | None = None) -> np.ndarray:
-        count = self.N - first if count is None else count
+    def db_read_state(self, field: int, first: int | None = None, count: int | None = None) -> np.ndarray:
+        first = self.first if first is None else first
+        count = self.first + self.count - first if count is None else count
         if field == FIELD_RING:
             out = np.empty((self.D, count, 4), np.int32)
         elif field in (FIELD_REF, FIELD_OUTDEG):
@@ -328,7 +339,8 @@ class Sim:
         self._ck(self.L.db_read_state(self.h, field, first, count, _p(out)))
         return out
 
-    def db_write_state(self, field: int, values: np.ndarray, first: int = 0):
+    def db_write_state(self, field: int, values: np.ndarray, first: int | None = None):
+        first = self.first if first is None else first
         dt = np.int32 if field in (FIELD_REF, FIELD_RING) else np.float32
         v = np.ascontiguousarray(values, dt)
         count = v.shape[1] if field == FIELD_RING else v.shape[0]

@@ -39,6 +39,9 @@ struct db_sim {
     int deliver_grid = 0;
     bool heavy = false;             // some row is longer than kInlineMax
     int32_t max_delay = 0;          // largest synaptic delay, in steps
+    int32_t min_delay = 1;          // smallest one (db_deliver_external: how late an outside spike may arrive)
+    int32_t* ext_ids_dev = nullptr; // db_deliver_external: device copy of the id list
+    uint64_t ext_ids_cap = 0;
     double list_rate_hz = 0.0;      // arrival lists: mean firing rate their capacity was sized for
     int update_sm = 0;              // two-kernel mode: SM count the update kernel is shaped for
     cudaGraphExec_t graph_exec = nullptr;
@@ -171,12 +174,20 @@ int32_t open_device(db_sim* sim, const db_runtime* rt) {
 }
 
 // Everything except the CSR arrays: state, ring, lists, counters.
-int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_regions,
-                     const int64_t* region_start, int32_t max_delay) {
+int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N_all, int32_t n_regions,
+                     const int64_t* region_start, int32_t max_delay, int64_t own_first, int64_t own_count) {
     SimDev& d = sim->dev;
     sim->params = *sp;
-    if (N < 1 || N >= (1ll << 30)) return fail(sim, DB_EINVAL, "N must be within 1..2^30-1");
+    if (N_all < 1 || N_all >= (1ll << 30)) return fail(sim, DB_EINVAL, "N must be within 1..2^30-1");
     if (n_regions < 1 || n_regions > 65536) return fail(sim, DB_EINVAL, "n_regions must be 1..65536");
+    if (own_count == 0) { own_first = 0; own_count = N_all; }
+    if (own_first < 0 || own_count < 1 || own_first + own_count > N_all || own_first % kNeuronPad != 0)
+        return fail(sim, DB_EINVAL, "own_first must be a multiple of 1024 and [own_first, own_first + own_count) lie inside the network");
+    if (own_count != N_all && sp->bold.enabled)
+        return fail(sim, DB_EINVAL, "the BOLD read-out needs whole regions: not available on a handle that owns part of the network");
+    const int64_t N = own_count;                       // neurons of this handle: state, ring and targets are local
+    d.n_rows = (int32_t)N_all;
+    d.id0 = (int32_t)own_first;
     d.N = (int32_t)N;
     d.Npad = (int32_t)(((N + kNeuronPad - 1) / kNeuronPad) * kNeuronPad);
     // internal ring depth: the persistent kernel lets blocks run up to two steps apart and needs
@@ -203,7 +214,7 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
         if (d.bin_steps > d.tc[t].R + 1) return fail(sim, DB_EINVAL, "spike_bin_steps must be <= round(Tref / dt) + 1 of every type");
 
     sim->region_start.assign(region_start, region_start + n_regions + 1);
-    if (sim->region_start.front() != 0 || sim->region_start.back() != N)
+    if (sim->region_start.front() != 0 || sim->region_start.back() != N_all)
         return fail(sim, DB_EINVAL, "region_start must run from 0 to N");
     std::vector<int32_t> rs32((size_t)n_regions + 1);
     for (int r = 0; r <= n_regions; ++r) {
@@ -295,7 +306,7 @@ int32_t setup_common(db_sim* sim, const db_sim_params* sp, int64_t N, int32_t n_
 int32_t build_arrival_lists(db_sim* sim, bool* ok) {
     SimDev& d = sim->dev;
     *ok = false;
-    const int64_t N = d.N;
+    const int64_t N = d.n_rows;                        // CSR rows: one per neuron of the whole network
     const int max_ahead = sim->max_delay + d.bin_steps - 1;        // furthest arrival, in steps after the spike
     if (max_ahead <= 1 || sim->Epad < 16) return DB_OK;
     // synapses per delay
@@ -526,8 +537,12 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     int32_t max_delay = 0;
     for (int64_t e = 0; e < E; ++e) max_delay = std::max<int32_t>(max_delay, csr->delay[e]);
     if (max_delay >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
-    if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start, max_delay))) return bail(rc);
+    int32_t min_delay = 255;
+    for (int64_t e = 0; e < E; ++e) min_delay = std::min<int32_t>(min_delay, csr->delay[e]);
+    if ((rc = setup_common(sim, sp, N, csr->n_regions, csr->region_start, max_delay, csr->own_first, csr->own_count))) return bail(rc);
     sim->max_delay = max_delay;
+    sim->min_delay = E > 0 ? min_delay : 1;
+    const int64_t own0 = sim->dev.id0, own1 = own0 + sim->dev.N;     // keep the synapses onto [own0, own1)
     SimDev& d = sim->dev;
 
     // padded row layout + validation
@@ -535,17 +550,23 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     std::vector<int32_t> row_len((size_t)N);
     int64_t pos = 0;
     uint64_t work_cap = 0, heavy_chunks = 0;
+    int64_t E_own = 0;
     for (int64_t j = 0; j < N; ++j) {
-        const int64_t len = csr->row_ptr[j + 1] - csr->row_ptr[j];
+        int64_t len = csr->row_ptr[j + 1] - csr->row_ptr[j];
         if (len < 0 || len > 0x7FFFFFFF) return bail(fail(sim, DB_EINVAL, "row_ptr must be non-decreasing"));
         if (csr->ntype[j] >= sp->n_types) return bail(fail(sim, DB_EINVAL, "ntype out of range"));
+        if (own1 - own0 != N) {                          // only the synapses onto the owned neurons stay in the row
+            len = 0;
+            for (int64_t s = csr->row_ptr[j]; s < csr->row_ptr[j + 1]; ++s) len += (csr->tgt[s] >= own0 && csr->tgt[s] < own1);
+        }
+        E_own += len;
         row_begin[(size_t)j] = pos; row_len[(size_t)j] = (int32_t)len;
         pos += (len + kRowAlign - 1) / kRowAlign * kRowAlign;
         work_cap += (uint64_t)((len + kChunk - 1) / kChunk);
         if (len > kInlineMax) heavy_chunks += (uint64_t)((len + kChunk - 1) / kChunk);
     }
     const int64_t Epad = pos + kRowAlign;
-    sim->E = E; sim->Epad = Epad;
+    sim->E = E_own; sim->Epad = Epad;
     std::vector<uint32_t> tr((size_t)Epad, 0u);
     std::vector<uint8_t> dl((size_t)Epad, 1);
     std::vector<float> wf;
@@ -553,13 +574,15 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     if (csr->weight_fp16) wh.assign((size_t)Epad, __float2half(0.0f)); else wf.assign((size_t)Epad, 0.0f);
     for (int64_t j = 0; j < N; ++j) {
         int64_t o = row_begin[(size_t)j];
-        for (int64_t s = csr->row_ptr[j]; s < csr->row_ptr[j + 1]; ++s, ++o) {
+        for (int64_t s = csr->row_ptr[j]; s < csr->row_ptr[j + 1]; ++s) {
             if (csr->tgt[s] < 0 || csr->tgt[s] >= N) return bail(fail(sim, DB_EINVAL, "target out of range"));
             if (csr->rec[s] > 3) return bail(fail(sim, DB_EINVAL, "receptor out of range"));
             if (csr->delay[s] < 1 || csr->delay[s] >= sp->D) return bail(fail(sim, DB_EINVAL, "delay must satisfy 1 <= delay < D"));
-            tr[(size_t)o] = ((uint32_t)csr->rec[s] << 30) | (uint32_t)csr->tgt[s];
+            if (csr->tgt[s] < own0 || csr->tgt[s] >= own1) continue;
+            tr[(size_t)o] = ((uint32_t)csr->rec[s] << 30) | (uint32_t)(csr->tgt[s] - own0);      // targets are local
             dl[(size_t)o] = csr->delay[s];
             if (csr->weight_fp16) wh[(size_t)o] = __float2half_rn(csr->w[s]); else wf[(size_t)o] = csr->w[s];
+            ++o;
         }
     }
     int64_t* rb_dev; int32_t* rl_dev; uint32_t* tr_dev; uint8_t* dl_dev; void* w_dev;
@@ -577,7 +600,7 @@ int32_t db_create_from_csr(const db_sim_params* sp, const db_csr_view* csr, cons
     if (up(rb_dev, row_begin.data(), (size_t)N * 8) != cudaSuccess || up(rl_dev, row_len.data(), (size_t)N * 4) != cudaSuccess ||
         up(tr_dev, tr.data(), (size_t)Epad * 4) != cudaSuccess || up(dl_dev, dl.data(), (size_t)Epad) != cudaSuccess ||
         up(w_dev, csr->weight_fp16 ? (const void*)wh.data() : (const void*)wf.data(), wbytes) != cudaSuccess ||
-        up(sim->ntype_dev, csr->ntype, (size_t)N) != cudaSuccess || cudaStreamSynchronize(sim->stream) != cudaSuccess)
+        up(sim->ntype_dev, csr->ntype + own0, (size_t)(own1 - own0)) != cudaSuccess || cudaStreamSynchronize(sim->stream) != cudaSuccess)
         return bail(fail(sim, DB_ECUDA, std::string("CSR upload: ") + cudaGetErrorString(cudaGetLastError())));
     d.row_begin = rb_dev; d.row_len = rl_dev; d.tgt_rec = tr_dev; d.delay = dl_dev; d.w = w_dev;
     d.w_fp16 = csr->weight_fp16 ? 1 : 0;
@@ -603,7 +626,10 @@ int32_t db_create(const db_network_spec* spec, uint64_t seed, db_sim** out) {
     int32_t max_delay = spec->delay_intra_max;
     if (tabs.K_inter > 0) max_delay = std::max(max_delay, spec->delay_inter_max);
     if (max_delay >= spec->sim.D) return bail(fail(sim, DB_EINVAL, "delays must be < D"));
-    if ((rc = setup_common(sim, &spec->sim, spec->N, spec->n_regions, tabs.region_start.data(), max_delay))) return bail(rc);
+    if (spec->own_count != 0 && spec->mode != DB_MODE_FIXED_INDEGREE)
+        return bail(fail(sim, DB_EINVAL, "a handle that owns part of the network needs DB_MODE_FIXED_INDEGREE (synapses are drawn per target)"));
+    if ((rc = setup_common(sim, &spec->sim, spec->N, spec->n_regions, tabs.region_start.data(), max_delay, spec->own_first, spec->own_count))) return bail(rc);
+    sim->min_delay = tabs.K_inter > 0 ? std::min(spec->delay_intra_min, spec->delay_inter_min) : spec->delay_intra_min;
 
     GenAlloc ga;
     ga.user = sim;
@@ -686,6 +712,33 @@ static int32_t step_batch(db_sim* sim, uint32_t n_steps) {
         CK(launch_update(sim->dev, sim->update_sm, 3, sim->stream));
         sim->launches += 1;
     }
+    return DB_OK;
+}
+
+int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n) {
+    if (!sim || (n && !ids)) return DB_EINVAL;
+    if (n == 0) return DB_OK;
+    CK(cudaSetDevice(sim->device));
+    const SimDev& d = sim->dev;
+    if (n > 0xFFFFFFFFull) return fail(sim, DB_EINVAL, "too many ids");
+    for (uint64_t k = 0; k < n; ++k) {
+        if (ids[k] < 0 || ids[k] >= d.n_rows) return fail(sim, DB_EINVAL, "id out of range");
+        if (ids[k] >= d.id0 && ids[k] < d.id0 + d.N) return fail(sim, DB_EINVAL, "id is owned by this handle: its spikes are delivered by db_step");
+    }
+    // the earliest arrival (end of the spike's time bin + smallest delay) must not be consumed yet
+    const uint64_t b = (uint64_t)d.bin_steps, nt = step - step % b + (b - 1);
+    if (nt + (uint64_t)sim->min_delay < sim->host_step) return fail(sim, DB_ERANGE, "too late: the handle has stepped past the arrival of these spikes");
+    if (nt + (uint64_t)sim->max_delay >= sim->host_step + (uint64_t)d.D - 2) return fail(sim, DB_ERANGE, "too early: the arrivals lie beyond the ring");
+    if (n > sim->ext_ids_cap) {
+        const uint64_t cap = std::max<uint64_t>(next_pow2(n), 4096);
+        int32_t* buf = static_cast<int32_t*>(dev_alloc(sim, (size_t)cap * 4));     // (the old one is freed with the handle)
+        if (!buf) return fail(sim, DB_ENOMEM, "device allocation for the external spike list failed");
+        sim->ext_ids_dev = buf; sim->ext_ids_cap = cap;
+    }
+    CK(cudaMemcpyAsync(sim->ext_ids_dev, ids, (size_t)n * 4, cudaMemcpyHostToDevice, sim->stream));
+    CK(cudaStreamSynchronize(sim->stream));            // `ids` is the caller's pageable memory
+    CK(launch_deliver_external(d, sim->n_sm, sim->ext_ids_dev, (unsigned)n, (unsigned long long)step, sim->stream));
+    sim->launches += 1;
     return DB_OK;
 }
 
@@ -835,7 +888,9 @@ int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint
 int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, void* dst) {
     if (!sim || !dst) return DB_EINVAL;
     const SimDev& d = sim->dev;
-    if (first < 0 || count < 0 || first + count > d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds");
+    if (first < d.id0 || count < 0 || first + count > (int64_t)d.id0 + d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds (ids are global; this handle owns [own_first, own_first + own_count))");
+    const int64_t first_global = first;
+    first -= d.id0;                                    // state and ring are indexed locally
     CK(cudaStreamSynchronize(sim->stream));
     if (count == 0) return DB_OK;
     const size_t Np = (size_t)d.Npad;
@@ -854,7 +909,7 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
         break;
     }
     case DB_FIELD_OUTDEG:
-        CK(cudaMemcpy(dst, d.row_len + first, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;
+        CK(cudaMemcpy(dst, d.row_len + first_global, (size_t)count * 4, cudaMemcpyDeviceToHost)); break;   // rows are keyed by global id
     case DB_FIELD_IOU:
         if (d.ou_on) CK(cudaMemcpy(dst, d.Iou + first, (size_t)count * 4, cudaMemcpyDeviceToHost));
         else std::memset(dst, 0, (size_t)count * 4);
@@ -906,7 +961,8 @@ int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count,
 int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, const void* src) {
     if (!sim || !src) return DB_EINVAL;
     const SimDev& d = sim->dev;
-    if (first < 0 || count < 0 || first + count > d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds");
+    if (first < d.id0 || count < 0 || first + count > (int64_t)d.id0 + d.N) return fail(sim, DB_ERANGE, "neuron range out of bounds (ids are global; this handle owns [own_first, own_first + own_count))");
+    first -= d.id0;
     CK(cudaStreamSynchronize(sim->stream));
     if (count == 0) return DB_OK;
     const size_t Np = (size_t)d.Npad;
@@ -1030,6 +1086,7 @@ int32_t db_export_csr(db_sim* sim, db_csr_host* out) {
     if (!sim || !out) return DB_EINVAL;
     std::memset(out, 0, sizeof(*out));
     const SimDev& d = sim->dev;
+    if (d.N != d.n_rows) return fail(sim, DB_ESTATE, "this handle owns part of the network: export the network from a handle that owns all of it");
     CK(cudaStreamSynchronize(sim->stream));
     const int64_t N = d.N;
     std::vector<int64_t> rb((size_t)N);

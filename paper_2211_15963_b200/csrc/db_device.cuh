@@ -55,7 +55,8 @@ static_assert(sizeof(Ctl) == 256, "Ctl layout");
 constexpr int kBgParts = 1024;       // background-event counter is spread over this many cells
 
 struct SimDev {                      // passed by value to every kernel
-    int32_t N, Npad;
+    int32_t N, Npad;                 // neurons this handle owns (state, ring, targets are indexed 0 .. N - 1)
+    int32_t id0, n_rows;             // global id of its first neuron (a multiple of 1024), neurons of the whole network = CSR rows
     int32_t D, S;
     float scale;                     // 2^-S
     float wscale;                    // 2^S

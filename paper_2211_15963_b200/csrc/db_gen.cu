@@ -208,6 +208,7 @@ bool gen_host_tables(const db_network_spec& sp, uint64_t seed, GenHostTables* ou
 // ---------------------------------------------------------------------------
 struct GenDev {
     int32_t N, R, K, K_intra, K_inter;
+    int32_t own0, ownN;            // the targets this handle owns: [own0, own0 + ownN) (the whole network: 0, N)
     uint32_t seed_lo, seed_hi;
     const int32_t* region_start;   // [R + 1]
     const int32_t* region_nexc;    // [R]
@@ -260,11 +261,12 @@ __device__ __forceinline__ void emit_synapse(const GenDev& g, uint64_t owner, ui
     (void)src;
 }
 
-__global__ void k_gen_types(const __grid_constant__ GenDev g, uint8_t* ntype) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.N) return;
+__global__ void k_gen_types(const __grid_constant__ GenDev g, uint8_t* ntype) {       // ntype[] is local: the owned neurons
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= g.ownN) return;
+    const int i = g.own0 + l;
     const int r = gen_region_of(g, i);
-    ntype[i] = (uint8_t)((i - g.region_start[r]) >= g.region_nexc[r]);
+    ntype[l] = (uint8_t)((i - g.region_start[r]) >= g.region_nexc[r]);
 }
 
 // Mode 0, one warp per target neuron i.  kFill = false: count out-degrees of
@@ -273,7 +275,8 @@ template <bool kFill>
 __global__ void __launch_bounds__(256) k_gen_indegree(const __grid_constant__ GenDev g) {
     const unsigned lane = threadIdx.x & 31u;
     const long long n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < g.N; i += n_warps) {
+    // (a handle that owns part of the network draws the inputs of ITS neurons only: the same draws, keyed by the global id)
+    for (long long i = g.own0 + (((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); i < g.own0 + g.ownN; i += n_warps) {
         int r = 0;
         uint4 key_in = make_uint4(0, 0, 0, 0), key_out = key_in;
         if (lane == 0) {
@@ -307,7 +310,7 @@ __global__ void __launch_bounds__(256) k_gen_indegree(const __grid_constant__ Ge
                 atomicAdd(g.row_len + src, 1);
             } else {
                 const int64_t pos = __ldg(g.row_begin + src) + atomicAdd(g.cursor + src, 1);
-                emit_synapse(g, (uint64_t)i, (uint64_t)k, src, (int)i, inh, inter, pos);
+                emit_synapse(g, (uint64_t)i, (uint64_t)k, src, (int)i - g.own0, inh, inter, pos);      // targets are stored locally
             }
         }
     }
@@ -355,6 +358,7 @@ cudaError_t generate_network(const db_network_spec& sp, uint64_t seed, const Gen
 #define GCK(x) do { e = (x); if (e != cudaSuccess) { *err = #x; return e; } } while (0)
 
     GenDev g{};
+    g.own0 = sp.own_count ? (int32_t)sp.own_first : 0; g.ownN = sp.own_count ? (int32_t)sp.own_count : (int32_t)N;
     g.N = (int32_t)N; g.R = R; g.K = sp.K; g.K_intra = tabs.K_intra; g.K_inter = tabs.K_inter;
     g.seed_lo = (uint32_t)seed; g.seed_hi = (uint32_t)(seed >> 32);
     g.inh_mult = (float)sp.inh_mult;
@@ -392,7 +396,7 @@ cudaError_t generate_network(const db_network_spec& sp, uint64_t seed, const Gen
     GCK(cudaMemsetAsync(cursor, 0, (size_t)N * 4, st));
     g.row_len = row_len; g.cursor = cursor; g.row_begin = row_begin;
 
-    k_gen_types<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(g, ntype_dev);
+    k_gen_types<<<(unsigned)((g.ownN + 255) / 256), 256, 0, st>>>(g, ntype_dev);
     GCK(cudaGetLastError());
 
     const unsigned warp_grid = (unsigned)std::min<int64_t>((N + 7) / 8, 148 * 64);

@@ -18,6 +18,7 @@ cudaError_t launch_deliver(const SimDev& p, int grid, unsigned parity, cudaStrea
 // (synapse - s0); add the records waiting in the arrival lists to a DB_FIELD_RING read-out
 cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t row1, int64_t s0, uint32_t* tgt_out, void* w_out,
                              uint8_t* delay_out, uint32_t* seg, cudaStream_t st);
+cudaError_t launch_deliver_external(const SimDev& p, int n_sm, const int32_t* ids_dev, unsigned n_ids, unsigned long long step, cudaStream_t st);
 cudaError_t launch_delay_hist(const uint8_t* delay, int64_t n, unsigned long long* hist /*[256], zeroed*/, int n_sm, cudaStream_t st);
 cudaError_t launch_lists_to_ring(const SimDev& p, int n_sm, int32_t* out, int first, int count, int D_api, cudaStream_t st);
 cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);

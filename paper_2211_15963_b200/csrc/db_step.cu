@@ -484,13 +484,13 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
     // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
     uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
     if (kB && (!kOU || p.bg_on))       // (with the OU drive the Poisson background is usually off: no draw then)
-        rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
+        rnd = philox4x32_10_rk(make_uint4((uint32_t)(grp + (p.id0 >> 2)), kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
     float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     float4 rnd_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     const bool ou = kOU && kA;
     if (ou) {                          // OU current of the four neurons and their N(0,1) draws (quantile table, top 16 bits of
         iou = ld_cg_f4(p.Iou + i0);    // a Philox word each); gathered here so that the latency hides behind the staged copies
-        const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
+        const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)(grp + (p.id0 >> 2)), kStreamOU << 24, (uint32_t)nA, (uint32_t)(nA >> 32)), p.rk);
         rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
                              __ldg(p.ntab + (wo.w >> 16)));
     }
@@ -523,8 +523,8 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
-            len[q] = __ldg(p.row_len + i0 + q);
-            rb[q] = __ldg(p.row_begin + i0 + q);
+            len[q] = __ldg(p.row_len + p.id0 + i0 + q);      // rows are keyed by the global id of the source
+            rb[q] = __ldg(p.row_begin + p.id0 + i0 + q);
             my_events += (unsigned)len[q];
         }
     const unsigned my_spk = (unsigned)__popc(spike_bits);
@@ -558,7 +558,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
-            const int i = i0 + q;
+            const int i = p.id0 + i0 + q;                   // the raster, the regions and the rows use global ids
             if (staged) bs->spk[par][at++] = i;
             else {
                 p.spike_ids[pos & p.spike_mask] = i;
@@ -584,7 +584,7 @@ __device__ __forceinline__ void run_task(const SimDev& p, const TypeSmem* s_tc, 
                 if (lane == 0) at = atomicAdd(&bs->heavy_n[nlo & 1u], 1u);
                 at = __shfl_sync(0xffffffffu, at, 0);
                 if (at < (unsigned)kHeavyListCap) {
-                    if (lane == 0) bs->heavy_row[nlo & 1u][at] = (task * 32 + src) * 4 + q;
+                    if (lane == 0) bs->heavy_row[nlo & 1u][at] = p.id0 + (task * 32 + src) * 4 + q;
                     continue;
                 }
             }
@@ -805,7 +805,7 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
-            len[q] = __ldg(p.row_len + i0 + q);
+            len[q] = __ldg(p.row_len + p.id0 + i0 + q);
             my_events += (unsigned)len[q];
             my_work += (unsigned)((len[q] + kChunk - 1) / kChunk);
         }
@@ -832,7 +832,7 @@ __device__ __noinline__ void emit_global(const SimDev& p, const unsigned long lo
 #pragma unroll
     for (int q = 0; q < 4; ++q)
         if (spike_bits & (1u << q)) {
-            const int i = i0 + q;
+            const int i = p.id0 + i0 + q;                   // global id
             p.spike_ids[spk_pos & p.spike_mask] = i;
             p.spike_tag[spk_pos & p.spike_mask] = (uint32_t)n;
             ++spk_pos;
@@ -898,12 +898,12 @@ __global__ void __launch_bounds__(kRunThreads, 1) k_update_stream(const __grid_c
         const int i0 = grp * 4;
         // one Philox block serves the four neurons (word q -> neuron i0 + q); drawn while the copies fly
         uint4 rnd = make_uint4(0u, 0u, 0u, 0u);
-        if (kB && (!kOU || p.bg_on)) rnd = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
+        if (kB && (!kOU || p.bg_on)) rnd = philox4x32_10_rk(make_uint4((uint32_t)(grp + (p.id0 >> 2)), kStreamBG << 24, (uint32_t)nB, (uint32_t)(nB >> 32)), p.rk);
         float4 iou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         float4 rnd_ou = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (kOU && kA) {
             iou = ld_cg_f4(p.Iou + i0);
-            const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)grp, kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
+            const uint4 wo = philox4x32_10_rk(make_uint4((uint32_t)(grp + (p.id0 >> 2)), kStreamOU << 24, (uint32_t)n, (uint32_t)(n >> 32)), p.rk);
             rnd_ou = make_float4(__ldg(p.ntab + (wo.x >> 16)), __ldg(p.ntab + (wo.y >> 16)), __ldg(p.ntab + (wo.z >> 16)),
                                  __ldg(p.ntab + (wo.w >> 16)));
         }
@@ -953,7 +953,7 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
     if (i >= p.Npad) return;
     const int tp = (i < p.N) ? ntype[i] : 0;
     const TypeConst& c = p.tc[tp];
-    const uint4 r = philox4x32_10(make_uint4((uint32_t)i, kStreamV0 << 24, 0u, 0u), p.seed_lo, p.seed_hi);
+    const uint4 r = philox4x32_10(make_uint4((uint32_t)(i + p.id0), kStreamV0 << 24, 0u, 0u), p.seed_lo, p.seed_hi);   // keyed by the global id
     const float U = __fmul_rn(__uint2float_rn(r.x >> 8), 5.9604644775390625e-08f);
     p.V[i] = (i < p.N) ? __fadd_rn(c.Vreset, __fmul_rn(__fsub_rn(c.Vth, c.Vreset), U)) : 0.0f;
     for (int u = 0; u < 4; ++u) p.g[(size_t)u * p.Npad + i] = 0.0f;
@@ -963,7 +963,7 @@ __global__ void k_init_state(const __grid_constant__ SimDev p, const uint8_t* __
         float v = 0.0f;
         if (i < p.N) {
             v = c.Iext;
-            if (c.ix_on) v = __fadd_rn(v, iext_tab[(size_t)tp * 65536u + (philox4x32_10(make_uint4((uint32_t)i, kStreamIEXT << 24, 0u, 0u), p.seed_lo, p.seed_hi).x >> 16)]);
+            if (c.ix_on) v = __fadd_rn(v, iext_tab[(size_t)tp * 65536u + (philox4x32_10(make_uint4((uint32_t)(i + p.id0), kStreamIEXT << 24, 0u, 0u), p.seed_lo, p.seed_hi).x >> 16)]);
         }
         p.iext[i] = v;
     }
@@ -1374,6 +1374,28 @@ __global__ void __launch_bounds__(256) k_lists_to_ring(const __grid_constant__ S
     }
 }
 
+// f3 (SI Eq.(6) second sum): a handle that owns the targets [id0, id0 + N) holds, for
+// EVERY source neuron of the network, the synapses onto its own targets (the paper's layout).  The
+// spikes of the neurons it does not own arrive from outside as a list of global ids that fired in step `step`; one warp
+// per (spike, 512-synapse chunk) pushes the row into the ring, exactly as k_deliver does for the handle's own spikes.
+template <bool kHalf>
+__global__ void __launch_bounds__(256) k_deliver_external(const __grid_constant__ SimDev p, const int32_t* __restrict__ ids,
+                                                          const unsigned n_ids, const unsigned long long step) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
+    const unsigned nto = (unsigned)transfer_step(p, step);
+    unsigned long long ev = 0ull;
+    for (unsigned q = warp; q < n_ids; q += n_warps) {
+        const int j = __ldg(ids + q);
+        const int64_t rb = __ldg(p.row_begin + j);
+        const int len = __ldg(p.row_len + j);
+        deliver_span<kHalf>(p, nto, rb, len, lane);
+        ev += (unsigned long long)len;
+    }
+    if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
+}
+
 // ---------------------------------------------------------------------------
 // host-side launchers (called from db_api.cu)
 // ---------------------------------------------------------------------------
@@ -1431,6 +1453,14 @@ cudaError_t launch_sort_rows(const SimDev& p, int n_sm, int64_t row0, int64_t ro
     if (grid <= 0) return cudaSuccess;
     if (p.w_fp16) k_sort_rows<true><<<grid, kSortWarps * 32, 0, st>>>(p, row0, row1, s0, tgt_out, w_out, delay_out, seg);
     else          k_sort_rows<false><<<grid, kSortWarps * 32, 0, st>>>(p, row0, row1, s0, tgt_out, w_out, delay_out, seg);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_deliver_external(const SimDev& p, int n_sm, const int32_t* ids_dev, unsigned n_ids, unsigned long long step, cudaStream_t st) {
+    const int grid = (int)std::min<unsigned>((n_ids + 7u) / 8u, (unsigned)n_sm * 8u);
+    if (grid <= 0) return cudaSuccess;
+    if (p.w_fp16) k_deliver_external<true><<<grid, 256, 0, st>>>(p, ids_dev, n_ids, step);
+    else          k_deliver_external<false><<<grid, 256, 0, st>>>(p, ids_dev, n_ids, step);
     return cudaGetLastError();
 }
 

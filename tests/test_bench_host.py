@@ -116,3 +116,56 @@ def test_ncu_traffic_is_tied_to_the_kernel_sources():
     v, why = bench._ncu_traffic("no such kernel")
     assert v is None and isinstance(why, str)
     assert len(bench._csrc_sha16()) == 16
+
+
+_SHARD_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import numpy as np, torch, torch.distributed as dist
+from paper_2211_15963_b200 import sharded
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%%s" %% os.environ["PORT"], rank=int(os.environ["RANK"]), world_size=2)
+rank = dist.get_rank()
+
+class FakeSim:                       # stands in for the CUDA handle: the exchange is host logic
+    def __init__(self):
+        self.got, self.steps = [], 0
+    def db_get_counters(self):
+        return {"steps": self.steps}
+    def db_step(self, k):
+        self.steps += k
+    def db_read_spikes(self, a, b):  # rank r fires neuron 1000 r + step in every step, twice in step 7 for rank 1
+        st = np.arange(a, b, dtype=np.uint64)
+        ids = (1000 * rank + st).astype(np.int32)
+        if rank == 1 and a <= 7 < b:
+            st, ids = np.append(st, np.uint64(7)), np.append(ids, np.int32(1999))
+        return st, ids
+    def db_deliver_external(self, step, ids):
+        self.got.append((int(step), [int(x) for x in ids]))
+
+sim = FakeSim()
+sharded.run(dist, torch, sim, 10, 4)
+print(json.dumps({"rank": rank, "got": sim.got, "own": [sharded.own_range(5000, r, 2) for r in range(2)]}))
+dist.barrier()
+dist.destroy_process_group()
+""" % ROOT
+
+
+def test_sharded_exchange_over_two_ranks_gloo():
+    # the host side of the region-sharded path (SURVEY 8(e)): all-gather of the variable-length spike lists every d_min
+    # steps, delivery of the OTHER ranks' spikes step by step; world_size 2 on the CPU (gloo)
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    procs = [subprocess.Popen([sys.executable, "-c", _SHARD_WORKER], cwd=ROOT, text=True, stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, env=dict(os.environ, RANK=str(r), PORT=str(port)))
+             for r in range(2)]
+    outs = [p.communicate(timeout=300) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e
+    res = {json.loads(o.strip().splitlines()[-1])["rank"]: json.loads(o.strip().splitlines()[-1]) for o, _ in outs}
+    assert res[0]["own"] == [[0, 3072], [3072, 1928]]
+    want0 = [(s, [1000 + s] + ([1999] if s == 7 else [])) for s in range(10)]        # rank 0 receives rank 1's spikes
+    want1 = [(s, [s]) for s in range(10)]
+    assert [(s, sorted(i)) for s, i in res[0]["got"]] == [(s, sorted(i)) for s, i in want0]
+    assert [(s, i) for s, i in res[1]["got"]] == want1

@@ -242,3 +242,82 @@ def test_per_neuron_external_current_from_a_gamma_law(db, oracle_mod, mode):
     with pytest.raises(db.DbError) as e:
         h.db_write_state(db.FIELD_IEXT, Io)
     assert e.value.code == db.binding.DB_ESTATE
+
+
+def _run_shards(db, shards, bounds, steps, every):
+    """Step the handles `shards` (owning [bounds[k], bounds[k + 1])) together: every `every` steps each one's new spikes go
+    to all the others (db_read_spikes -> db_deliver_external, step by step).  Returns the merged raster."""
+    done, all_st, all_id = 0, [], []
+    while done < steps:
+        n = min(every, steps - done)
+        for s in shards:
+            s.db_step(n)
+        fresh = [s.db_read_spikes(done, done + n) for s in shards]
+        for k, dst in enumerate(shards):
+            for j, (st, ids) in enumerate(fresh):
+                if j == k:
+                    continue
+                for step in np.unique(st):
+                    dst.db_deliver_external(int(step), ids[st == step])
+        for st, ids in fresh:
+            all_st.append(st); all_id.append(ids)
+        done += n
+    st, ids = np.concatenate(all_st), np.concatenate(all_id)
+    order = np.lexsort((ids, st))
+    return st[order], ids[order]
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("source", ["csr", "generator"])
+def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, oracle_mod, mode, source):
+    # SURVEY 8(f) row 3, the half that one GPU can test (SI Eq.(6) P:L498-503; layout P:L494): each handle owns a range of
+    # targets -- state, ring and the synapses onto them from EVERY source -- and receives the other's spikes as id lists
+    # every d_min steps.  Raster, state, ring and counters must be those of the oracle's single whole network, bit for bit.
+    cfg = db_inputs.config(2, scale=0.004)                       # 20,000 neurons in regions, K = 160 + 40, inter delays 20..200
+    cfg["net"].update(n_regions=8, delay_intra_min=3, delay_inter_min=20)
+    t = db_inputs.type_params(bg_weight=0.02)
+    t.update(G=[0.5, 0.125, 0.5, 0.5], ou_mu=0.3, ou_sigma=0.1, ou_tau_ms=10.0)       # Poisson and OU draws: both keyed by global id
+    cfg["sim"]["types"] = [t, dict(t)]
+    N = cfg["net"]["N"]
+    net = oracle_mod.generate(cfg["net"], db_inputs.GEN_SEED)
+    o = oracle_mod.OracleSim(cfg["sim"], net, db_inputs.DYN_SEED)
+    cut = 9 * 1024                                               # not a region boundary, not half
+    bounds = [0, cut, N]
+    if source == "csr":
+        shards = [db.Sim.db_create_from_csr(cfg["sim"], net, exec_mode=mode, own=(bounds[k], bounds[k + 1] - bounds[k])) for k in range(2)]
+    else:
+        shards = [db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, exec_mode=mode,
+                                   own=(bounds[k], bounds[k + 1] - bounds[k])) for k in range(2)]
+    Vo = o.state()[0].astype(np.float32)
+    for k, s in enumerate(shards):
+        assert np.array_equal(s.db_read_state(db.FIELD_V), Vo[bounds[k]:bounds[k + 1]])          # V0 keyed by global id
+        assert np.array_equal(s.db_read_state(db.FIELD_TYPE), net["ntype"][bounds[k]:bounds[k + 1]])
+    steps, d_min = 300, 3
+    st, ids = _run_shards(db, shards, bounds, steps, d_min)
+    o.step(steps)
+    so, io = o.spikes()
+    order = np.lexsort((io, so))
+    assert np.array_equal(st, so[order]) and np.array_equal(ids, io[order]) and len(ids) > 500
+    assert np.count_nonzero(ids < cut) > 100 and np.count_nonzero(ids >= cut) > 100
+    Vo, go, ro = o.state()
+    ring = o.ring()
+    for k, s in enumerate(shards):
+        a, b = bounds[k], bounds[k + 1]
+        Vg, gg, rg = s.state()
+        assert np.array_equal(Vg, Vo[a:b].astype(np.float32)) and np.array_equal(gg, go[a:b].astype(np.float32)) and np.array_equal(rg, ro[a:b])
+        assert np.array_equal(s.db_read_state(db.FIELD_RING), ring[:, a:b, :])
+        assert np.array_equal(s.db_read_state(db.FIELD_IOU), o.iou()[a:b].astype(np.float32))
+    cs = [s.db_get_counters() for s in shards]
+    co = o.counters()
+    assert sum(c["events"] for c in cs) == co["events"] and sum(c["spikes"] for c in cs) == co["spikes"]
+    assert sum(c["bg_events"] for c in cs) == co["bg_events"]
+    # argument checks: an owned id, an id out of range, a spike whose arrivals are already in the past
+    with pytest.raises(db.DbError):
+        shards[0].db_deliver_external(steps - 1, np.array([5], np.int32))
+    with pytest.raises(db.DbError):
+        shards[0].db_deliver_external(steps - 1, np.array([N], np.int32))
+    with pytest.raises(db.DbError) as e:
+        shards[0].db_deliver_external(steps - 10, np.array([cut + 1], np.int32))
+    assert e.value.code == db.binding.DB_ERANGE
+    with pytest.raises(db.DbError):
+        shards[1].db_read_state(db.FIELD_V, first=0, count=10)       # not its neurons
