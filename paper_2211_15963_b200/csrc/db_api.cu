@@ -323,24 +323,25 @@ int32_t build_arrival_lists(db_sim* sim, bool* ok) {
     // target windows: one ring slot (16 B per neuron) is swept window by window, each window small enough to stay in L2
     int W = 1;
     while (W < 4 && 16.0 * (double)d.Npad / W > 48.0 * 1048576.0) W *= 2;
-    // parallel lists per (slot, window): atomics on one cursor serialise in L2 (~90 ns each, profiles/), so the records
-    // of a step are spread over enough cursors that each sees a few dozen reservations per step
-    const double ev_step = (e_near + e_far) * 30.0 * sim->params.dt_ms * 1e-3;      // records per step at 30 Hz
-    int P = 8;
-    while (P < 256 && ev_step / (W * P) > 16384.0) P *= 2;
+    // one list per (slot, window) and BLOCK of the delivery kernel: a block appends to its own lists through cursors in
+    // its shared memory (no global atomics) and reduces them itself when their step comes
+    const int P = sim->n_sm * 4;                       // k_deliver_lists: four blocks of 256 threads per SM, all resident
     const int64_t win = ((((int64_t)d.Npad + W - 1) / W + kNeuronPad - 1) / kNeuronPad) * kNeuronPad;
+    const uint64_t cur_near = (uint64_t)Dn * W, cur_far = e_far > 0 ? (uint64_t)d.D * W : 0;
+    if (cur_near + cur_far > 8192) return DB_OK;       // (cursors of a block live in its shared memory)
     // capacity: the records of one step at the design rate, split over the lists of a slot; any excess spills into the
     // dense ring (exact, only slower).  Halve the design rate until the lists fit into half of the free memory.
     size_t free_b = 0, total_b = 0;
     CK(cudaMemGetInfo(&free_b, &total_b));
     const double dt_s = sim->params.dt_ms * 1e-3;
-    uint64_t cap_near = 0, cap_far = 0, n_near = (uint64_t)Dn * W * P, n_far = e_far > 0 ? (uint64_t)d.D * W * P : 0;
+    uint64_t cap_near = 0, cap_far = 0;
+    const uint64_t n_near = cur_near * (uint64_t)P, n_far = cur_far * (uint64_t)P;
     double rate = 60.0;
     for (;; rate *= 0.5) {
         if (rate < 4.0) return DB_OK;                              // no room for useful lists
         auto cap_of = [&](double synapses) {
             const double per_list = synapses * rate * dt_s / (double)(W * P);
-            return (uint64_t)std::max(1024.0, std::ceil(per_list / 16.0) * 16.0);
+            return (uint64_t)std::max(256.0, std::ceil(per_list / 16.0) * 16.0);
         };
         cap_near = cap_of(e_near);
         cap_far = n_far ? cap_of(e_far) : 0;
@@ -352,9 +353,9 @@ int32_t build_arrival_lists(db_sim* sim, bool* ok) {
     const size_t n_rec = (size_t)(n_near * cap_near + n_far * cap_far);
     rec = static_cast<uint2*>(dev_alloc(sim, n_rec * sizeof(uint2)));
     if (!rec) return DB_OK;                                        // fall back rather than fail
-    if ((rc = alloc_zero(sim, &cnt, (size_t)(n_near + n_far) * 8))) return rc;
+    if ((rc = alloc_zero(sim, &cnt, (size_t)(cur_near + cur_far) * (size_t)P))) return rc;
     d.ev_direct = 1; d.ev_near_lim = near_lim; d.ev_near_d = std::max(near_lim - (d.bin_steps - 1), 0); d.ev_Dn = Dn; d.ev_D = d.D; d.ev_W = W; d.ev_P = P;
-    d.ev_n_near = (int32_t)n_near; d.ev_n_far = (int32_t)n_far;
+    d.ev_n_cur = (int32_t)(cur_near + cur_far); d.ev_n_far = (int32_t)n_far;
     d.ev_cap_near = (uint32_t)cap_near; d.ev_cap_far = (uint32_t)cap_far;
     for (int k = 0; k < 3; ++k) d.ev_wb[k] = (k + 1 < W) ? (uint32_t)std::min<int64_t>((int64_t)(k + 1) * win, 0x7FFFFFFF) : 0xFFFFFFFFu;
     d.ev_rec = rec; d.ev_cnt = cnt;

@@ -81,8 +81,10 @@ struct SimDev {                      // passed by value to every kernel
     const uint8_t* delay;            // [Epad]
     int32_t w_fp16;
     // DB_EXEC_KERNELS_DEFERRED: arrival lists (db_step.cu).  8-byte records (receptor << 30 | target, fixed-point weight)
-    // waiting for their arrival step; list ((slot * ev_W + window) * ev_P + part), near family first, cursor of list l
-    // at ev_cnt[8 l] (one per 32-byte sector)
+    // waiting for their arrival step.  Lists are private to the blocks of the delivery kernel: block b owns one list per
+    // cursor index c = slot * ev_W + window (near family: slot = arrival & (ev_Dn - 1); far family after it: slot = arrival
+    // & (ev_D - 1)); its records start at ev_rec[(c * ev_P + b) * capacity] and its cursor is ev_cnt[b * ev_n_cur + c]
+    // between launches (shared memory during one)
     int32_t ev_on;                   // 0: every synapse is pushed into the ring when its neuron fires
     int32_t ev_direct;               // arrivals <= this many steps ahead (1) go straight into the ring
     int32_t ev_near_lim;             // arrivals <= this many steps ahead go to the near family (ring of ev_Dn slots)
@@ -90,8 +92,8 @@ struct SimDev {                      // passed by value to every kernel
     const uint32_t* seg;             // [N][ev_near_d * ev_W + 1] rows sorted by (delay, window): first synapse (relative to the row) of every
                                      // (delay, window) run of the near part; the last entry starts the far part
     int32_t ev_Dn, ev_D;             // slots of the near / far family (powers of two; ev_D = D)
-    int32_t ev_W, ev_P;              // target windows per slot (1, 2 or 4), parallel lists per window (power of two)
-    int32_t ev_n_near, ev_n_far;     // lists per family (ev_n_far = 0: no delay beyond ev_near_lim)
+    int32_t ev_W, ev_P;              // target windows per slot (1, 2 or 4), blocks of the delivery kernel (= lists per cursor index)
+    int32_t ev_n_cur, ev_n_far;      // cursor indices per block (both families); ev_n_far = 0: no delay beyond ev_near_lim
     uint32_t ev_cap_near, ev_cap_far;// records per list
     uint32_t ev_wb[3];               // first neuron of the windows 1, 2, 3 (0xFFFFFFFF when unused)
     uint2* ev_rec;                   // near lists, then far lists

@@ -233,6 +233,15 @@ __device__ __forceinline__ uint4 ld_cg_u4(const uint4* p) {
     asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
 }
+// cache-streaming accesses (evict-first in L2): data that is read or written once and must not push the hot ring window out
+__device__ __forceinline__ uint4 ld_cs_u4(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.cs.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_cs_u2(uint2* p, const uint2 v) {
+    asm volatile("st.global.cs.v2.u32 [%0], {%1,%2};" :: "l"(p), "r"(v.x), "r"(v.y) : "memory");
+}
 __device__ __forceinline__ float4 ld_cg_f4(const float* p) {
     float4 r;
     asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
@@ -1049,30 +1058,30 @@ __global__ void __launch_bounds__(kSortWarps * 32) k_sort_rows(const __grid_cons
     }
 }
 
-// Index of the list that takes a record arriving `ahead` steps after step n (ahead > ev_direct) at target tg, and its
-// capacity.  Lists are numbered near family first: ((slot * W + window) * P + part).
-__device__ __forceinline__ unsigned ev_list_of(const SimDev& p, const unsigned arrival, const unsigned ahead, const unsigned tg,
-                                               const unsigned part) {
+// Lists are private to the blocks of the delivery kernel: block b appends to its own list of every (arrival slot,
+// window) and reduces its own lists when their step comes, so the list cursors live in the block's shared memory during
+// a launch (ev_cnt[b * ev_n_cur + cursor] between launches) and no append needs a global atomic.  Cursor index of the
+// list that takes a record arriving `ahead` steps after step n (ahead > ev_direct) at target tg: near family first.
+__device__ __forceinline__ unsigned ev_cursor_of(const SimDev& p, const unsigned arrival, const unsigned ahead, const unsigned tg) {
     const unsigned w = ev_window(p, tg);
-    if (ahead <= (unsigned)p.ev_near_lim)
-        return (((arrival & (unsigned)(p.ev_Dn - 1)) * (unsigned)p.ev_W + w) * (unsigned)p.ev_P) + part;
-    return (unsigned)p.ev_n_near + (((arrival & (unsigned)(p.ev_D - 1)) * (unsigned)p.ev_W + w) * (unsigned)p.ev_P) + part;
+    if (ahead <= (unsigned)p.ev_near_lim) return (arrival & (unsigned)(p.ev_Dn - 1)) * (unsigned)p.ev_W + w;
+    return (unsigned)(p.ev_Dn * p.ev_W) + (arrival & (unsigned)(p.ev_D - 1)) * (unsigned)p.ev_W + w;
 }
-__device__ __forceinline__ uint2* ev_records(const SimDev& p, const unsigned list) {
-    return list < (unsigned)p.ev_n_near ? p.ev_rec + (size_t)list * p.ev_cap_near
-                                        : p.ev_rec + (size_t)p.ev_n_near * p.ev_cap_near + (size_t)(list - (unsigned)p.ev_n_near) * p.ev_cap_far;
+__device__ __forceinline__ uint2* ev_records(const SimDev& p, const unsigned cur, const unsigned block) {
+    const unsigned n_near = (unsigned)(p.ev_Dn * p.ev_W);
+    return cur < n_near ? p.ev_rec + ((size_t)cur * p.ev_P + block) * p.ev_cap_near
+                        : p.ev_rec + (size_t)n_near * p.ev_P * p.ev_cap_near + ((size_t)(cur - n_near) * p.ev_P + block) * p.ev_cap_far;
 }
-__device__ __forceinline__ unsigned ev_capacity(const SimDev& p, const unsigned list) {
-    return list < (unsigned)p.ev_n_near ? p.ev_cap_near : p.ev_cap_far;
+__device__ __forceinline__ unsigned ev_capacity(const SimDev& p, const unsigned cur) {
+    return cur < (unsigned)(p.ev_Dn * p.ev_W) ? p.ev_cap_near : p.ev_cap_far;
 }
-constexpr int kEvCntStride = 8;      // one list cursor per 32-byte sector
 
 // Turn `len` synapses starting at `rb` into records: the lanes take 32 consecutive synapses per pass, four passes of
 // loads in flight; the lanes of a pass whose records go to the same list (a run of the sorted row) reserve their
 // positions with ONE atomic on the list's cursor.  n = step of the spike, nto = its transfer step (R29).
 template <bool kHalf>
 __device__ __forceinline__ void bin_span(const SimDev& p, const unsigned n_lo, const unsigned nto_lo, const int64_t rb,
-                                         const int len, const unsigned lane, const unsigned part, unsigned& spilled) {
+                                         const int len, const unsigned lane, unsigned* s_cur, unsigned& spilled) {
     const size_t Np = (size_t)p.Npad;
     const unsigned Dm = (unsigned)(p.D - 1);
     const unsigned shift = nto_lo - n_lo;                // steps until the end of the spike's time bin
@@ -1097,10 +1106,10 @@ __device__ __forceinline__ void bin_span(const SimDev& p, const unsigned n_lo, c
             if (base + r * 32 >= len) continue;          // warp-uniform
             const bool valid = base + r * 32 + (int)lane < len;
             const unsigned ahead = shift + dl[r];
-            if (valid && ahead > (unsigned)p.ev_direct) list[r] = ev_list_of(p, nto_lo + dl[r], ahead, tr[r] & 0x3FFFFFFFu, part);
+            if (valid && ahead > (unsigned)p.ev_direct) list[r] = ev_cursor_of(p, nto_lo + dl[r], ahead, tr[r] & 0x3FFFFFFFu);
             peers[r] = __match_any_sync(0xffffffffu, list[r]);
             if (lane == (unsigned)__ffs(peers[r]) - 1u && list[r] != 0xFFFFFFFFu)
-                pos[r] = atomicAdd(p.ev_cnt + (size_t)list[r] * kEvCntStride, (unsigned)__popc(peers[r]));
+                pos[r] = atomicAdd(s_cur + list[r], (unsigned)__popc(peers[r]));      // shared memory: the block's own cursor
         }
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
@@ -1109,7 +1118,7 @@ __device__ __forceinline__ void bin_span(const SimDev& p, const unsigned n_lo, c
             if (base + r * 32 + (int)lane >= len) continue;
             const int wq = __float2int_rn(__fmul_rn(wf[r], p.wscale));
             if (list[r] != 0xFFFFFFFFu && at < ev_capacity(p, list[r])) {
-                ev_records(p, list[r])[at] = make_uint2(tr[r], (unsigned)wq);
+                st_cs_u2(ev_records(p, list[r], blockIdx.x) + at, make_uint2(tr[r], (unsigned)wq));
             } else {                                     // next step's arrivals, or a full list: straight into the ring
                 red_add_s32(p.ring + ((size_t)((nto_lo + dl[r]) & Dm) * 4 + (tr[r] >> 30)) * Np + (tr[r] & 0x3FFFFFFFu), wq);
                 if (list[r] != 0xFFFFFFFFu) ++spilled;
@@ -1126,33 +1135,16 @@ __device__ __forceinline__ void bin_span(const SimDev& p, const unsigned n_lo, c
 constexpr int kEvKeysMax = 128;      // (delay, window) runs of the near part: ev_near_d <= 29 delays x W <= 4 windows
 template <bool kHalf>
 __device__ __forceinline__ void bin_near(const SimDev& p, const unsigned n_lo, const unsigned nto_lo, const int j, const int64_t rb0,
-                                         const int c0, const int c1, const unsigned lane, const unsigned part,
+                                         const int c0, const int c1, const unsigned lane, unsigned* s_cur,
                                          int* tab_off, unsigned* tab_list, unsigned& spilled) {
     const unsigned W = (unsigned)p.ev_W;
     const int K = p.ev_near_d * (int)W;
     const uint32_t* sg = p.seg + (size_t)j * (size_t)(K + 1);
     const unsigned shift = nto_lo - n_lo;
-    for (int q = (int)lane; q < K; q += 32) {
-        const int s0 = max((int)__ldg(sg + q), c0), s1 = min((int)__ldg(sg + q + 1), c1);
-        unsigned list = 0xFFFFFFFFu;
-        int off = 0;
-        if (s1 > s0) {
-            const unsigned d = (unsigned)q / W + 1u, w = (unsigned)q % W;
-            if (shift + d > (unsigned)p.ev_direct) {
-                list = (((nto_lo + d) & (unsigned)(p.ev_Dn - 1)) * W + w) * (unsigned)p.ev_P + part;
-                off = (int)atomicAdd(p.ev_cnt + (size_t)list * kEvCntStride, (unsigned)(s1 - s0)) - s0;
-            }
-        }
-        tab_off[q] = off;
-        tab_list[q] = list;
-    }
-    __syncwarp();
     const size_t Np = (size_t)p.Npad;
     const unsigned Dm = (unsigned)(p.D - 1);
-    constexpr int kRounds = 4;
-    for (int base = c0; base < c1; base += 32 * kRounds) {
-        unsigned tr[kRounds], dl[kRounds];
-        float wf[kRounds];
+    constexpr int kRounds = 4;                           // 128 synapses per batch; two batches in flight
+    auto load = [&](const int base, unsigned (&tr)[kRounds], unsigned (&dl)[kRounds], float (&wf)[kRounds]) {
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
             const int e = base + r * 32 + (int)lane;
@@ -1164,6 +1156,8 @@ __device__ __forceinline__ void bin_near(const SimDev& p, const unsigned n_lo, c
                 else       wf[r] = __ldg(static_cast<const float*>(p.w) + rb0 + e);
             }
         }
+    };
+    auto store = [&](const int base, const unsigned (&tr)[kRounds], const unsigned (&dl)[kRounds], const float (&wf)[kRounds]) {
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
             const int e = base + r * 32 + (int)lane;
@@ -1174,11 +1168,38 @@ __device__ __forceinline__ void bin_near(const SimDev& p, const unsigned n_lo, c
             const unsigned pos = (unsigned)(tab_off[q] + e);
             const int wq = __float2int_rn(__fmul_rn(wf[r], p.wscale));
             if (list != 0xFFFFFFFFu && pos < p.ev_cap_near) {
-                p.ev_rec[(size_t)list * p.ev_cap_near + pos] = make_uint2(tr[r], (unsigned)wq);
+                st_cs_u2(p.ev_rec + ((size_t)list * p.ev_P + blockIdx.x) * p.ev_cap_near + pos, make_uint2(tr[r], (unsigned)wq));
             } else {                                     // a full list, or next step's arrivals: straight into the ring
                 red_add_s32(p.ring + ((size_t)((nto_lo + dl[r]) & Dm) * 4 + (tr[r] >> 30)) * Np + tg, wq);
                 if (list != 0xFFFFFFFFu) ++spilled;
             }
+        }
+    };
+    unsigned trA[kRounds], dlA[kRounds], trB[kRounds], dlB[kRounds];
+    float wfA[kRounds], wfB[kRounds];
+    load(c0, trA, dlA, wfA);                             // on their way while the positions are reserved
+    for (int q = (int)lane; q < K; q += 32) {
+        const int s0 = max((int)__ldg(sg + q), c0), s1 = min((int)__ldg(sg + q + 1), c1);
+        unsigned list = 0xFFFFFFFFu;
+        int off = 0;
+        if (s1 > s0) {
+            const unsigned d = (unsigned)q / W + 1u, w = (unsigned)q % W;
+            if (shift + d > (unsigned)p.ev_direct) {
+                list = ((nto_lo + d) & (unsigned)(p.ev_Dn - 1)) * W + w;              // cursor index (near family)
+                off = (int)atomicAdd(s_cur + list, (unsigned)(s1 - s0)) - s0;
+            }
+        }
+        tab_off[q] = off;
+        tab_list[q] = list;
+    }
+    __syncwarp();
+    for (int base = c0; base < c1; base += 64 * kRounds) {
+        const bool two = base + 32 * kRounds < c1;
+        if (two) load(base + 32 * kRounds, trB, dlB, wfB);
+        store(base, trA, dlA, wfA);
+        if (two) {
+            if (base + 64 * kRounds < c1) load(base + 64 * kRounds, trA, dlA, wfA);
+            store(base + 32 * kRounds, trB, dlB, wfB);
         }
     }
     __syncwarp();
@@ -1204,149 +1225,116 @@ __global__ void __launch_bounds__(256) k_delay_hist(const uint8_t* __restrict__ 
     if (s_h[threadIdx.x]) atomicAdd(hist + threadIdx.x, (unsigned long long)s_h[threadIdx.x]);
 }
 
-constexpr int kEvChunk = 2048;       // records per apply work unit (one block pass: 256 threads x 8)
-constexpr int kEvMaxLists = 2048;    // lists of one arrival step: 2 families x W <= 4 x P <= 256
-constexpr int kEvMapMax = 6144;      // chunks of one arrival step whose list is looked up in a table (else: binary search)
+constexpr int kEvChunk = 2048;       // records per pass of a block over one of its lists (256 threads x 8)
 
 // The delivery kernel of step n in list mode.  It touches nothing the NEXT update kernel (B_n, A_(n+1): reads ring slot
-// n) reads -- ring slot n + 1 and later, the lists, the work list of step n -- so it runs BESIDE that kernel on a second
-// branch of the step graph (db_api.cu) and has to be done before the update kernel after it (B_(n+1)) starts:
-//   1. the records that arrive in step n + 1 (written by the delivery kernels of the earlier steps) are streamed into
-//      ring slot n + 1, window by window: the only slot that takes reductions here;
-//   2. the rows that fired in step n: their synapses that arrive in step n + 1 are reduced into that slot straight from
-//      the CSR, the later ones become records in the lists of their arrival steps.
+// n) reads -- ring slot n + 1 and later, the lists, the work list of step n -- so it sits on a second branch of the step
+// graph (db_api.cu) and has to be done before the update kernel after that one (B_(n+1)) starts.  Every block
+//   1. streams ITS OWN lists of arrival step n + 1 (filled by its earlier launches) into ring slot n + 1, window by
+//      window -- all blocks sweep the windows together, so the reductions of the whole grid stay inside one L2-sized
+//      part of the slot at a time -- and empties them;
+//   2. takes its share of the rows that fired in step n: the synapses that arrive in step n + 1 are reduced into that
+//      slot straight from the CSR, the later ones become records in its lists of their arrival steps.
 // It takes n from the cell the update kernel left for it (Ctl::step moves on meanwhile).
 template <bool kHalf>
-__global__ void __maxnreg__(56) k_deliver_lists(const __grid_constant__ SimDev p, const unsigned parity) {
-    __shared__ unsigned s_count[kEvMaxLists], s_first[kEvMaxLists + 1];
-    __shared__ unsigned short s_map[kEvMapMax];
-    __shared__ unsigned s_warp[8];
+__global__ void __maxnreg__(64) k_deliver_lists(const __grid_constant__ SimDev p, const unsigned parity) {
+    extern __shared__ unsigned s_cur[];              // [ev_n_cur] cursors of this block's lists
     __shared__ int s_tab_off[8][kEvKeysMax];
     __shared__ unsigned s_tab_list[8][kEvKeysMax];
-    __shared__ unsigned s_last;
     const unsigned long long n = p.ctl->work_step[parity];
-    const unsigned long long counts = p.ctl->step_counts[n & 3ull];
-    const unsigned n_work = (unsigned)counts;
+    const unsigned n_work = (unsigned)p.ctl->step_counts[n & 3ull];
     const unsigned lane = threadIdx.x & 31u;
+    unsigned* const g_cur = p.ev_cnt + (size_t)blockIdx.x * p.ev_n_cur;
+    for (unsigned k = threadIdx.x; k < (unsigned)p.ev_n_cur; k += blockDim.x) s_cur[k] = g_cur[k];
+    __syncthreads();
+    // ---- 1. this block's lists of step m = n + 1: (window, family) in window-major order
     const unsigned m = (unsigned)n + (unsigned)p.ev_direct;
-    const unsigned fams = p.ev_n_far ? 2u : 1u, P = (unsigned)p.ev_P;
-    const unsigned n_lists = (unsigned)p.ev_W * fams * P;
-    auto list_of = [&](const unsigned k) {
-        const unsigned part = k % P, fam = (k / P) % fams, w = k / (P * fams);
-        const unsigned slot = fam ? (m & (unsigned)(p.ev_D - 1)) : (m & (unsigned)(p.ev_Dn - 1));
-        return (fam ? (unsigned)p.ev_n_near : 0u) + ((slot * (unsigned)p.ev_W + w) * P) + part;
-    };
-    unsigned spilled = 0u;
-    {
-        // ---- 1. the lists of step m, window-major (so that the blocks sweep the slot window by window): entry k of the
-        // table = (window, family, part); s_first[k] = first 2048-record chunk of list k (block-wide exclusive scan)
-        {
-            const unsigned per = (n_lists + 255u) / 256u, k0 = threadIdx.x * per;
-            unsigned sum = 0u;
-            for (unsigned k = k0; k < min(k0 + per, n_lists); ++k) {
-                const unsigned list = list_of(k);
-                const unsigned c = min(ld_cg_u32(p.ev_cnt + (size_t)list * kEvCntStride), ev_capacity(p, list));
-                s_count[k] = c;
-                s_first[k] = sum;                            // exclusive inside the thread's run
-                sum += (c + kEvChunk - 1u) / kEvChunk;
-            }
-            unsigned inc = sum;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
-                if (lane >= (unsigned)d) inc += o;
-            }
-            if (lane == 31u) s_warp[threadIdx.x >> 5] = inc;
-            __syncthreads();
-            unsigned before = inc - sum;
-            for (unsigned w2 = 0; w2 < (threadIdx.x >> 5); ++w2) before += s_warp[w2];
-            for (unsigned k = k0; k < min(k0 + per, n_lists); ++k) {
-                const unsigned f = s_first[k] + before, nc = (s_count[k] + kEvChunk - 1u) / kEvChunk;
-                s_first[k] = f;
-                for (unsigned c = f; c < min(f + nc, (unsigned)kEvMapMax); ++c) s_map[c] = (unsigned short)k;
-            }
-            if (threadIdx.x == 255u) s_first[n_lists] = before + sum;
-            __syncthreads();
+    const size_t Np = (size_t)p.Npad;
+    int32_t* const ring_slot = p.ring + (size_t)(m & (unsigned)(p.D - 1)) * 4 * Np;
+    const unsigned fams = p.ev_n_far ? 2u : 1u;
+    // The slot is cold: nobody has touched it since it was consumed D steps ago, so the FIRST reduction into each of its
+    // sectors would be a random DRAM read (a third of all reductions at configs 3 / 4: measured, profiles/).  Instead
+    // the blocks stream the window they are about to sweep into L2 with sequential prefetches (one per 128-byte line,
+    // 16 B x window neurons in all), one window ahead of the reductions.
+    auto prefetch_window = [&](const unsigned w) {
+        const unsigned lo = w ? p.ev_wb[w - 1] : 0u;
+        const unsigned hi = min(w + 1u < (unsigned)p.ev_W ? p.ev_wb[w] : (unsigned)p.Npad, (unsigned)p.Npad);
+        if (hi <= lo) return;
+        const unsigned lines = (hi - lo) / 32u;          // per receptor plane (window bounds are multiples of 1024 neurons)
+        for (unsigned l = blockIdx.x * blockDim.x + threadIdx.x; l < 4u * lines; l += gridDim.x * blockDim.x) {
+            const int32_t* a = ring_slot + (size_t)(l / lines) * Np + lo + (size_t)(l % lines) * 32u;
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(a));
         }
-        const unsigned n_chunks = s_first[n_lists];
-        const size_t Np = (size_t)p.Npad;
-        int32_t* const ring_slot = p.ring + (size_t)(m & (unsigned)(p.D - 1)) * 4 * Np;
-        auto chunk_range = [&](const unsigned c, const uint2*& rec, unsigned& r0, unsigned& r1) {
-            unsigned k;
-            if (c < (unsigned)kEvMapMax) k = s_map[c];
-            else {                                           // largest k with s_first[k] <= c
-                unsigned hi = n_lists;
-                k = 0u;
-                while (hi - k > 1u) { const unsigned mid = (k + hi) >> 1; if (s_first[mid] <= c) k = mid; else hi = mid; }
-            }
-            r0 = (c - s_first[k]) * kEvChunk; r1 = min(r0 + (unsigned)kEvChunk, s_count[k]);
-            rec = ev_records(p, list_of(k));
-        };
-        auto load_chunk = [&](const uint2* rec, const unsigned r0, const unsigned r1, uint4 (&v)[4]) {
+    };
+    prefetch_window(0u);
+    for (unsigned k = 0; k < (unsigned)p.ev_W * fams; ++k) {
+        const unsigned w = k / fams, fam = k % fams;
+        if (fam == 0u && w + 1u < (unsigned)p.ev_W) prefetch_window(w + 1u);
+        const unsigned cur = fam ? (unsigned)(p.ev_Dn * p.ev_W) + (m & (unsigned)(p.ev_D - 1)) * (unsigned)p.ev_W + w
+                                 : (m & (unsigned)(p.ev_Dn - 1)) * (unsigned)p.ev_W + w;
+        const unsigned c = min(s_cur[cur], ev_capacity(p, cur));
+        const uint2* rec = ev_records(p, cur, blockIdx.x);
+        for (unsigned r0 = 0u; r0 < c; r0 += (unsigned)kEvChunk) {
+            uint4 v[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {                    // two records per 128-bit load, four loads in flight
+            for (int u = 0; u < 4; ++u) {                // two records per 128-bit load, four loads in flight
                 const unsigned r = r0 + ((unsigned)u * 256u + threadIdx.x) * 2u;
                 v[u] = make_uint4(0u, 0u, 0u, 0u);
-                if (r + 1u < r1) v[u] = ld_cg_u4(reinterpret_cast<const uint4*>(rec + r));
-                else if (r < r1) { const uint2 a = rec[r]; v[u] = make_uint4(a.x, a.y, 0u, 0u); }
+                if (r + 1u < c) v[u] = ld_cs_u4(reinterpret_cast<const uint4*>(rec + r));
+                else if (r < c) { const uint2 a = rec[r]; v[u] = make_uint4(a.x, a.y, 0u, 0u); }
             }
-        };
-        // the records of the next chunk are requested before the reductions of this one are issued
-        const uint2* rec = nullptr;
-        unsigned r0 = 0u, r1 = 0u;
-        uint4 v[4], vn[4];
-        unsigned c = blockIdx.x;
-        if (c < n_chunks) { chunk_range(c, rec, r0, r1); load_chunk(rec, r0, r1, v); }
-        while (c < n_chunks) {
-            const unsigned cn = c + gridDim.x;
-            const uint2* recn = nullptr;
-            unsigned r0n = 0u, r1n = 0u;
-            if (cn < n_chunks) { chunk_range(cn, recn, r0n, r1n); load_chunk(recn, r0n, r1n, vn); }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const unsigned r = r0 + ((unsigned)u * 256u + threadIdx.x) * 2u;
-                if (r < r1) red_add_s32(ring_slot + (size_t)(v[u].x >> 30) * Np + (v[u].x & 0x3FFFFFFFu), (int)v[u].y);
-                if (r + 1u < r1) red_add_s32(ring_slot + (size_t)(v[u].z >> 30) * Np + (v[u].z & 0x3FFFFFFFu), (int)v[u].w);
+                if (r < c) red_add_s32(ring_slot + (size_t)(v[u].x >> 30) * Np + (v[u].x & 0x3FFFFFFFu), (int)v[u].y);
+                if (r + 1u < c) red_add_s32(ring_slot + (size_t)(v[u].z >> 30) * Np + (v[u].z & 0x3FFFFFFFu), (int)v[u].w);
             }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) v[u] = vn[u];
-            r0 = r0n; r1 = r1n; c = cn;
         }
+        __syncthreads();                                 // every thread has read the count
+        if (threadIdx.x == 0) s_cur[cur] = 0u;           // consumed (the appends below go to later steps: other cursors)
     }
+    __syncthreads();
+    // ---- 2. the rows that fired in step n
     {
-        // ---- 2. the rows that fired in step n
         const unsigned bwarp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
         const unsigned n_bwarps = (gridDim.x * blockDim.x) >> 5;
         const unsigned nto = (unsigned)transfer_step(p, n);
-        const unsigned part = bwarp & (unsigned)(p.ev_P - 1);   // many cursors per slot: same-address atomics serialise in L2
+        unsigned spilled = 0u;
         int* const tab_off = s_tab_off[threadIdx.x >> 5];
         unsigned* const tab_list = s_tab_list[threadIdx.x >> 5];
         const int K = p.ev_near_d * p.ev_W;
         const int2* const work = p.work + (size_t)(n & 1ull) * p.work_half;
-        for (unsigned q = bwarp; q < n_work; q += n_bwarps) {
-            const int2 wk = work[q];
-            const int64_t rb0 = __ldg(p.row_begin + wk.x);
-            const int c0 = wk.y * kChunk, c1 = min(c0 + kChunk, __ldg(p.row_len + wk.x));
-            const int near_end = (int)__ldg(p.seg + (size_t)wk.x * (size_t)(K + 1) + (size_t)K);
-            if (c0 < near_end) bin_near<kHalf>(p, (unsigned)n, nto, wk.x, rb0, c0, min(c1, near_end), lane, part, tab_off, tab_list, spilled);
-            if (c1 > near_end) {                             // far part: runs of about one synapse, positions by vote + atomic
-                const int f0 = max(c0, near_end);
-                bin_span<kHalf>(p, (unsigned)n, nto, rb0 + f0, c1 - f0, lane, part, spilled);
-            }
+        // the descriptor of the next item (work entry two ahead, row start / length / end of the near part one ahead) is
+        // requested while this one is processed
+        int2 wk = make_int2(0, 0), wk1 = make_int2(0, 0);
+        if (bwarp < n_work) wk = work[bwarp];
+        if (bwarp + n_bwarps < n_work) wk1 = work[bwarp + n_bwarps];
+        int64_t rb0 = 0, rb0n = 0;
+        int rlen = 0, rlenn = 0, near_end = 0, near_endn = 0;
+        if (bwarp < n_work) {
+            rb0 = __ldg(p.row_begin + wk.x); rlen = __ldg(p.row_len + wk.x);
+            near_end = (int)__ldg(p.seg + (size_t)wk.x * (size_t)(K + 1) + (size_t)K);
         }
+        for (unsigned q = bwarp; q < n_work; q += n_bwarps) {
+            int2 wk2 = make_int2(0, 0);
+            if (q + 2u * n_bwarps < n_work) wk2 = work[q + 2u * n_bwarps];
+            if (q + n_bwarps < n_work) {
+                rb0n = __ldg(p.row_begin + wk1.x); rlenn = __ldg(p.row_len + wk1.x);
+                near_endn = (int)__ldg(p.seg + (size_t)wk1.x * (size_t)(K + 1) + (size_t)K);
+            }
+            const int c0 = wk.y * kChunk, c1 = min(c0 + kChunk, rlen);
+            if (c0 < near_end) bin_near<kHalf>(p, (unsigned)n, nto, wk.x, rb0, c0, min(c1, near_end), lane, s_cur, tab_off, tab_list, spilled);
+            if (c1 > near_end) {                         // far part: runs of about one synapse, positions by vote + shared-memory atomic
+                const int f0 = max(c0, near_end);
+                bin_span<kHalf>(p, (unsigned)n, nto, rb0 + f0, c1 - f0, lane, s_cur, spilled);
+            }
+            wk = wk1; wk1 = wk2; rb0 = rb0n; rlen = rlenn; near_end = near_endn;
+        }
+        spilled = __reduce_add_sync(0xffffffffu, spilled);
+        if (lane == 0 && spilled) atomicAdd(&p.ctl->ev_spilled, (unsigned long long)spilled);
     }
-    spilled = __reduce_add_sync(0xffffffffu, spilled);
-    if (lane == 0 && spilled) atomicAdd(&p.ctl->ev_spilled, (unsigned long long)spilled);
     __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        s_last = (atomicAdd(&p.ctl->done_lists, 1u) == gridDim.x - 1) ? 1u : 0u;
-    }
-    __syncthreads();
-    if (s_last) {                                 // every block has read the cursors of step m: they start again at zero
-        for (unsigned k = threadIdx.x; k < n_lists; k += blockDim.x) p.ev_cnt[(size_t)list_of(k) * kEvCntStride] = 0u;
-        if (threadIdx.x == 0) p.ctl->done_lists = 0u;
-    }
+    for (unsigned k = threadIdx.x; k < (unsigned)p.ev_n_cur; k += blockDim.x) g_cur[k] = s_cur[k];     // for the next launch
 }
 
 // Read-back of the ring in list mode: the arrivals still to come are the ring's content PLUS the records waiting in
@@ -1355,17 +1343,18 @@ __global__ void __maxnreg__(56) k_deliver_lists(const __grid_constant__ SimDev p
 __global__ void __launch_bounds__(256) k_lists_to_ring(const __grid_constant__ SimDev p, int32_t* __restrict__ out,
                                                        const int first, const int count, const int D_api) {
     const unsigned long long n = p.ctl->step;
-    const unsigned total = (unsigned)(p.ev_n_near + p.ev_n_far);
-    const unsigned per_slot = (unsigned)(p.ev_W * p.ev_P);
-    for (unsigned list = blockIdx.x; list < total; list += gridDim.x) {
-        const bool far = list >= (unsigned)p.ev_n_near;
+    const unsigned n_near = (unsigned)(p.ev_Dn * p.ev_W);
+    const unsigned total = (unsigned)p.ev_n_cur * (unsigned)p.ev_P;
+    for (unsigned l = blockIdx.x; l < total; l += gridDim.x) {
+        const unsigned block = l / (unsigned)p.ev_n_cur, cur = l % (unsigned)p.ev_n_cur;
+        const bool far = cur >= n_near;
         const unsigned depth = far ? (unsigned)p.ev_D : (unsigned)p.ev_Dn;
-        const unsigned slot = (far ? list - (unsigned)p.ev_n_near : list) / per_slot;
+        const unsigned slot = (far ? cur - n_near : cur) / (unsigned)p.ev_W;
         // the one step in [n, n + depth) that maps to this slot
         const unsigned long long arrive = n + (unsigned long long)((slot - (unsigned)n) & (depth - 1u));
         const size_t api_slot = (size_t)(arrive % (unsigned long long)D_api);
-        const unsigned c = min(p.ev_cnt[(size_t)list * kEvCntStride], ev_capacity(p, list));
-        const uint2* rec = ev_records(p, list);
+        const unsigned c = min(p.ev_cnt[(size_t)block * p.ev_n_cur + cur], ev_capacity(p, cur));
+        const uint2* rec = ev_records(p, cur, block);
         for (unsigned r = threadIdx.x; r < c; r += blockDim.x) {
             const uint2 v = rec[r];
             const int tg = (int)(v.x & 0x3FFFFFFFu) - first;
@@ -1438,8 +1427,9 @@ cudaError_t launch_update(const SimDev& p, int n_sm, int mode, cudaStream_t st) 
 
 cudaError_t launch_deliver(const SimDev& p, int grid, unsigned parity, cudaStream_t st) {
     if (p.ev_on) {
-        if (p.w_fp16) k_deliver_lists<true><<<grid, 256, 0, st>>>(p, parity);
-        else          k_deliver_lists<false><<<grid, 256, 0, st>>>(p, parity);
+        const size_t smem = (size_t)p.ev_n_cur * sizeof(unsigned);
+        if (p.w_fp16) k_deliver_lists<true><<<p.ev_P, 256, smem, st>>>(p, parity);        // the grid the lists were laid out for
+        else          k_deliver_lists<false><<<p.ev_P, 256, smem, st>>>(p, parity);
     } else {
         if (p.w_fp16) k_deliver<true><<<grid, 256, 0, st>>>(p);
         else          k_deliver<false><<<grid, 256, 0, st>>>(p);
