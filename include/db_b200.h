@@ -219,7 +219,8 @@ int32_t db_create_from_csr(const db_sim_params* sim, const db_csr_view* csr,
 
 int32_t db_destroy(db_sim* sim);
 
-/* a1-a4 for n_steps consecutive time steps; asynchronous on the stream. */
+/* a1-a4 (one iteration per time step: SI "Numerical method" P:L469-490, Supp. Alg. 2) for n_steps consecutive
+ * time steps; asynchronous on the stream. */
 int32_t db_step(db_sim* sim, uint32_t n_steps);
 
 /* Region-sharded simulation, second sum of SI Eq.(6): the neurons `ids` [n] (global ids, HOST pointer; neurons
@@ -234,18 +235,24 @@ int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint
  * until done.  For per-kernel roofline measurement. */
 int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out);
 
-/* Spikes with step_begin <= step < step_end, sorted by (step, id).  Writes at
+/* a5, the simulator's first output (Supp. Alg. 2 "Output: spike trains"; recorded per ms in the paper).
+ * Spikes with step_begin <= step < step_end, sorted by (step, id).  Writes at
  * most `cap` pairs, *n_out = number available.  DB_ERANGE if part of the range
  * was already overwritten in the raster ring or lies in the future. */
 int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end,
                        uint64_t* steps, int32_t* ids, uint64_t cap, uint64_t* n_out);
 
-/* State of neurons [first, first+count) into dst (layout per DB_FIELD_*). */
+/* a5, the second output (Alg. 2 "Output: ... membrane potentials"; "state variables of neurons"): state of
+ * the neurons [first, first + count) -- GLOBAL ids, inside the range the handle owns -- into dst (layout per DB_FIELD_*).
+ * DB_FIELD_RING = the arrivals still to come, in every execution mode (ring content plus records waiting in arrival lists). */
 int32_t db_read_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, void* dst);
-/* Test hook: overwrite state (identical-state one-step parity). */
+/* Overwrite state: the test hook of the identical-state one-step parity case, and how an outer loop (the paper's
+ * assimilation, out of scope here) replaces parameters such as DB_FIELD_IEXT.  DB_FIELD_RING only before the
+ * first step when arrival lists are in use (DB_ESTATE otherwise). */
 int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count, const void* src);
 
-/* Firing rate in Hz per (window, region) for the completed windows still kept:
+/* a4 (K7 "firing rates of neuron groups"; "over a sliding window").
+ * Firing rate in Hz per (window, region) for the completed windows still kept:
  * spikes / (region size * window seconds) (R24).  rates_hz[w * n_regions + r];
  * *first_window = index of the first window returned. */
 int32_t db_region_rates(db_sim* sim, float* rates_hz, uint64_t cap_windows,
