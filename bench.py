@@ -50,14 +50,16 @@ DELIVER_BYTES_PER_EVENT = {0: 17, 1: 15}   # tgt|rec 4 + w 4 (fp32) / 2 (fp16) +
 LIST_BYTES_PER_EVENT = 16              # list mode: the 8-byte record of an event is written once and read once on top of that
 
 
+STEP_KERNEL_SOURCES = ("db_device.cuh", "db_philox.cuh", "db_step.cu")     # where every kernel of the step loop is defined
+
+
 def _csrc_sha16() -> str:
-    """Hash of the kernel sources: ties a committed ncu capture to the tree it was taken from."""
+    """Hash of the sources of the step kernels: ties a committed ncu capture to the kernels it was taken from."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2211_15963_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh", ".h")):
-            h.update(open(os.path.join(d, f), "rb").read())
+    for f in STEP_KERNEL_SOURCES:
+        h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()[:16]
 
 

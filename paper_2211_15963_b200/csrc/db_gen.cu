@@ -399,7 +399,10 @@ cudaError_t generate_network(const db_network_spec& sp, uint64_t seed, const Gen
     k_gen_types<<<(unsigned)((g.ownN + 255) / 256), 256, 0, st>>>(g, ntype_dev);
     GCK(cudaGetLastError());
 
-    const unsigned warp_grid = (unsigned)std::min<int64_t>((N + 7) / 8, 148 * 64);
+    int dev = 0, n_sm = 0;
+    GCK(cudaGetDevice(&dev));
+    GCK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    const unsigned warp_grid = (unsigned)std::min<int64_t>((N + 7) / 8, (int64_t)n_sm * 64);
     if (sp.mode == DB_MODE_FIXED_INDEGREE) {
         k_gen_indegree<false><<<warp_grid, 256, 0, st>>>(g);
     } else {
