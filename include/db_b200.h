@@ -48,7 +48,9 @@ extern "C" {
 #define DB_ERANGE  (-4)   /* requested steps / elements are not (or no longer) available */
 #define DB_ESTATE  (-5)   /* call not valid in the current state of the handle */
 
-#define DB_MAX_TYPES 4    /* neuron types; 0 = excitatory, 1 = inhibitory */
+#define DB_MAX_TYPES 8    /* neuron types, each with its own constants (property table P:L816-832 held per type, R-D1): the generator
+                             uses 0 = excitatory, 1 = inhibitory; a CSR may use all eight (e.g. the populations of a micro-column,
+                             Ext. Table 3, or (region group, type) pairs) */
 #define DB_N_RECEPTORS 4  /* 0 AMPA, 1 NMDA, 2 GABA_A, 3 GABA_B */
 
 typedef struct db_sim db_sim;

@@ -47,7 +47,7 @@ class TypeParams(C.Structure):
 
 class SimParams(C.Structure):
     _fields_ = [("dt_ms", C.c_double), ("S", C.c_int32), ("D", C.c_int32), ("window_steps", C.c_int32),
-                ("n_types", C.c_int32), ("type", TypeParams * 4), ("spike_bin_steps", C.c_int32)]
+                ("n_types", C.c_int32), ("type", TypeParams * 8), ("spike_bin_steps", C.c_int32)]
 
 
 class NetSpec(C.Structure):

@@ -253,7 +253,7 @@ struct orc_sim_params {
     int32_t D;            // ring depth, power of two, > max delay
     int32_t window_steps; // region-rate window (R24)
     int32_t n_types;
-    orc_type_params type[4];
+    orc_type_params type[8];
     // Time bin for transferring spikes, b_t, in steps (SI "Numerical method"; the paper sets
     // b_t = 1 ms even at dt = 0.1 ms).  Reading R29: A_j(t) = 1 only at the bin boundaries t = k b_t,
     // for the neurons that fired in (t - b_t, t].  0 or 1: every step is a boundary.

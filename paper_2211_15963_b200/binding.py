@@ -49,7 +49,7 @@ class BoldParams(C.Structure):
 
 class SimParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("dt_ms", C.c_double), ("S", C.c_int32), ("D", C.c_int32),
-                ("window_steps", C.c_int32), ("n_types", C.c_int32), ("type", TypeParams * 4),
+                ("window_steps", C.c_int32), ("n_types", C.c_int32), ("type", TypeParams * 8),
                 ("dyn_seed", C.c_uint64), ("raster_capacity", C.c_uint64), ("max_windows", C.c_uint32),
                 ("exec_mode", C.c_int32), ("spike_bin_steps", C.c_int32), ("bold", BoldParams)]
 
@@ -149,7 +149,7 @@ def _fill_sim_params(p: SimParams, d: dict, dyn_seed: int, exec_mode: int, raste
     p.struct_size = C.sizeof(SimParams)
     p.dt_ms, p.S, p.D, p.window_steps = d["dt_ms"], d["S"], d["D"], d["window_steps"]
     p.n_types = len(d["types"])
-    for i, t in enumerate(d["types"]):
+    for i, t in enumerate(d["types"][:len(p.type)]):       # (more than DB_MAX_TYPES: n_types says so and the library refuses)
         q = p.type[i]
         for k in ("C", "gL", "VL", "Vth", "Vreset", "Tref_ms", "Iext", "bg_rate_hz", "bg_weight"):
             setattr(q, k, float(t[k]))

@@ -154,7 +154,7 @@ int32_t check_sim_params(db_sim* sim, const db_sim_params* sp) {
     if (sp->S < 0 || sp->S > 30) return fail(sim, DB_EINVAL, "S must be within 0..30");
     if (sp->D < 2 || sp->D > 65536 || (sp->D & (sp->D - 1))) return fail(sim, DB_EINVAL, "D must be a power of two in 2..65536");
     if (sp->window_steps < 1) return fail(sim, DB_EINVAL, "window_steps must be >= 1");
-    if (sp->n_types < 1 || sp->n_types > DB_MAX_TYPES) return fail(sim, DB_EINVAL, "n_types must be 1..4");
+    if (sp->n_types < 1 || sp->n_types > DB_MAX_TYPES) return fail(sim, DB_EINVAL, "n_types must be 1..8");
     if (sp->exec_mode < DB_EXEC_AUTO || sp->exec_mode > DB_EXEC_KERNELS_DEFERRED) return fail(sim, DB_EINVAL, "bad exec_mode");
     if (sp->spike_bin_steps < 0 || sp->spike_bin_steps > 4096) return fail(sim, DB_EINVAL, "spike_bin_steps must be within 0..4096");
     return DB_OK;

@@ -6,7 +6,7 @@
 
 namespace dbk {
 
-constexpr int kMaxTypes = 4;
+constexpr int kMaxTypes = 8;          // neuron types with their own constants (rt keeps the type in 4 bits); 8 = the populations of a micro-column (Ext. Table 3)
 constexpr int kPoissonMax = 32;
 constexpr int kNeuronPad = 1024;     // Npad is a multiple of this: whole warps, 128-bit accesses
 constexpr int kRowAlign = 4;         // CSR rows start on a multiple of 4 synapses (128-bit target loads)

@@ -321,3 +321,40 @@ def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, o
     assert e.value.code == db.binding.DB_ERANGE
     with pytest.raises(db.DbError):
         shards[1].db_read_state(db.FIELD_V, first=0, count=10)       # not its neurons
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_eight_neuron_types_with_their_own_constants(db, oracle_mod, mode):
+    # R-D1: the property table is held per type; eight types cover the populations of a micro-column (Ext. Table 3)
+    # or (region group, type) pairs.  Types are interleaved neuron by neuron, so almost every 4-neuron group of a thread
+    # mixes types (the slow path of neuron_group), and every constant differs between types.
+    rng = np.random.default_rng(77)
+    types = []
+    for k in range(8):
+        t = db_inputs.type_params(bg_weight=0.006 + 0.001 * k, bg_rate_hz=800.0 + 100.0 * k)
+        t.update(Iext=0.02 * k - 0.05, C=0.8 + 0.05 * k, gL=0.025 + 0.002 * k, VL=-76.0 + 0.5 * k, Vth=-51.0 + 0.3 * k,
+                 Vreset=-66.0 + 0.4 * k, Tref_ms=2.0 + 0.5 * k,
+                 G=[1.0 + 0.05 * k, 0.25 - 0.01 * k, 1.0 - 0.03 * k, 1.0 + 0.02 * k],
+                 E=[0.0 + 0.5 * k, -1.0 * k, -70.0 - k, -100.0 + k], tau_ms=[2.0 + 0.1 * k, 40.0 - k, 10.0 + 0.5 * k, 50.0 - 2 * k])
+        if k in (2, 5):
+            t.update(ou_mu=0.5, ou_sigma=0.1, ou_tau_ms=8.0 + k)
+        if k in (3, 5):
+            t.update(iext_gamma_shape=2.0, iext_gamma_scale=0.03)
+        types.append(t)
+    sim = db_inputs.sim_params(types=types)
+    N = 5000 + 11
+    net = db_inputs.random_csr(N=N, mean_outdeg=25, seed=55)
+    net["ntype"] = rng.integers(0, 8, N).astype(np.uint8)
+    net["rec"] = (2 * (net["ntype"][np.repeat(np.arange(N), np.diff(net["row_ptr"]))] % 2) + (net["rec"] % 2)).astype(np.uint8)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    assert np.array_equal(g.db_read_state(db.FIELD_TYPE), net["ntype"])
+    assert np.array_equal(g.db_read_state(db.FIELD_IEXT), o.iext().astype(np.float32))
+    for upto in (1, 3, 90, 500):
+        g.db_step(upto - int(g.db_get_counters()["steps"])); o.step(upto - o.step_index)
+        n = _check(g, o, upto)
+        assert np.array_equal(g.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32))
+    ids = g.db_read_spikes(0, 500)[1]
+    assert all(np.count_nonzero(net["ntype"][ids] == k) > 5 for k in range(8)), np.bincount(net["ntype"][ids], minlength=8)
+    with pytest.raises(db.DbError):
+        db.Sim.db_create_from_csr(db_inputs.sim_params(types=types + [types[0]]), net)      # nine types

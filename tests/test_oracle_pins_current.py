@@ -199,3 +199,27 @@ def test_ring_wraps_in_twos_complement_and_raises_the_sticky_flag(oracle_mod, fp
         assert o.counters()["overflow"] == int(trips), val
         o.step(5)
         assert o.counters()["overflow"] == int(trips)
+
+
+def test_eight_types_each_relax_to_their_own_fixed_point(oracle_mod):
+    # up to eight neuron types with their own constants (the populations of a micro-column, Ext. Table 3, or
+    # (region group, type) pairs): neuron i of type i mod 8 relaxes to ITS fixed point
+    types = []
+    for k in range(8):
+        types.append(_frozen_type(Iext=0.05 * k - 0.1, gL=0.02 + 0.005 * k, VL=-78.0 + 1.5 * k, C=0.7 + 0.1 * k,
+                                  G=[1.3 - 0.1 * k, 0.21 + 0.02 * k, 0.77 + 0.05 * k, 1.9 - 0.15 * k],
+                                  E=[3.0 - k, -11.0 + k, -68.0 - 0.5 * k, -97.0 + k]))
+    N = 64
+    ntype = (np.arange(N) % 8).astype(np.uint8)
+    s, _ = _lone_neurons(oracle_mod, N, 0.1, types, ntype=ntype)
+    V, g, ref = s.state()
+    V[:] = -66.0
+    g[:] = [0.02, 0.01, 0.03, 0.015]
+    s.set_state(V, g, ref)
+    s.step(40000)
+    got = s.state()[0]
+    for i in range(N):
+        t = types[i % 8]
+        a = [t["G"][u] * g[i, u] for u in range(4)]
+        Vinf = (t["gL"] * t["VL"] + sum(a[u] * t["E"][u] for u in range(4)) + t["Iext"]) / (t["gL"] + sum(a))
+        assert abs(got[i] - Vinf) < 1e-9, i
