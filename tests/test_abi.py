@@ -74,3 +74,25 @@ def test_create_fails_loudly_without_a_gpu():
     rc = L.db_create_from_csr(ctypes.byref(sp), ctypes.byref(v), None, ctypes.byref(h))
     assert rc == db.binding.DB_ECUDA and not h
     assert b"CUDA" in L.db_last_error(None)
+
+
+def test_create_from_csr_rejects_bad_sizes_before_touching_the_arrays():
+    # N, E and n_regions are checked before row_ptr[N] or delay[0..E) is read (no device needed: the checks come first)
+    import numpy as np
+    import db_inputs
+    import paper_2211_15963_b200 as db
+    L = db.load()
+    sp = db.binding.SimParams()
+    db.binding._fill_sim_params(sp, db_inputs.sim_params(), 1, 0, 0, 0)
+    net = db_inputs.random_csr(64, 5, 1)
+    keep = [np.ascontiguousarray(net["region_start"], np.int64), net["ntype"], net["row_ptr"], net["tgt"], net["w"],
+            net["delay"], net["rec"]]
+    ptrs = [a.ctypes.data_as(ctypes.c_void_p) for a in keep]
+    for N, E, R in ((-1, 10, 1), (0, 0, 1), (1 << 30, 10, 1), (64, -3, 1), (64, int(net["E"]), 0), (64, int(net["E"]), 70000)):
+        v = db.binding.CsrView(N, E, R, *ptrs, 0, 0, 0)
+        h = ctypes.c_void_p()
+        rc = L.db_create_from_csr(ctypes.byref(sp), ctypes.byref(v), None, ctypes.byref(h))
+        assert rc == db.binding.DB_EINVAL and not h, (N, E, R, rc)
+    v = db.binding.CsrView(64, int(net["E"]), 1, None, *ptrs[1:], 0, 0, 0)          # a missing array
+    h = ctypes.c_void_p()
+    assert L.db_create_from_csr(ctypes.byref(sp), ctypes.byref(v), None, ctypes.byref(h)) == db.binding.DB_EINVAL

@@ -358,3 +358,21 @@ def test_eight_neuron_types_with_their_own_constants(db, oracle_mod, mode):
     assert all(np.count_nonzero(net["ntype"][ids] == k) > 5 for k in range(8)), np.bincount(net["ntype"][ids], minlength=8)
     with pytest.raises(db.DbError):
         db.Sim.db_create_from_csr(db_inputs.sim_params(types=types + [types[0]]), net)      # nine types
+
+
+def test_bold_readout_keeps_up_inside_db_step_profiled(db, oracle_mod):
+    # db_step_profiled (CUDA events around every kernel) lets the BOLD read-out catch up before its short count history wraps
+    N, R = 3000, 5
+    net = db_inputs.random_csr(N=N, mean_outdeg=25, seed=8, n_regions=R)
+    t = db_inputs.type_params(bg_weight=0.02)
+    sim = db_inputs.sim_params(types=[t, dict(t)])
+    sim["bold"] = dict(oracle_mod.BOLD_DEFAULTS)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=1, max_windows=16)     # history of 13 windows = 130 steps
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    prof = g.db_step_profiled(700)
+    o.step(700)
+    assert prof["steps"] == 700 and prof["update_ms"] > 0 and prof["deliver_ms"] > 0
+    y, st, n = g.db_read_bold()
+    sizes = np.diff(net["region_start"])
+    ys, so = oracle_mod.bold_run(o.region_counts()[:n], sizes, sim["window_steps"] * sim["dt_ms"] * 1e-3, sim["bold"])
+    assert n == 70 and np.max(np.abs(st - so)) < 1e-10 and np.max(np.abs(y - ys[-1])) < 1e-10
