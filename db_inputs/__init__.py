@@ -185,3 +185,108 @@ def bulk_csr(N: int, base_outdeg: int, seed: int, heavy_rows: dict | None = None
     rec = (2 * src_type + (rng.random(E) < 0.2)).astype(np.uint8)
     return dict(N=N, E=E, n_regions=n_regions, region_start=bounds, ntype=ntype, row_ptr=row_ptr, tgt=tgt, w=w,
                 delay=delay, rec=rec)
+
+
+# ---- Cortical laminar micro-column (Extended Data Table 3) --------------------------------
+# Average number of synapses received by one neuron of the postsynaptic population (rows) from each presynaptic
+# population (columns), as the paper prints it; blanks are 0.  The table has no presynaptic e1 column.  CC = other
+# cortical regions.
+MC_POPS = ("e1", "i1", "e2/3", "i2/3", "e4", "i4", "e5", "i5", "e6", "i6")
+MC_PRE = ("i1", "e2/3", "i2/3", "e4", "i4", "e5", "i5", "e6", "i6", "CC")
+MC_TABLE3 = np.array([
+    [1323,  823, 200,   15,   1,   9,   0,    0,   0, 10133],   # e1
+    [ 901,  560, 149,   10,   1,   6,   0,    0,   0,  6899],   # i1
+    [ 133, 3554, 804,  881,  45, 431,   0,  136,   0,  1020],   # e2/3
+    [  52, 1778, 532,  456,  29, 217,   0,   69,   0,   396],   # i2/3
+    [  27,  417,  84, 1070, 782,  79,   8, 1686,   0,  1489],   # e4
+    [   0,  168,  41,  628, 538,  36,   0, 1028,   0,   790],   # i4
+    [ 147, 2550, 176,  765,  99, 621, 596,  363,   0,  1591],   # e5
+    [   0, 1357,  76,  380,  32, 375, 403,  129,   0,   214],   # i5
+    [   2,  643,  46,  549, 196, 327, 126,  925, 597,  2609],   # e6
+    [   0,   80,   8,   92,   3, 159,  11,   76, 499,  1794],   # i6
+], np.float64)
+
+
+def microcolumn_sizes(voxel_neurons: int) -> np.ndarray:
+    """Neurons per population of one voxel.  The paper takes them 'proportional to the statistics given in Du et al.'
+     and does not print them: here every layer gets a fifth of the voxel, 80 % of it excitatory; the
+    last population takes the rounding remainder.  A synthetic stand-in."""
+    per_layer = voxel_neurons // 5
+    sizes = []
+    for layer in range(5):
+        n = per_layer if layer < 4 else voxel_neurons - 4 * per_layer
+        ne = int(round(0.8 * n))
+        sizes += [ne, n - ne]
+    return np.array(sizes, np.int64)
+
+
+def microcolumn_indegrees(voxel_neurons: int, d_in: float, with_cc: bool = True) -> np.ndarray:
+    """Integer in-degrees [10 post][10 pre incl. CC]: Table 3 scaled by ONE factor so that the average number of input
+    synapses per neuron of the voxel is d_in (P:L402 'fixing the average number of input synapses of neurons in this
+    voxel as constant d_in'), rounded to nearest."""
+    sizes = microcolumn_sizes(voxel_neurons).astype(np.float64)
+    T = MC_TABLE3.copy()
+    if not with_cc:
+        T[:, 9] = 0.0
+    mean_in = float((sizes * T.sum(axis=1)).sum() / sizes.sum())
+    return np.rint(T * (d_in / mean_in)).astype(np.int64)
+
+
+def microcolumn_csr(n_voxels: int, voxel_neurons: int, d_in: float, seed: int, w_scale: float = 0.008,
+                    inh_mult: float = 4.0, slow_frac: float = 0.2, delay_intra: tuple = (1, 8),
+                    delay_cc: tuple = (10, 20)) -> dict:
+    """Voxels of the cortical laminar model as a presynaptic-major CSR: region = voxel, ten populations per
+    voxel in the order of MC_POPS.  Every neuron of population p draws, with repetition, microcolumn_indegrees()[p][q]
+    sources uniformly from population q of ITS OWN voxel, and the CC share uniformly from the excitatory neurons of the
+    OTHER voxels ('we allocated the output synapses from the excitatory neurons across all layers based on their
+    population sizes'; with one voxel the CC column is dropped).  Weights ~ w_scale * U[0,1], inhibitory
+    sources times inh_mult; receptors AMPA / NMDA for excitatory sources, GABA_A / GABA_B for inhibitory ones, the slow
+    one with probability slow_frac; delays uniform in delay_intra inside the voxel, in delay_cc between voxels (steps).
+    Neuron type: 0 excitatory, 1 inhibitory."""
+    rng = np.random.default_rng(seed)
+    sizes = microcolumn_sizes(voxel_neurons)
+    off = np.concatenate([[0], np.cumsum(sizes)])
+    N = n_voxels * voxel_neurons
+    with_cc = n_voxels > 1
+    K = microcolumn_indegrees(voxel_neurons, d_in, with_cc)
+    pre_pop = [MC_POPS.index(q) for q in MC_PRE[:9]]           # column -> population index
+    pop_of = np.repeat(np.arange(10), sizes)                   # inside one voxel
+    ntype = np.tile((pop_of % 2).astype(np.uint8), n_voxels)
+    exc_local = np.flatnonzero(pop_of % 2 == 0)
+    srcs, tgts, inter = [], [], []
+    for v in range(n_voxels):
+        base = v * voxel_neurons
+        for p in range(10):
+            post = base + off[p] + np.arange(sizes[p])
+            for c in range(9):
+                k = int(K[p][c])
+                if k == 0:
+                    continue
+                q = pre_pop[c]
+                srcs.append(base + off[q] + rng.integers(0, sizes[q], sizes[p] * k))
+                tgts.append(np.repeat(post, k))
+                inter.append(np.zeros(sizes[p] * k, bool))
+            k = int(K[p][9])
+            if k:
+                n = sizes[p] * k
+                ov = rng.integers(0, n_voxels - 1, n)
+                ov += ov >= v                                  # any voxel but v
+                srcs.append(ov * voxel_neurons + exc_local[rng.integers(0, len(exc_local), n)])
+                tgts.append(np.repeat(post, k))
+                inter.append(np.ones(n, bool))
+    src = np.concatenate(srcs).astype(np.int64)
+    tgt = np.concatenate(tgts).astype(np.int64)
+    inter = np.concatenate(inter)
+    E = len(src)
+    w = (w_scale * rng.random(E)).astype(np.float32)
+    src_inh = ntype[src] == 1
+    w = np.where(src_inh, w * np.float32(inh_mult), w).astype(np.float32)
+    rec = (2 * src_inh + (rng.random(E) < slow_frac)).astype(np.uint8)
+    delay = np.where(inter, rng.integers(delay_cc[0], delay_cc[1] + 1, E),
+                     rng.integers(delay_intra[0], delay_intra[1] + 1, E)).astype(np.uint8)
+    order = np.lexsort((tgt, src))                             # presynaptic-major, targets ascending inside a row
+    row_ptr = np.zeros(N + 1, np.int64)
+    row_ptr[1:] = np.cumsum(np.bincount(src, minlength=N))
+    return dict(N=N, E=E, n_regions=n_voxels, region_start=np.arange(n_voxels + 1, dtype=np.int64) * voxel_neurons,
+                ntype=ntype, row_ptr=row_ptr, tgt=tgt[order].astype(np.int32), w=w[order], delay=delay[order],
+                rec=rec[order])

@@ -376,3 +376,26 @@ def test_bold_readout_keeps_up_inside_db_step_profiled(db, oracle_mod):
     sizes = np.diff(net["region_start"])
     ys, so = oracle_mod.bold_run(o.region_counts()[:n], sizes, sim["window_steps"] * sim["dt_ms"] * 1e-3, sim["bold"])
     assert n == 70 and np.max(np.abs(st - so)) < 1e-10 and np.max(np.abs(y - ys[-1])) < 1e-10
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_cortical_microcolumn_workload(db, oracle_mod, mode):
+    # SURVEY 8(f), unranked extra: voxels of the cortical laminar model (Extended Data Table 3),
+    # ten populations per voxel with the table's population-specific in-degrees, cortico-cortical input from the
+    # excitatory neurons of the other voxels (db_inputs.microcolumn_csr; 8 voxels x 4,000 neurons, d_in = 100:
+    # 3.2e6 synapses, in-degrees 38-180, out-degrees 0-~500).  Voxel = region, so a4 gives the voxel rates.
+    net = db_inputs.microcolumn_csr(8, 4000, 100, seed=21)
+    t = db_inputs.type_params(bg_weight=0.0072)
+    sim = db_inputs.sim_params(types=[t, dict(t)], D=32)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    assert g.db_get_counters()["exec_mode"] == mode
+    for steps in (1, 50, 400):
+        g.db_step(steps - int(g.db_get_counters()["steps"])); o.step(steps - int(o.counters()["steps"]))
+        n = _check(g, o, steps)
+    assert n > 2000                                                # ~14 Hz (tests/test_inputs_microcolumn.py)
+    cnt, first = g.db_region_counts()
+    assert len(cnt) >= 30 and np.array_equal(cnt, o.region_counts()[first:first + len(cnt)])
+    # e1 neurons (the first 640 of every voxel) send nothing inside their voxel: only their cortico-cortical share
+    deg = np.diff(net["row_ptr"])
+    assert deg[:640].mean() < 0.5 * deg[800:1440].mean()
