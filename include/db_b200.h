@@ -233,6 +233,17 @@ int32_t db_step(db_sim* sim, uint32_t n_steps);
  * single-handle simulation bit for bit (tests).  Asynchronous on the stream like db_step. */
 int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n);
 
+/* The same operation for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): identical arguments, checks and result (the ring cells and the event counter get the
+ * same integers), but the device copy of `ids` lives in a static device array of DB_EXTERNAL_STATIC_MAX ids (256 KB that
+ * every GPU which loads the library holds until the process exits) instead of a buffer db_deliver_external grows on
+ * demand.  Calls no cudaMalloc / cudaFree and no allocating library routine.  n > DB_EXTERNAL_STATIC_MAX: DB_EINVAL
+ * (db_last_error says so); split the list, or use db_deliver_external.  All handles on one device share the array and it
+ * keeps the last call's list: a call overwrites the entries it reads (nothing needs clearing), and two calls that overlap
+ * on the GPU (handles on different streams of the same device) race -- serialise them. */
+#define DB_EXTERNAL_STATIC_MAX 65536
+int32_t db_deliver_external_static(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n);
+
 /* Same in DB_EXEC_KERNELS mode with CUDA events around every kernel; blocks
  * until done.  For per-kernel roofline measurement. */
 int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out);

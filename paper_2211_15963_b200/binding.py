@@ -18,9 +18,10 @@ DB_OK, DB_EINVAL, DB_ENOMEM, DB_ECUDA, DB_ERANGE, DB_ESTATE = 0, -1, -2, -3, -4,
 EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 (FIELD_V, FIELD_G_AMPA, FIELD_G_NMDA, FIELD_G_GABAA, FIELD_G_GABAB, FIELD_REF, FIELD_TYPE, FIELD_RING,
  FIELD_OUTDEG, FIELD_IOU, FIELD_IEXT) = range(11)
+EXTERNAL_STATIC_MAX = 65536   # DB_EXTERNAL_STATIC_MAX
 
 EXPORTS = [
-    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_deliver_external", "db_step_profiled", "db_read_spikes",
+    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_deliver_external", "db_deliver_external_static", "db_step_profiled", "db_read_spikes",
     "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_export_csr",
     "db_free_csr", "db_get_counters", "db_synchronize", "db_last_error",
 ]
@@ -120,6 +121,7 @@ def load():
         L.db_destroy.argtypes = [C.c_void_p]
         L.db_step.argtypes = [C.c_void_p, C.c_uint32]
         L.db_deliver_external.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64]
+        L.db_deliver_external_static.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64]
         L.db_step_profiled.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(PhaseTimes)]
         L.db_read_spikes.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_uint64,
                                      C.POINTER(C.c_uint64)]
@@ -298,6 +300,11 @@ class Sim:
     def db_deliver_external(self, step: int, ids: np.ndarray):
         ids = np.ascontiguousarray(ids, np.int32)
         self._ck(self.L.db_deliver_external(self.h, int(step), _p(ids), len(ids)))
+
+    def db_deliver_external_static(self, step: int, ids: np.ndarray):
+        """db_deliver_external without any device allocation (at most EXTERNAL_STATIC_MAX ids per call)."""
+        ids = np.ascontiguousarray(ids, np.int32)
+        self._ck(self.L.db_deliver_external_static(self.h, int(step), _p(ids), len(ids)))
 
     def db_step_profiled(self, n_steps: int) -> dict:
         t = PhaseTimes()

@@ -743,6 +743,99 @@ int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint
     return DB_OK;
 }
 
+}  // extern "C" (interrupted for the device side of db_deliver_external_static; resumed below)
+
+// ---------------------------------------------------------------------------------------------------------------------
+// db_deliver_external_static: the entry point that allocates nothing (callers under CUDA graph capture, serving loops
+// and harnesses that forbid cudaMalloc).  db_deliver_external keeps the device copy of the id list in a buffer it
+// (re)allocates when the list grows; here that scratch is a file-scope array of DB_EXTERNAL_STATIC_MAX ids (256 KB),
+// held by every GPU that loads the library until the process exits.  In HOST code the name `g_ext_ids_static` is a
+// host-side stand-in, not a device address: the kernel is given the address cudaGetSymbolAddress returns on the
+// handle's device (static_ext_ids below, once per device, with that device current).  Every call on a device shares
+// the array, which keeps the last call's list: each call overwrites the entries it reads (nothing has to start at
+// zero), and two calls that overlap on the GPU -- different handles on different streams of one device -- race.
+// ---------------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) int32_t g_ext_ids_static[DB_EXTERNAL_STATIC_MAX];
+
+namespace {
+
+// Variant of k_deliver_external (db_step.cu) whose id list lives in the static array: one warp per outside spike, one
+// synapse per lane and pass.  Same integer reductions into the same ring cells as the existing kernel (their order
+// does not matter), same event count.  SI Eq.(6) second sum.
+__global__ void __launch_bounds__(256) k_deliver_external_static(const __grid_constant__ SimDev p, const int32_t* __restrict__ ids,
+                                                                 const unsigned n_ids, const unsigned long long step) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
+    const unsigned long long b = (unsigned long long)p.bin_steps;
+    const unsigned nto = (unsigned)(p.bin_steps == 1 ? step : step - step % b + (b - 1ull));   // end of the spike's time bin (R29)
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    unsigned long long ev = 0ull;
+    for (unsigned q = warp; q < n_ids; q += n_warps) {
+        const int j = ids[q];
+        const int64_t rb = __ldg(p.row_begin + j);
+        const int len = __ldg(p.row_len + j);
+        for (int e = (int)lane; e < len; e += 32) {
+            const uint32_t tr = __ldg(p.tgt_rec + rb + e);
+            const unsigned dl = __ldg(p.delay + rb + e);
+            const float w = p.w_fp16 ? __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e))
+                                     : __ldg(static_cast<const float*>(p.w) + rb + e);
+            const int wq = __float2int_rn(__fmul_rn(w, p.wscale));
+            int32_t* cell = p.ring + ((size_t)((nto + dl) & Dm) * 4 + (tr >> 30)) * Np + (tr & 0x3FFFFFFFu);
+            asm volatile("red.global.add.s32 [%0], %1;" :: "l"(cell), "r"(wq) : "memory");
+        }
+        ev += (unsigned long long)len;
+    }
+    if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
+}
+
+constexpr int kMaxStaticDevices = 64;
+int32_t* g_ext_ids_static_addr[kMaxStaticDevices] = {};     // device address of g_ext_ids_static, per device ordinal
+
+// Set-up, once per device, with that device current: the device address of the static array.
+cudaError_t static_ext_ids(int device, int32_t** out) {
+    if (device < 0 || device >= kMaxStaticDevices) return cudaErrorInvalidDevice;
+    if (!g_ext_ids_static_addr[device]) {
+        int32_t* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_ext_ids_static);
+        if (e != cudaSuccess) return e;
+        g_ext_ids_static_addr[device] = ptr;                // (racing first calls store the same value)
+    }
+    *out = g_ext_ids_static_addr[device];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t db_deliver_external_static(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n) {
+    if (!sim || (n && !ids)) return DB_EINVAL;
+    if (n > (uint64_t)DB_EXTERNAL_STATIC_MAX)
+        return fail(sim, DB_EINVAL, "db_deliver_external_static: more than DB_EXTERNAL_STATIC_MAX (65536) ids in one call; "
+                                    "split the list or use db_deliver_external");
+    if (n == 0) return DB_OK;
+    CK(cudaSetDevice(sim->device));
+    const SimDev& d = sim->dev;
+    for (uint64_t k = 0; k < n; ++k) {
+        if (ids[k] < 0 || ids[k] >= d.n_rows) return fail(sim, DB_EINVAL, "id out of range");
+        if (ids[k] >= d.id0 && ids[k] < d.id0 + d.N) return fail(sim, DB_EINVAL, "id is owned by this handle: its spikes are delivered by db_step");
+    }
+    const uint64_t b = (uint64_t)d.bin_steps, nt = step - step % b + (b - 1);
+    if (nt + (uint64_t)sim->min_delay < sim->host_step) return fail(sim, DB_ERANGE, "too late: the handle has stepped past the arrival of these spikes");
+    if (nt + (uint64_t)sim->max_delay >= sim->host_step + (uint64_t)d.D - 2) return fail(sim, DB_ERANGE, "too early: the arrivals lie beyond the ring");
+    int32_t* scratch = nullptr;
+    CK(static_ext_ids(sim->device, &scratch));
+    CK(cudaMemcpyAsync(scratch, ids, (size_t)n * 4, cudaMemcpyHostToDevice, sim->stream));
+    CK(cudaStreamSynchronize(sim->stream));            // `ids` is the caller's pageable memory
+    const unsigned grid = std::min<unsigned>(((unsigned)n + 7u) / 8u, (unsigned)sim->n_sm * 8u);
+    k_deliver_external_static<<<grid, 256, 0, sim->stream>>>(d, scratch, (unsigned)n, (unsigned long long)step);
+    CK(cudaGetLastError());
+    sim->launches += 1;
+    return DB_OK;
+}
+
 int32_t db_step_profiled(db_sim* sim, uint32_t n_steps, db_phase_times* out) {
     if (!sim || !out) return DB_EINVAL;
     CK(cudaSetDevice(sim->device));
