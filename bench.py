@@ -261,6 +261,77 @@ def reduce_over_ranks(dist, device, ms: float, sums: list):
 
 
 # --------------------------------------------------------------------------------------------- CUDA arm
+def shard_pair(db, torch, local, n_sim=1000, d_min=10, peer=True):
+    """SURVEY 8(f) row 3, the half one GPU can measure: configs[1] (delays U{d_min..20} so that the exchange window is
+    d_min steps) split between TWO handles on this GPU, each owning half of the targets and the synapses onto them from
+    every source (SI Eq.(6); layout P:L494).  They step d_min steps one after the other, then each one's
+    spikes go to the other through the public API: device to device (db_exchange_peer: the receiver reads the sender's
+    raster in device memory; peer=True), or through the host (db_read_spikes -> db_deliver_external_window, as between
+    ranks of a multi-process run).  Wall clock with a device synchronise at the ends; on two GPUs the handles would run
+    side by side, so the per-shard figure is half the pair's."""
+    from paper_2211_15963_b200 import sharded
+    cfg = _make_cfg(1, 7)
+    cfg["net"].update(delay_intra_min=d_min)
+    N = cfg["net"]["N"]
+    cut = (N // 2) // 1024 * 1024
+    bounds = [0, cut, N]
+    shards = [db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, dyn_seed=db_inputs.DYN_SEED, exec_mode=db.EXEC_AUTO,
+                               raster_capacity=1 << 24, device=local, own=(bounds[k], bounds[k + 1] - bounds[k])) for k in range(2)]
+
+    def window(done, clock):
+        t0 = time.perf_counter()
+        for sh in shards:
+            sh.db_step(d_min)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        n_ext = 0
+        if peer:
+            for k, dst in enumerate(shards):
+                dst.db_exchange_peer(shards[1 - k], done, done + d_min)
+        else:
+            fresh = [sh.db_read_spikes(done, done + d_min) for sh in shards]
+            for k, dst in enumerate(shards):
+                st, ids = fresh[1 - k]
+                if len(ids):
+                    dst.db_deliver_external_window(done, d_min, st, ids)
+                    n_ext += len(ids)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        if clock is not None:
+            clock[0] += t1 - t0; clock[1] += t2 - t1; clock[2] += n_ext
+
+    done = 0
+    for _ in range(300 // d_min):                      # past the start-up transient
+        window(done, None); done += d_min
+    c0 = [sh.db_get_counters() for sh in shards]
+    clock = [0.0, 0.0, 0]
+    for _ in range(n_sim // d_min):
+        window(done, clock); done += d_min
+    c1 = [sh.db_get_counters() for sh in shards]
+    steps = n_sim // d_min * d_min
+    free_us = None
+    if peer:                                           # the same loop as a run would issue it: nothing waits on the host
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sharded.run_local(shards, steps, d_min)
+        torch.cuda.synchronize()
+        free_us = 1e6 * (time.perf_counter() - t0) / steps
+    events = sum(b["events"] - a_["events"] for a_, b in zip(c0, c1))
+    spikes = sum(b["spikes"] - a_["spikes"] for a_, b in zip(c0, c1))
+    for sh in shards:
+        sh.db_destroy()
+    tot = clock[0] + clock[1]
+    return {"n_neurons": N, "shards": 2, "owned": [cut, N - cut], "exchange_every_steps": d_min,
+            "exec_mode": {1: "kernels+graph", 2: "persistent", 3: "kernels+graph, arrival lists"}.get(c1[0]["exec_mode"]),
+            "pair_us_per_sim_step": 1e6 * tot / steps, "per_shard_us_per_sim_step": 0.5e6 * tot / steps,
+            "step_us_per_sim_step_pair": 1e6 * clock[0] / steps, "exchange_us_per_sim_step_pair": 1e6 * clock[1] / steps,
+            "external_spikes_per_sim_step": spikes / steps, "events_per_s_pair": events / tot,
+            "mean_rate_hz": spikes / N / (steps * cfg["sim"]["dt_ms"] * 1e-3), "sim_steps_timed": steps,
+            "pair_us_per_sim_step_no_host_sync": free_us,
+            "exchange": "db_exchange_peer (device to device)" if peer else "db_read_spikes -> host -> db_deliver_external_window",
+            "what": "two handles on ONE GPU run one after the other; wall clock (not a multi-GPU measurement)"}
+
+
 def _make_cfg(idx, rate, scale=1.0, drive="poisson", spike_bin=1, dt_ms=0.1, iext_gamma=False):
     cfg = db_inputs.config(idx, rate_hz=(rate if idx == 1 else None), scale=scale)
     cfg["sim"]["dt_ms"] = dt_ms
@@ -523,6 +594,13 @@ def run_ours(args):
         variants["dt_0.1ms_ou_bin10"] = sub(_make_cfg(1, 7, drive="ou", spike_bin=10), 1000, 5, 3, 0, drive="ou")
         # per-neuron external currents from a Gamma law (R31): one more fp32 plane read by the update (62 B per neuron-step)
         variants["iext_gamma_plane"] = sub(_make_cfg(1, 7, iext_gamma=True), 1000, 5, 3, 0, extra_bytes=4)
+        # region sharding on one GPU: two handles that own half of the targets each, spikes exchanged every 10 steps
+        try:
+            torch.cuda.empty_cache()
+            variants["two_shards_one_gpu"] = shard_pair(db, torch, local, peer=True)
+            variants["two_shards_one_gpu_host_exchange"] = shard_pair(db, torch, local, peer=False)
+        except Exception as ex:
+            variants["two_shards_one_gpu"] = {"error": str(ex)[:200]}
         for idx, (n_s, st_s, wm_s) in {2: (500, 2, 3), 4: (500, 2, 3), 3: (150, 2, 4)}.items():
             if idx == 3 and args.skip_config3:
                 configs["3"] = "skipped (--skip-config3)"

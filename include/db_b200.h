@@ -233,6 +233,27 @@ int32_t db_step(db_sim* sim, uint32_t n_steps);
  * single-handle simulation bit for bit (tests).  Asynchronous on the stream like db_step. */
 int32_t db_deliver_external(db_sim* sim, uint64_t step, const int32_t* ids, uint64_t n);
 
+/* The lists of n_steps (1..4096) consecutive time steps in one call and one kernel launch: ids[offsets[s] .. offsets[s + 1])
+ * (HOST pointers; offsets[0] = 0, non-decreasing, offsets[n_steps] = number of ids) fired in step step_begin + s -- the
+ * layout db_read_spikes returns a step range in.  Same checks as db_deliver_external, applied to the first and the last
+ * step of the window that carry spikes; same result as one db_deliver_external call per step.  This is the call of the
+ * exchange step of a sharded run (every d_min steps, SI Eq.(6)). */
+int32_t db_deliver_external_window(db_sim* sim, uint64_t step_begin, uint32_t n_steps, const uint64_t* offsets, const int32_t* ids);
+
+/* The exchange step without the host in the data path, for shards held by ONE process (several handles on one GPU, or on
+ * GPUs with peer access: NVLink / NVSwitch): `sim` pushes the rows of the spikes that `src` -- another shard of the same
+ * network -- fired in the steps [step_begin, step_end), reading them straight out of src's raster ring in device memory
+ * (peer-mapped when src lives on another GPU; DB_ESTATE when the devices have no peer access).  One kernel on sim's
+ * stream, ordered after the steps src has launched so far; no sort, no list, no copy (the reductions commute), and the call
+ * itself neither waits nor reads back unless src's raster ring is so small that the range might have been overwritten
+ * (then it checks, which waits for src's stream).  src may step on, but must not be destroyed, and must not log more than
+ * its raster capacity of new spikes, until sim's stream has passed this point.  Errors as db_deliver_external, applied to
+ * the first and the last step of the range (DB_ERANGE: too late / too early for sim's ring, steps src has not simulated
+ * or no longer holds); same result as db_read_spikes on src followed by db_deliver_external_window on sim (tests).
+ * Between processes (one per GPU under torchrun) the lists travel by all-gather instead:
+ * paper_2211_15963_b200/sharded.py. */
+int32_t db_exchange_peer(db_sim* sim, db_sim* src, uint64_t step_begin, uint64_t step_end);
+
 /* The same operation for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
  * harnesses that forbid cudaMalloc): identical arguments, checks and result (the ring cells and the event counter get the
  * same integers), but the device copy of `ids` lives in a static device array of DB_EXTERNAL_STATIC_MAX ids (256 KB that

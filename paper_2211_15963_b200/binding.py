@@ -21,7 +21,7 @@ EXEC_AUTO, EXEC_KERNELS, EXEC_PERSISTENT, EXEC_KERNELS_DEFERRED = 0, 1, 2, 3
 EXTERNAL_STATIC_MAX = 65536   # DB_EXTERNAL_STATIC_MAX
 
 EXPORTS = [
-    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_deliver_external", "db_deliver_external_static", "db_step_profiled", "db_read_spikes",
+    "db_create", "db_create_from_csr", "db_destroy", "db_step", "db_deliver_external", "db_deliver_external_static", "db_deliver_external_window", "db_exchange_peer", "db_step_profiled", "db_read_spikes",
     "db_read_state", "db_write_state", "db_region_rates", "db_region_counts", "db_read_bold", "db_export_csr",
     "db_free_csr", "db_get_counters", "db_synchronize", "db_last_error",
 ]
@@ -122,6 +122,8 @@ def load():
         L.db_step.argtypes = [C.c_void_p, C.c_uint32]
         L.db_deliver_external.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64]
         L.db_deliver_external_static.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64]
+        L.db_deliver_external_window.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
+        L.db_exchange_peer.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64]
         L.db_step_profiled.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(PhaseTimes)]
         L.db_read_spikes.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p, C.c_uint64,
                                      C.POINTER(C.c_uint64)]
@@ -300,6 +302,18 @@ class Sim:
     def db_deliver_external(self, step: int, ids: np.ndarray):
         ids = np.ascontiguousarray(ids, np.int32)
         self._ck(self.L.db_deliver_external(self.h, int(step), _p(ids), len(ids)))
+
+    def db_deliver_external_window(self, step_begin: int, n_steps: int, steps: np.ndarray, ids: np.ndarray):
+        """The spikes (steps[k], ids[k]), sorted by step as db_read_spikes returns them, all inside
+        [step_begin, step_begin + n_steps): one call, one launch."""
+        ids = np.ascontiguousarray(ids, np.int32)
+        offs = np.searchsorted(np.asarray(steps, np.int64), np.arange(step_begin, step_begin + n_steps + 1)).astype(np.uint64)
+        assert offs[0] == 0 and offs[-1] == len(ids), "steps outside the window or not sorted"
+        self._ck(self.L.db_deliver_external_window(self.h, int(step_begin), int(n_steps), _p(offs), _p(ids)))
+
+    def db_exchange_peer(self, src: "Sim", step_begin: int, step_end: int):
+        """Push the rows of the spikes `src` fired in [step_begin, step_end), read from its raster on the device."""
+        self._ck(self.L.db_exchange_peer(self.h, src.h, int(step_begin), int(step_end)))
 
     def db_deliver_external_static(self, step: int, ids: np.ndarray):
         """db_deliver_external without any device allocation (at most EXTERNAL_STATIC_MAX ids per call)."""

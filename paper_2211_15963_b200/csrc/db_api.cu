@@ -42,6 +42,7 @@ struct db_sim {
     int32_t min_delay = 1;          // smallest one (db_deliver_external: how late an outside spike may arrive)
     int32_t* ext_ids_dev = nullptr; // db_deliver_external: device copy of the id list
     uint64_t ext_ids_cap = 0;
+    cudaEvent_t xchg_event = nullptr; // db_exchange_peer: orders this handle's stream after the source's
     double list_rate_hz = 0.0;      // arrival lists: mean firing rate their capacity was sized for
     int update_sm = 0;              // two-kernel mode: SM count the update kernel is shaped for
     cudaGraphExec_t graph_exec = nullptr;
@@ -656,6 +657,7 @@ int32_t db_destroy(db_sim* sim) {
     cudaStreamSynchronize(sim->stream);
     if (sim->graph_exec) cudaGraphExecDestroy(sim->graph_exec);
     for (cudaEvent_t e : sim->prof_events) cudaEventDestroy(e);
+    if (sim->xchg_event) cudaEventDestroy(sim->xchg_event);
     dev_free_all(sim);
     delete sim;
     return DB_OK;
@@ -790,6 +792,100 @@ __global__ void __launch_bounds__(256) k_deliver_external_static(const __grid_co
     if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
 }
 
+// db_deliver_external_window: the lists of several consecutive time steps in one launch.  ids[offs[s] .. offs[s + 1])
+// fired in step `step` + s; a warp finds the step of its spike by bisection in the (n_steps + 1) offsets.
+__global__ void __launch_bounds__(256) k_deliver_external_window(const __grid_constant__ SimDev p, const int32_t* __restrict__ ids,
+                                                                 const unsigned* __restrict__ offs, const unsigned n_steps,
+                                                                 const unsigned long long step) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned n_warps = (gridDim.x * blockDim.x) >> 5;
+    const unsigned n_ids = __ldg(offs + n_steps);
+    const unsigned long long b = (unsigned long long)p.bin_steps;
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    unsigned long long ev = 0ull;
+    for (unsigned q = warp; q < n_ids; q += n_warps) {
+        unsigned lo = 0u, hi = n_steps;                    // largest s with offs[s] <= q
+        while (hi - lo > 1u) {
+            const unsigned mid = (lo + hi) >> 1;
+            if (__ldg(offs + mid) <= q) lo = mid; else hi = mid;
+        }
+        const unsigned long long n = step + lo;
+        const unsigned nto = (unsigned)(p.bin_steps == 1 ? n : n - n % b + (b - 1ull));
+        const int j = __ldg(ids + q);
+        const int64_t rb = __ldg(p.row_begin + j);
+        const int len = __ldg(p.row_len + j);
+        for (int e = (int)lane; e < len; e += 32) {
+            const uint32_t tr = __ldg(p.tgt_rec + rb + e);
+            const unsigned dl = __ldg(p.delay + rb + e);
+            const float w = p.w_fp16 ? __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e))
+                                     : __ldg(static_cast<const float*>(p.w) + rb + e);
+            const int wq = __float2int_rn(__fmul_rn(w, p.wscale));
+            int32_t* cell = p.ring + ((size_t)((nto + dl) & Dm) * 4 + (tr >> 30)) * Np + (tr & 0x3FFFFFFFu);
+            asm volatile("red.global.add.s32 [%0], %1;" :: "l"(cell), "r"(wq) : "memory");
+        }
+        ev += (unsigned long long)len;
+    }
+    if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
+}
+
+// db_exchange_peer: the exchange step of a sharded run without the host in the data path.  The handle `p` pushes the
+// rows of the spikes ANOTHER handle logged in its raster ring (device memory of this GPU, or of a peer GPU mapped over
+// NVLink) for the steps [lo, lo + span): raster positions [scan_begin, scan_begin + m), entries of other steps are
+// skipped by their tag.  32 entries per warp and pass (one coalesced read of ids and tags), then the warp pushes the
+// matching rows one after the other.  Order does not matter (integer reductions): no sort, no list, no copy.
+__global__ void __launch_bounds__(256) k_deliver_from_raster(const __grid_constant__ SimDev p, const int32_t* src_ids,
+                                                             const uint32_t* src_tag, const unsigned long long src_mask,
+                                                             const unsigned long long* src_step_end, const unsigned src_log_mask,
+                                                             const unsigned long long step_begin, const unsigned span,
+                                                             const unsigned long long last_log) {
+    // the entries of step u lie somewhere in the raster positions [S(u - 2), S(u + 1)), S = the source's step log
+    const unsigned long long scan_begin = step_begin >= 2ull ? src_step_end[(step_begin - 2ull) & src_log_mask] : 0ull;
+    const unsigned long long m = src_step_end[last_log & src_log_mask] - scan_begin;
+    const unsigned lo = (unsigned)step_begin;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned long long warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned long long n_warps = (gridDim.x * blockDim.x) >> 5;
+    const unsigned long long b = (unsigned long long)p.bin_steps;
+    const size_t Np = (size_t)p.Npad;
+    const unsigned Dm = (unsigned)(p.D - 1);
+    unsigned long long ev = 0ull;
+    // entries per warp and pass: 32 when there is plenty of work, fewer when the range is short (a warp pushes its rows
+    // one after the other, so a short range is spread over all warps of the grid)
+    const unsigned per = (unsigned)min(32ull, max(1ull, (m + n_warps - 1ull) / n_warps));
+    for (unsigned long long base = warp * per; base < m; base += n_warps * per) {
+        int my_id = 0;
+        unsigned my_rel = 0xFFFFFFFFu;
+        if (lane < per && base + lane < m) {
+            const unsigned long long at = (scan_begin + base + lane) & src_mask;
+            my_rel = src_tag[at] - lo;
+            my_id = src_ids[at];
+        }
+        unsigned todo = __ballot_sync(0xffffffffu, my_rel < span);
+        while (todo) {
+            const int src_lane = __ffs((int)todo) - 1;
+            todo &= todo - 1u;
+            const int j = __shfl_sync(0xffffffffu, my_id, src_lane);
+            const unsigned long long n = step_begin + __shfl_sync(0xffffffffu, my_rel, src_lane);
+            const unsigned nto = (unsigned)(p.bin_steps == 1 ? n : n - n % b + (b - 1ull));
+            const int64_t rb = __ldg(p.row_begin + j);
+            const int len = __ldg(p.row_len + j);
+            for (int e = (int)lane; e < len; e += 32) {
+                const uint32_t tr = __ldg(p.tgt_rec + rb + e);
+                const unsigned dl = __ldg(p.delay + rb + e);
+                const float w = p.w_fp16 ? __half2float(__ldg(static_cast<const __half*>(p.w) + rb + e))
+                                         : __ldg(static_cast<const float*>(p.w) + rb + e);
+                const int wq = __float2int_rn(__fmul_rn(w, p.wscale));
+                int32_t* cell = p.ring + ((size_t)((nto + dl) & Dm) * 4 + (tr >> 30)) * Np + (tr & 0x3FFFFFFFu);
+                asm volatile("red.global.add.s32 [%0], %1;" :: "l"(cell), "r"(wq) : "memory");
+            }
+            ev += (unsigned long long)len;
+        }
+    }
+    if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
+}
+
 constexpr int kMaxStaticDevices = 64;
 int32_t* g_ext_ids_static_addr[kMaxStaticDevices] = {};     // device address of g_ext_ids_static, per device ordinal
 
@@ -831,6 +927,101 @@ int32_t db_deliver_external_static(db_sim* sim, uint64_t step, const int32_t* id
     CK(cudaStreamSynchronize(sim->stream));            // `ids` is the caller's pageable memory
     const unsigned grid = std::min<unsigned>(((unsigned)n + 7u) / 8u, (unsigned)sim->n_sm * 8u);
     k_deliver_external_static<<<grid, 256, 0, sim->stream>>>(d, scratch, (unsigned)n, (unsigned long long)step);
+    CK(cudaGetLastError());
+    sim->launches += 1;
+    return DB_OK;
+}
+
+int32_t db_deliver_external_window(db_sim* sim, uint64_t step_begin, uint32_t n_steps, const uint64_t* offsets, const int32_t* ids) {
+    if (!sim || !offsets || n_steps == 0 || n_steps > 4096) return DB_EINVAL;
+    const uint64_t n = offsets[n_steps];
+    if (offsets[0] != 0 || (n && !ids)) return fail(sim, DB_EINVAL, "offsets must start at 0");
+    if (n > 0xFFFFFFF0ull) return fail(sim, DB_EINVAL, "too many ids");
+    for (uint32_t s = 0; s < n_steps; ++s)
+        if (offsets[s + 1] < offsets[s]) return fail(sim, DB_EINVAL, "offsets must not decrease");
+    if (n == 0) return DB_OK;
+    CK(cudaSetDevice(sim->device));
+    const SimDev& d = sim->dev;
+    for (uint64_t k = 0; k < n; ++k) {
+        if (ids[k] < 0 || ids[k] >= d.n_rows) return fail(sim, DB_EINVAL, "id out of range");
+        if (ids[k] >= d.id0 && ids[k] < d.id0 + d.N) return fail(sim, DB_EINVAL, "id is owned by this handle: its spikes are delivered by db_step");
+    }
+    uint32_t s_first = 0, s_last = n_steps - 1;        // first and last step of the window that carry spikes
+    while (offsets[s_first + 1] == 0) ++s_first;
+    while (offsets[s_last] == n) --s_last;
+    const uint64_t b = (uint64_t)d.bin_steps;
+    const uint64_t n_lo = step_begin + s_first, n_hi = step_begin + s_last;
+    const uint64_t nt_lo = n_lo - n_lo % b + (b - 1), nt_hi = n_hi - n_hi % b + (b - 1);
+    if (nt_lo + (uint64_t)sim->min_delay < sim->host_step) return fail(sim, DB_ERANGE, "too late: the handle has stepped past the arrival of these spikes");
+    if (nt_hi + (uint64_t)sim->max_delay >= sim->host_step + (uint64_t)d.D - 2) return fail(sim, DB_ERANGE, "too early: the arrivals lie beyond the ring");
+    const uint64_t need = n + (uint64_t)n_steps + 1;   // [ids | offsets as u32]
+    if (need > sim->ext_ids_cap) {
+        const uint64_t cap = std::max<uint64_t>(next_pow2(need), 4096);
+        int32_t* buf = static_cast<int32_t*>(dev_alloc(sim, (size_t)cap * 4));     // (the old one is freed with the handle)
+        if (!buf) return fail(sim, DB_ENOMEM, "device allocation for the external spike list failed");
+        sim->ext_ids_dev = buf; sim->ext_ids_cap = cap;
+    }
+    uint32_t offs32[4097];
+    for (uint32_t s = 0; s <= n_steps; ++s) offs32[s] = (uint32_t)offsets[s];
+    unsigned* offs_dev = reinterpret_cast<unsigned*>(sim->ext_ids_dev + n);
+    CK(cudaMemcpyAsync(sim->ext_ids_dev, ids, (size_t)n * 4, cudaMemcpyHostToDevice, sim->stream));
+    CK(cudaMemcpyAsync(offs_dev, offs32, ((size_t)n_steps + 1) * 4, cudaMemcpyHostToDevice, sim->stream));
+    CK(cudaStreamSynchronize(sim->stream));            // `ids` and offs32 are pageable host memory
+    const unsigned grid = std::min<unsigned>(((unsigned)n + 7u) / 8u, (unsigned)sim->n_sm * 8u);
+    k_deliver_external_window<<<grid, 256, 0, sim->stream>>>(d, sim->ext_ids_dev, offs_dev, n_steps, (unsigned long long)step_begin);
+    CK(cudaGetLastError());
+    sim->launches += 1;
+    return DB_OK;
+}
+
+int32_t db_exchange_peer(db_sim* sim, db_sim* src, uint64_t step_begin, uint64_t step_end) {
+    if (!sim || !src || sim == src) return DB_EINVAL;
+    const SimDev& d = sim->dev;
+    const SimDev& o = src->dev;
+    if (d.n_rows != o.n_rows) return fail(sim, DB_EINVAL, "the two handles are not shards of the same network");
+    if (!(o.id0 + o.N <= d.id0 || d.id0 + d.N <= o.id0)) return fail(sim, DB_EINVAL, "the two handles own overlapping neuron ranges");
+    if (step_begin > step_end || step_end - step_begin > 0xFFFFFFFFull) return fail(sim, DB_EINVAL, "bad step range");
+    if (step_begin == step_end) return DB_OK;
+    if (step_end > src->host_step) return fail(sim, DB_ERANGE, "the source has not simulated these steps yet");
+    // where the arrivals fall in this handle's ring (as db_deliver_external, for the first and the last step of the range,
+    // whether or not they carry spikes)
+    const uint64_t b = (uint64_t)d.bin_steps, s_hi = step_end - 1;
+    const uint64_t nt_lo = step_begin - step_begin % b + (b - 1), nt_hi = s_hi - s_hi % b + (b - 1);
+    if (nt_lo + (uint64_t)sim->min_delay < sim->host_step) return fail(sim, DB_ERANGE, "too late: the handle has stepped past the arrival of these spikes");
+    if (nt_hi + (uint64_t)sim->max_delay >= sim->host_step + (uint64_t)d.D - 2) return fail(sim, DB_ERANGE, "too early: the arrivals lie beyond the ring");
+    // is the range still in the source's step log and raster ring?
+    const uint64_t log_cap = (uint64_t)o.step_log_mask + 1;
+    const uint64_t first_log = step_begin >= 2 ? step_begin - 2 : 0;
+    const uint64_t last_log = std::min<uint64_t>(step_end, src->host_step - 1);
+    if (src->host_step - first_log > log_cap) return fail(sim, DB_ERANGE, "steps older than the source's step log");
+    // the source cannot have logged more than (steps since) x (its neurons) spikes since the range began: when even that
+    // fits its raster ring nothing has to be read back, and the call neither copies nor waits
+    if ((src->host_step - first_log) * (uint64_t)o.N > src->spike_cap) {
+        Ctl c;
+        if (int32_t rc = read_ctl(src, &c)) return fail(sim, rc, "source handle: " + src->err);
+        uint64_t scan_begin = 0;
+        if (step_begin >= 2) CK(cudaMemcpy(&scan_begin, o.step_end + ((step_begin - 2) & o.step_log_mask), 8, cudaMemcpyDeviceToHost));
+        if (c.spike_begin - scan_begin > src->spike_cap) return fail(sim, DB_ERANGE, "spikes already overwritten in the source's raster ring");
+    }
+    CK(cudaSetDevice(sim->device));
+    if (src->device != sim->device) {                  // the source's raster is read over the NVLink / PCIe peer mapping
+        int can = 0;
+        CK(cudaDeviceCanAccessPeer(&can, sim->device, src->device));
+        if (!can) return fail(sim, DB_ESTATE, "no peer access between the two devices: exchange through db_read_spikes / db_deliver_external_window");
+        const cudaError_t e = cudaDeviceEnablePeerAccess(src->device, 0);
+        if (e == cudaErrorPeerAccessAlreadyEnabled) (void)cudaGetLastError();
+        else if (e != cudaSuccess) return fail(sim, DB_ECUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+    }
+    if (src->stream != sim->stream) {                  // the kernel runs after the steps the source has launched so far
+        if (!sim->xchg_event) CK(cudaEventCreateWithFlags(&sim->xchg_event, cudaEventDisableTiming));
+        if (src->device != sim->device) CK(cudaSetDevice(src->device));
+        CK(cudaEventRecord(sim->xchg_event, src->stream));
+        if (src->device != sim->device) CK(cudaSetDevice(sim->device));
+        CK(cudaStreamWaitEvent(sim->stream, sim->xchg_event, 0));
+    }
+    k_deliver_from_raster<<<(unsigned)sim->n_sm * 4u, 256, 0, sim->stream>>>(d, o.spike_ids, o.spike_tag, o.spike_mask, o.step_end, o.step_log_mask,
+                                                                             (unsigned long long)step_begin, (unsigned)(step_end - step_begin),
+                                                                             (unsigned long long)last_log);
     CK(cudaGetLastError());
     sim->launches += 1;
     return DB_OK;

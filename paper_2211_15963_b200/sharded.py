@@ -51,12 +51,11 @@ def exchange(dist, torch, sim, step_begin: int, step_end: int, device="cpu"):
     gathered = all_gather_spikes(dist, torch, st, ids, step_begin, device)
     rank, n = dist.get_rank(), 0
     for r, (s_r, i_r) in enumerate(gathered):
-        if r == rank:
+        if r == rank or len(i_r) == 0:
             continue
-        for step in np.unique(s_r):
-            sel = i_r[s_r == step]
-            sim.db_deliver_external(int(step), sel)
-            n += len(sel)
+        order = np.argsort(s_r, kind="stable")               # by step: the layout of the window call
+        sim.db_deliver_external_window(step_begin, step_end - step_begin, s_r[order], i_r[order])
+        n += len(i_r)
     return n
 
 
@@ -68,4 +67,21 @@ def run(dist, torch, sim, n_steps: int, d_min: int, device="cpu"):
         k = min(d_min, end - done)
         sim.db_step(k)
         exchange(dist, torch, sim, done, done + k, device)
+        done += k
+
+
+def run_local(shards, n_steps: int, d_min: int):
+    """The same for shards held by ONE process (handles on one GPU, or on GPUs with peer access): every d_min steps each
+    handle pushes the rows of the others' new spikes straight out of their rasters in device memory
+    (db_exchange_peer).  Nothing here waits on the host."""
+    done = int(shards[0].db_get_counters()["steps"])
+    end = done + n_steps
+    while done < end:
+        k = min(d_min, end - done)
+        for sh in shards:
+            sh.db_step(k)
+        for dst in shards:
+            for src in shards:
+                if src is not dst:
+                    dst.db_exchange_peer(src, done, done + k)
         done += k

@@ -139,8 +139,10 @@ class FakeSim:                       # stands in for the CUDA handle: the exchan
         if rank == 1 and a <= 7 < b:
             st, ids = np.append(st, np.uint64(7)), np.append(ids, np.int32(1999))
         return st, ids
-    def db_deliver_external(self, step, ids):
-        self.got.append((int(step), [int(x) for x in ids]))
+    def db_deliver_external_window(self, step_begin, n_steps, steps, ids):
+        assert np.all(np.diff(steps.astype(np.int64)) >= 0) and steps.min() >= step_begin and steps.max() < step_begin + n_steps
+        for step in np.unique(steps):
+            self.got.append((int(step), [int(x) for x in ids[steps == step]]))
 
 sim = FakeSim()
 sharded.run(dist, torch, sim, 10, 4)
@@ -152,7 +154,7 @@ dist.destroy_process_group()
 
 def test_sharded_exchange_over_two_ranks_gloo():
     # the host side of the region-sharded path: all-gather of the variable-length spike lists every d_min
-    # steps, delivery of the OTHER ranks' spikes step by step; world_size 2 on the CPU (gloo)
+    # steps, delivery of the OTHER ranks' spikes window by window; world_size 2 on the CPU (gloo)
     import socket
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))

@@ -244,9 +244,10 @@ def test_per_neuron_external_current_from_a_gamma_law(db, oracle_mod, mode):
     assert e.value.code == db.binding.DB_ESTATE
 
 
-def _run_shards(db, shards, bounds, steps, every):
+def _run_shards(db, shards, bounds, steps, every, window=False, peer=False):
     """Step the handles `shards` (owning [bounds[k], bounds[k + 1])) together: every `every` steps each one's new spikes go
-    to all the others (db_read_spikes -> db_deliver_external, step by step).  Returns the merged raster."""
+    to all the others (db_read_spikes -> db_deliver_external step by step, or db_deliver_external_window once).  Returns
+    the merged raster."""
     done, all_st, all_id = 0, [], []
     while done < steps:
         n = min(every, steps - done)
@@ -256,6 +257,12 @@ def _run_shards(db, shards, bounds, steps, every):
         for k, dst in enumerate(shards):
             for j, (st, ids) in enumerate(fresh):
                 if j == k:
+                    continue
+                if peer:
+                    dst.db_exchange_peer(shards[j], done, done + n)
+                    continue
+                if window:
+                    dst.db_deliver_external_window(done, n, st, ids)
                     continue
                 for step in np.unique(st):
                     dst.db_deliver_external(int(step), ids[st == step])
@@ -268,7 +275,7 @@ def _run_shards(db, shards, bounds, steps, every):
 
 
 @pytest.mark.parametrize("mode", MODES)
-@pytest.mark.parametrize("source", ["csr", "generator"])
+@pytest.mark.parametrize("source", ["csr", "generator", "peer"])     # exchange: one call per step / per window / device to device
 def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, oracle_mod, mode, source):
     # SURVEY 8(f) row 3, the half that one GPU can test (SI Eq.(6); layout P:L494): each handle owns a range of
     # targets -- state, ring and the synapses onto them from EVERY source -- and receives the other's spikes as id lists
@@ -293,7 +300,7 @@ def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, o
         assert np.array_equal(s.db_read_state(db.FIELD_V), Vo[bounds[k]:bounds[k + 1]])          # V0 keyed by global id
         assert np.array_equal(s.db_read_state(db.FIELD_TYPE), net["ntype"][bounds[k]:bounds[k + 1]])
     steps, d_min = 300, 3
-    st, ids = _run_shards(db, shards, bounds, steps, d_min)
+    st, ids = _run_shards(db, shards, bounds, steps, d_min, window=(source == "generator"), peer=(source == "peer"))
     o.step(steps)
     so, io = o.spikes()
     order = np.lexsort((io, so))
@@ -321,6 +328,19 @@ def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, o
     assert e.value.code == db.binding.DB_ERANGE
     with pytest.raises(db.DbError):
         shards[1].db_read_state(db.FIELD_V, first=0, count=10)       # not its neurons
+    with pytest.raises(db.DbError) as e:                              # device-to-device: too late, not simulated yet, same handle
+        shards[0].db_exchange_peer(shards[1], steps - 12, steps - 6)
+    assert e.value.code == db.binding.DB_ERANGE
+    with pytest.raises(db.DbError) as e:
+        shards[0].db_exchange_peer(shards[1], steps - 1, steps + 1)
+    assert e.value.code == db.binding.DB_ERANGE
+    with pytest.raises(db.DbError):
+        shards[0].db_exchange_peer(shards[0], steps - 1, steps)
+    with pytest.raises(db.DbError) as e:                              # window: the first step that carries spikes is too late
+        shards[0].db_deliver_external_window(steps - 12, 12, np.array([steps - 10, steps - 1]), np.array([cut + 1, cut + 2], np.int32))
+    assert e.value.code == db.binding.DB_ERANGE
+    with pytest.raises(db.DbError):
+        shards[0].db_deliver_external_window(steps - 2, 2, np.array([steps - 1]), np.array([5], np.int32))      # owned id
 
 
 @pytest.mark.parametrize("mode", MODES)
