@@ -886,6 +886,12 @@ __global__ void __launch_bounds__(256) k_deliver_from_raster(const __grid_consta
     if (lane == 0 && ev) atomicAdd(&p.ctl->events, ev);
 }
 
+// db_write_state(DB_FIELD_REF): the refractory counter of neuron i goes into the low bits of rt[i]; the type bits stay.
+__global__ void __launch_bounds__(256) k_write_ref(uint16_t* __restrict__ rt, const int32_t* __restrict__ ref, const int64_t count) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (int64_t)gridDim.x * blockDim.x)
+        rt[i] = (uint16_t)((rt[i] & ~kRefMask) | ref[i]);
+}
+
 constexpr int kMaxStaticDevices = 64;
 int32_t* g_ext_ids_static_addr[kMaxStaticDevices] = {};     // device address of g_ext_ids_static, per device ordinal
 
@@ -1134,15 +1140,11 @@ int32_t db_read_spikes(db_sim* sim, uint64_t step_begin, uint64_t step_end, uint
     *n_out = n;
     if (n == 0 || cap == 0) return DB_OK;
     const uint64_t m = scan_end - scan_begin;
-    if (m >= 2048) {                    // long ranges: select and sort on the device (db_raster.cu)
-        std::vector<unsigned long long> keys;
-        CK(raster_sorted_keys(sim->dev, sim->n_sm, scan_begin, m, (uint32_t)step_begin, (uint32_t)(step_end - step_begin), n, &keys, sim->stream));
-        if (keys.size() < n || keys[(size_t)n - 1] == ~0ull || (keys.size() > n && keys[(size_t)n] != ~0ull))
-            return fail(sim, DB_ESTATE, "raster log is inconsistent");
-        for (uint64_t o = 0; o < n && o < cap; ++o) {
-            if (steps) steps[o] = step_begin + (keys[(size_t)o] >> 32);
-            if (ids) ids[o] = (int32_t)(uint32_t)keys[(size_t)o];
-        }
+    if (m >= 2048) {                    // long ranges: select, sort and split on the device (db_raster.cu), copy into the caller's arrays
+        bool consistent = false;
+        CK(raster_sorted_read(sim->dev, sim->n_sm, scan_begin, m, (uint32_t)step_begin, (uint32_t)(step_end - step_begin), n, step_begin,
+                              steps, ids, cap, &consistent, sim->stream));
+        if (!consistent) return fail(sim, DB_ESTATE, "raster log is inconsistent");
         return DB_OK;
     }
     std::vector<int32_t> id_raw((size_t)m);
@@ -1262,15 +1264,18 @@ int32_t db_write_state(db_sim* sim, uint32_t field, int64_t first, int64_t count
     case DB_FIELD_IEXT:
         if (!d.iext) return fail(sim, DB_ESTATE, "no neuron type draws its external current per neuron (iext_gamma_shape = 0)");
         CK(cudaMemcpy(d.iext + first, src, (size_t)count * 4, cudaMemcpyHostToDevice)); break;
-    case DB_FIELD_REF: {
-        std::vector<uint16_t> t((size_t)count);
-        CK(cudaMemcpy(t.data(), d.rt + first, (size_t)count * 2, cudaMemcpyDeviceToHost));
-        for (int64_t i = 0; i < count; ++i) {
-            const int32_t r = static_cast<const int32_t*>(src)[i];
-            if (r < 0 || r > kRefMask) return fail(sim, DB_EINVAL, "ref out of range");
-            t[(size_t)i] = (uint16_t)((t[(size_t)i] & ~kRefMask) | r);
-        }
-        CK(cudaMemcpy(d.rt + first, t.data(), (size_t)count * 2, cudaMemcpyHostToDevice));
+    case DB_FIELD_REF: {                               // the counter shares a 16-bit word with the neuron type: merged on the device
+        const int32_t* in = static_cast<const int32_t*>(src);
+        int32_t lo = 0, hi = 0;
+        for (int64_t i = 0; i < count; ++i) { lo = std::min(lo, in[i]); hi = std::max(hi, in[i]); }
+        if (lo < 0 || hi > kRefMask) return fail(sim, DB_EINVAL, "ref out of range");
+        int32_t* tmp = nullptr;
+        CK(cudaMallocAsync(&tmp, (size_t)count * 4, sim->stream));
+        CK(cudaMemcpyAsync(tmp, in, (size_t)count * 4, cudaMemcpyHostToDevice, sim->stream));
+        k_write_ref<<<(unsigned)std::min<int64_t>((count + 255) / 256, (int64_t)sim->n_sm * 16), 256, 0, sim->stream>>>(d.rt + first, tmp, count);
+        CK(cudaGetLastError());
+        CK(cudaFreeAsync(tmp, sim->stream));
+        CK(cudaStreamSynchronize(sim->stream));        // `src` is the caller's memory
         break;
     }
     case DB_FIELD_RING: {

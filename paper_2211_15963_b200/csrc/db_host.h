@@ -25,11 +25,12 @@ cudaError_t persistent_fits(const SimDev& p, bool heavy, int n_sm, bool* ok);
 cudaError_t launch_persistent(const SimDev& p, bool heavy, unsigned n_steps, int n_sm, cudaStream_t st);
 
 // ---- db_raster.cu ----------------------------------------------------------
-// sorted keys (step - step_begin) << 32 | id of the raster entries at positions [scan_begin, scan_begin + m) whose step
-// lies in [lo, lo + span); entries of other steps sort behind them as ~0
+// the raster entries at positions [scan_begin, scan_begin + m) whose step lies in [lo, lo + span), sorted by (step, id):
+// keys (step - step_begin) << 32 | id, entries of other steps sort behind them as ~0
 cudaError_t raster_pool_setup(int device);                                 // per handle: keep the read-back scratch in the stream-ordered pool
-cudaError_t raster_sorted_keys(const SimDev& p, int n_sm, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
-                               std::vector<unsigned long long>* keys_host, cudaStream_t st);
+cudaError_t raster_sorted_read(const SimDev& p, int n_sm, uint64_t scan_begin, uint64_t m, uint32_t lo, uint32_t span, uint64_t n,
+                               uint64_t step_begin, uint64_t* steps_host, int32_t* ids_host, uint64_t cap, bool* consistent,
+                               cudaStream_t st);
 
 // ---- db_bold.cu ------------------------------------------------------------
 cudaError_t launch_bold_init(const BoldDev& b, int n_regions, cudaStream_t st);
