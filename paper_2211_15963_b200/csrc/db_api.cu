@@ -700,7 +700,7 @@ static int32_t step_batch(db_sim* sim, uint32_t n_steps) {
         CK(launch_step(sim, true, sim->stream));
         left -= 1;
     }
-    if (sim->graph_exec && left > (uint32_t)sim->graph_steps && (sim->host_step & 1ull)) {   // the graph starts on even steps
+    if (sim->graph_exec && left >= (uint32_t)sim->graph_steps && (sim->host_step & 1ull)) {  // the graph starts on even steps (its launches carry the parity)
         CK(launch_step(sim, false, sim->stream));
         left -= 1;
     }

@@ -419,3 +419,21 @@ def test_cortical_microcolumn_workload(db, oracle_mod, mode):
     # e1 neurons (the first 640 of every voxel) send nothing inside their voxel: only their cortico-cortical share
     deg = np.diff(net["row_ptr"])
     assert deg[:640].mean() < 0.5 * deg[800:1440].mean()
+
+
+@pytest.mark.parametrize("mode", [1, 3])
+def test_graph_replay_starts_on_an_even_step_whatever_the_batch_sizes(db, oracle_mod, mode):
+    # The step graph of the two-kernel modes (32 steps) carries the parity of the work-list half in its launches, so it may
+    # only be replayed from an even step.  Found by tests/test_gpu_parity_random.py: a db_step call that reached the graph
+    # with an odd step count and EXACTLY 32 steps left replayed it misaligned (list mode: wrong arrival lists consumed).
+    net = db_inputs.random_csr(N=3000 + 21, mean_outdeg=40, seed=33, max_delay=20)
+    t = db_inputs.type_params(bg_weight=0.012)
+    sim = db_inputs.sim_params(types=[t, dict(t)])
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    assert g.db_get_counters()["exec_mode"] == mode
+    done = 0
+    for b in (40, 33, 32, 31, 65, 33, 1, 32, 64, 34):      # graph built by the first call; 33 = prologue + 32 from an odd step
+        g.db_step(b); o.step(b); done += b
+        _check(g, o, done)
+    assert g.db_get_counters()["spikes"] > 500
