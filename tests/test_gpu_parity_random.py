@@ -100,3 +100,147 @@ def test_random_configuration_matches_the_oracle(db, oracle_mod, seed):
         if ou:
             assert np.array_equal(g.db_read_state(db.FIELD_IOU), o.iou().astype(np.float32)), (seed, mode)
         g.db_destroy()
+
+
+def _draw_spec(seed):
+    """A random network SPEC for the on-device generator (both sides generate it themselves) and plain constants."""
+    rng = np.random.default_rng(5000 + seed)
+    mode = int(rng.random() < 0.3)
+    n_regions = 1 if mode else int(rng.choice([1, 1, 4, 9]))           # the out-degree recipe has one region
+    N = int(rng.choice([3000, 5037, 8192, 12001]))
+    K = int(rng.choice([20, 60, 120]))
+    d_lo = int(rng.choice([1, 1, 3]))
+    net = db_inputs._net(N=N, n_regions=n_regions, region_size_sigma=float(rng.choice([0.0, 0.7])), mode=mode,
+                         K=0 if mode else K, intra_frac=1.0 if n_regions == 1 else float(rng.choice([0.6, 0.8])),
+                         outdeg_mean=float(rng.choice([30.0, 80.0])), outdeg_sigma=float(rng.choice([0.5, 1.0])), outdeg_cap=int(rng.choice([400, 2500])),
+                         delay_intra_min=d_lo, delay_intra_max=int(rng.choice([d_lo, 8, 20])),
+                         delay_inter_min=int(rng.choice([5, 20])), delay_inter_max=int(rng.choice([20, 40, 90])),
+                         weight_fp16=int(rng.random() < 0.3))
+    max_delay = max(net["delay_intra_max"], net["delay_inter_max"] if n_regions > 1 else 0)
+    D = 32
+    while D < max_delay + 4:
+        D *= 2
+    t = db_inputs.type_params(bg_weight=float(rng.uniform(0.008, 0.02)))
+    u = dict(t)
+    u.update(Vth=-51.0, Tref_ms=1.0, G=[0.9, 0.3, 1.1, 0.8])
+    sim = db_inputs.sim_params(D=D, window_steps=int(rng.integers(1, 12)), types=[t, u])
+    return rng, net, sim
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("DB_RANDOM_CASES", "8"))))
+def test_random_call_sequences_on_generated_networks(db, oracle_mod, seed):
+    # db_step, db_step_profiled (two-kernel modes), state writes and partial read-backs interleaved at random
+    rng, net, sim = _draw_spec(seed)
+    csr = oracle_mod.generate(net, db_inputs.GEN_SEED + seed)
+    N = net["N"]
+    ops = []
+    for _ in range(10):
+        r = rng.random()
+        if r < 0.55:
+            ops.append(("step", int(rng.integers(1, 70))))
+        elif r < 0.75:
+            ops.append(("prof", int(rng.integers(1, 40))))
+        elif r < 0.9:
+            ops.append(("write", int(rng.integers(0, 1 << 30))))
+        else:
+            ops.append(("read", None))
+    for mode in (1, 2, 3):
+        g = db.Sim.db_create(net, sim, seed=db_inputs.GEN_SEED + seed, exec_mode=mode)
+        o = oracle_mod.OracleSim(sim, csr, db_inputs.DYN_SEED)
+        used = g.db_get_counters()["exec_mode"]
+        done = 0
+        for op, arg in ops:
+            if op == "step" or (op == "prof" and used == 2):
+                g.db_step(arg); o.step(arg); done += arg
+            elif op == "prof":
+                g.db_step_profiled(arg); o.step(arg); done += arg
+            elif op == "write":
+                r2 = np.random.default_rng(arg)
+                V = r2.uniform(-75.0, -49.5, N).astype(np.float32)
+                gg = r2.gamma(1.0, 0.03, (N, 4)).astype(np.float32)
+                ref = np.where(r2.random(N) < 0.1, r2.integers(1, 15, N), 0).astype(np.int32)
+                g.set_state(V, gg, ref); o.set_state(V, gg, ref)
+            elif done:
+                a = int(rng.integers(0, done)); b = int(rng.integers(a, done + 1))
+                sg, ig = g.db_read_spikes(a, b)
+                so, io = o.spikes()
+                sel = (so >= a) & (so < b)
+                order = np.lexsort((io[sel], so[sel]))
+                assert np.array_equal(sg, so[sel][order]) and np.array_equal(ig, io[sel][order]), (seed, mode, a, b)
+            assert np.array_equal(g.db_read_state(db.FIELD_RING), o.ring()), (seed, mode, op, done)
+        Vg, gg, rg = g.state()
+        Vo, go, ro = o.state()
+        assert np.array_equal(rg, ro) and np.array_equal(Vg, Vo.astype(np.float32)) and np.array_equal(gg, go.astype(np.float32)), (seed, mode)
+        sg, ig = g.db_read_spikes(0, done)
+        so, io = o.spikes()
+        order = np.lexsort((io, so))
+        assert np.array_equal(sg, so[order]) and np.array_equal(ig, io[order]), (seed, mode)
+        cg, co = g.db_get_counters(), o.counters()
+        for k in ("steps", "spikes", "events", "bg_events"):
+            assert cg[k] == co[k], (k, seed, mode)
+        cnt, first = g.db_region_counts()
+        assert np.array_equal(cnt, o.region_counts()[first:first + len(cnt)]), (seed, mode)
+        g.db_destroy()
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("DB_RANDOM_CASES", "6"))))
+def test_random_shardings_reproduce_the_whole_network(db, oracle_mod, seed):
+    # two to four handles that own random 1024-aligned ranges, random exchange window <= the smallest delay, the three
+    # exchange calls chosen at random per window (SURVEY 8(f) row 3)
+    rng, net, sim = _draw_spec(seed)
+    net.update(mode=0, K=int(rng.choice([40, 100])) if net["N"] >= 5000 else 40, delay_intra_min=int(rng.choice([2, 3, 6])))
+    if net["n_regions"] > 1 and net["N"] < 5000:
+        net["region_size_sigma"] = 0.0                 # small regions must still hold K distinct sources
+    net["delay_intra_max"] = max(net["delay_intra_max"], net["delay_intra_min"])
+    net["delay_inter_min"] = max(net["delay_inter_min"], net["delay_intra_min"])
+    net["delay_inter_max"] = max(net["delay_inter_max"], net["delay_inter_min"])
+    try:
+        csr = oracle_mod.generate(net, db_inputs.GEN_SEED + seed)
+    except ValueError:                                 # a region smaller than the in-degree drawn from it: not a network
+        pytest.skip("random spec not realisable")
+    N = net["N"]
+    n_sh = min(int(rng.integers(2, 5)), (N - 1) // 1024 + 1)
+    cuts = sorted(int(c) * 1024 for c in rng.choice(np.arange(1, (N - 1) // 1024 + 1), n_sh - 1, replace=False))
+    bounds = [0] + cuts + [N]
+    d_min = int(rng.integers(1, net["delay_intra_min"] + 1))
+    o = oracle_mod.OracleSim(sim, csr, db_inputs.DYN_SEED)
+    mode = int(rng.integers(1, 4))
+    shards = [db.Sim.db_create(net, sim, seed=db_inputs.GEN_SEED + seed, exec_mode=mode, own=(bounds[k], bounds[k + 1] - bounds[k]))
+              for k in range(n_sh)]
+    steps, done = 90, 0
+    while done < steps:
+        n = min(d_min, steps - done)
+        for s in shards:
+            s.db_step(n)
+        how = int(rng.integers(0, 3))
+        fresh = [s.db_read_spikes(done, done + n) for s in shards] if how < 2 else None
+        for k, dst in enumerate(shards):
+            for j, src in enumerate(shards):
+                if j == k:
+                    continue
+                if how == 2:
+                    dst.db_exchange_peer(src, done, done + n)
+                elif how == 1:
+                    if len(fresh[j][1]):
+                        dst.db_deliver_external_window(done, n, fresh[j][0], fresh[j][1])
+                else:
+                    for step in np.unique(fresh[j][0]):
+                        dst.db_deliver_external(int(step), fresh[j][1][fresh[j][0] == step])
+        done += n
+    o.step(steps)
+    Vo, go, ro = o.state()
+    ring = o.ring()
+    so, io = o.spikes()
+    order = np.lexsort((io, so))
+    st = np.concatenate([s.db_read_spikes(0, steps)[0] for s in shards])
+    ids = np.concatenate([s.db_read_spikes(0, steps)[1] for s in shards])
+    od = np.lexsort((ids, st))
+    assert np.array_equal(st[od], so[order]) and np.array_equal(ids[od], io[order]), (seed, mode, bounds, d_min)
+    for k, s in enumerate(shards):
+        a, b = bounds[k], bounds[k + 1]
+        Vg, gg, rg = s.state()
+        assert np.array_equal(Vg, Vo[a:b].astype(np.float32)) and np.array_equal(gg, go[a:b].astype(np.float32)) and np.array_equal(rg, ro[a:b]), (seed, k)
+        assert np.array_equal(s.db_read_state(db.FIELD_RING), ring[:, a:b, :]), (seed, k)
+    assert sum(s.db_get_counters()["events"] for s in shards) == o.counters()["events"]
+    for s in shards:
+        s.db_destroy()
