@@ -133,6 +133,12 @@ def test_random_call_sequences_on_generated_networks(db, oracle_mod, seed):
     rng, net, sim = _draw_spec(seed)
     csr = oracle_mod.generate(net, db_inputs.GEN_SEED + seed)
     N = net["N"]
+    bold = seed % 2 == 1                               # BOLD read-out with a short count history: db_step lets it catch up
+    if bold:
+        sim["bold"] = dict(oracle_mod.BOLD_DEFAULTS)
+    max_windows = int(rng.choice([16, 64])) if bold else 0
+    sizes = np.diff(csr["region_start"])
+    win_s = sim["window_steps"] * sim["dt_ms"] * 1e-3
     ops = []
     for _ in range(10):
         r = rng.random()
@@ -145,7 +151,7 @@ def test_random_call_sequences_on_generated_networks(db, oracle_mod, seed):
         else:
             ops.append(("read", None))
     for mode in (1, 2, 3):
-        g = db.Sim.db_create(net, sim, seed=db_inputs.GEN_SEED + seed, exec_mode=mode)
+        g = db.Sim.db_create(net, sim, seed=db_inputs.GEN_SEED + seed, exec_mode=mode, max_windows=max_windows)
         o = oracle_mod.OracleSim(sim, csr, db_inputs.DYN_SEED)
         used = g.db_get_counters()["exec_mode"]
         done = 0
@@ -180,6 +186,12 @@ def test_random_call_sequences_on_generated_networks(db, oracle_mod, seed):
             assert cg[k] == co[k], (k, seed, mode)
         cnt, first = g.db_region_counts()
         assert np.array_equal(cnt, o.region_counts()[first:first + len(cnt)]), (seed, mode)
+        if bold:
+            y, stb, n = g.db_read_bold()
+            assert n == done // sim["window_steps"]
+            if n:
+                ys, sob = oracle_mod.bold_run(o.region_counts()[:n], sizes, win_s, sim["bold"])
+                assert np.max(np.abs(stb - sob)) < 1e-10 and np.max(np.abs(y - ys[-1])) < 1e-10, (seed, mode)
         g.db_destroy()
 
 
