@@ -256,3 +256,51 @@ def test_random_shardings_reproduce_the_whole_network(db, oracle_mod, seed):
     assert sum(s.db_get_counters()["events"] for s in shards) == o.counters()["events"]
     for s in shards:
         s.db_destroy()
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("DB_RANDOM_CASES", "4"))))
+def test_random_bursts_in_networks_where_a_block_owns_thousands_of_neurons(db, oracle_mod, seed):
+    # 60,000 - 300,000 neurons (a block of the persistent kernel owns 400 - 2,000 of them, several tasks per warp), a
+    # random number of rows longer than kInlineMax = 1024 synapses, and synchronised bursts of a random share of the
+    # neurons at random times: the per-block spike and heavy-row lists fill to random levels, overflow or not
+    rng = np.random.default_rng(9000 + seed)
+    N = int(rng.choice([60_000, 160_000, 300_000])) + int(rng.integers(0, 128))
+    n_heavy = int(rng.choice([0, 5, 300, 900]))
+    heavy = {int(r): int(d) for r, d in zip(rng.choice(N, n_heavy, replace=False), rng.integers(1025, 1800, n_heavy))} if n_heavy else None
+    net = db_inputs.bulk_csr(N, base_outdeg=int(rng.choice([2, 6])), seed=seed, heavy_rows=heavy, max_delay=int(rng.choice([3, 20])),
+                             n_regions=int(rng.choice([1, 5])))
+    t = db_inputs.type_params(bg_weight=float(rng.uniform(0.01, 0.03)))
+    sim = db_inputs.sim_params(types=[t, dict(t)], window_steps=int(rng.integers(1, 12)))
+    plan = []
+    for _ in range(4):
+        plan.append((int(rng.integers(1, 30)), float(rng.choice([0.0, 0.02, 0.4, 1.0]))))     # (steps, share of the neurons set above threshold first)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    snaps = []
+    for steps, share in plan:
+        V, gg, ref = o.state()
+        sel = np.random.default_rng(int(share * 1000) + steps).random(N) < share
+        V[sel] = -45.0
+        ref[sel] = 0
+        o.set_state(V, gg, ref)
+        o.step(steps)
+        snaps.append((sel, o.ring().copy(), o.counters()["spikes"]))
+    Vo, go, ro = o.state()
+    so, io = o.spikes()
+    order = np.lexsort((io, so))
+    done = sum(s for s, _ in plan)
+    for mode in (1, 2, 3):
+        g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode)
+        for (steps, share), (sel, ring, n_sp) in zip(plan, snaps):
+            V, gg, ref = g.state()
+            V[sel] = -45.0
+            ref[sel] = 0
+            g.set_state(V, gg, ref)
+            g.db_step(steps)
+            assert g.db_get_counters()["spikes"] == n_sp, (seed, mode)
+            assert np.array_equal(g.db_read_state(db.FIELD_RING), ring), (seed, mode)
+        Vg, gg, rg = g.state()
+        assert np.array_equal(rg, ro) and np.array_equal(Vg, Vo.astype(np.float32)) and np.array_equal(gg, go.astype(np.float32)), (seed, mode)
+        sg, ig = g.db_read_spikes(0, done)
+        assert np.array_equal(sg, so[order]) and np.array_equal(ig, io[order]), (seed, mode)
+        assert g.db_get_counters()["events"] == o.counters()["events"]
+        g.db_destroy()
