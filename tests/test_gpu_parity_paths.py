@@ -437,3 +437,39 @@ def test_graph_replay_starts_on_an_even_step_whatever_the_batch_sizes(db, oracle
         g.db_step(b); o.step(b); done += b
         _check(g, o, done)
     assert g.db_get_counters()["spikes"] > 500
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_long_run_past_the_wrap_of_the_step_log_and_the_raster_ring(db, oracle_mod, mode):
+    # 70,000 steps (7 s of model time at dt 0.1 ms): the step log (2^16 entries) and a small raster ring wrap several
+    # times, the rotating arrival counters of the persistent kernel run through 70,000 units in a few launches, the region
+    # history wraps.  State, ring, counters and the recent raster must still be the oracle's; old ranges are refused.
+    N = 1500 + 11
+    net = db_inputs.random_csr(N=N, mean_outdeg=15, seed=44, max_delay=20, n_regions=3)
+    t = db_inputs.type_params(bg_weight=0.012)
+    sim = db_inputs.sim_params(types=[t, dict(t)], window_steps=7)
+    g = db.Sim.db_create_from_csr(sim, net, exec_mode=mode, raster_capacity=1 << 13, max_windows=64)
+    o = oracle_mod.OracleSim(sim, net, db_inputs.DYN_SEED)
+    done = 0
+    for b in (1, 33001, 999, 32768, 3231):
+        g.db_step(b); o.step(b); done += b
+        Vg, gg, rg = g.state()
+        Vo, go, ro = o.state()
+        assert np.array_equal(rg, ro) and np.array_equal(Vg, Vo.astype(np.float32)) and np.array_equal(gg, go.astype(np.float32)), done
+        assert np.array_equal(g.db_read_state(db.FIELD_RING), o.ring()), done
+    assert done == 70000
+    cg, co = g.db_get_counters(), o.counters()
+    for k in ("steps", "spikes", "events", "bg_events"):
+        assert cg[k] == co[k], k
+    assert co["spikes"] > 5 * (1 << 13)                               # the raster ring has wrapped several times
+    so, io = o.spikes()
+    for a, b in ((done - 300, done), (done - 1200, done - 900), (done - 1, done)):      # ~4.6 spikes per step: 8192 entries hold ~1,700 steps
+        sg, ig = g.db_read_spikes(a, b)
+        sel = (so >= a) & (so < b)
+        order = np.lexsort((io[sel], so[sel]))
+        assert np.array_equal(sg, so[sel][order]) and np.array_equal(ig, io[sel][order]), (a, b)
+    with pytest.raises(db.DbError) as e:
+        g.db_read_spikes(0, 100)                                       # overwritten long ago
+    assert e.value.code == db.binding.DB_ERANGE
+    cnt, first = g.db_region_counts()
+    assert first > 0 and np.array_equal(cnt, o.region_counts()[first:first + len(cnt)])
