@@ -293,7 +293,9 @@ def test_two_handles_that_own_half_of_the_targets_each_reproduce_the_whole(db, o
     if source == "csr":
         shards = [db.Sim.db_create_from_csr(cfg["sim"], net, exec_mode=mode, own=(bounds[k], bounds[k + 1] - bounds[k])) for k in range(2)]
     else:
+        # a small raster ring makes db_exchange_peer check the sender's counters first (its slower, validating path)
         shards = [db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, exec_mode=mode,
+                                   raster_capacity=(1 << 14) if (source == "peer" and mode != 2) else 0,
                                    own=(bounds[k], bounds[k + 1] - bounds[k])) for k in range(2)]
     Vo = o.state()[0].astype(np.float32)
     for k, s in enumerate(shards):
