@@ -171,3 +171,34 @@ def test_sharded_exchange_over_two_ranks_gloo():
     want1 = [(s, [s]) for s in range(10)]
     assert [(s, sorted(i)) for s, i in res[0]["got"]] == [(s, sorted(i)) for s, i in want0]
     assert [(s, i) for s, i in res[1]["got"]] == want1
+
+
+def test_sharded_run_local_orders_steps_and_exchanges():
+    # single-process sharding (handles on one GPU or on peer GPUs): every window each handle steps, then pulls the window
+    # of every OTHER handle with db_exchange_peer; host logic only, with stand-ins for the CUDA handles
+    from paper_2211_15963_b200 import sharded
+    log = []
+
+    class Fake:
+        def __init__(self, name):
+            self.name, self.steps = name, 0
+        def db_get_counters(self):
+            return {"steps": self.steps}
+        def db_step(self, k):
+            log.append(("step", self.name, self.steps, k)); self.steps += k
+        def db_exchange_peer(self, src, a, b):
+            assert src is not self and src.steps >= b and self.steps >= b      # both have simulated the window
+            log.append(("pull", self.name, src.name, a, b))
+
+    shards = [Fake("a"), Fake("b"), Fake("c")]
+    sharded.run_local(shards, 10, 4)
+    assert [s.steps for s in shards] == [10, 10, 10]
+    windows = [(0, 4), (4, 8), (8, 10)]
+    for (a, b) in windows:
+        pulls = [e for e in log if e[0] == "pull" and e[3:] == (a, b)]
+        assert sorted((e[1], e[2]) for e in pulls) == [(x, y) for x in "abc" for y in "abc" if x != y]
+    # inside a window every step precedes every pull
+    for (a, b) in windows:
+        idx_steps = [i for i, e in enumerate(log) if e[0] == "step" and e[2] == a]
+        idx_pulls = [i for i, e in enumerate(log) if e[0] == "pull" and e[3] == a]
+        assert max(idx_steps) < min(idx_pulls)
