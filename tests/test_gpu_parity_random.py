@@ -131,7 +131,10 @@ def _draw_spec(seed):
 def test_random_call_sequences_on_generated_networks(db, oracle_mod, seed):
     # db_step, db_step_profiled (two-kernel modes), state writes and partial read-backs interleaved at random
     rng, net, sim = _draw_spec(seed)
-    csr = oracle_mod.generate(net, db_inputs.GEN_SEED + seed)
+    try:
+        csr = oracle_mod.generate(net, db_inputs.GEN_SEED + seed)
+    except ValueError:                                 # a region smaller than the in-degree drawn from it: not a network
+        pytest.skip("random spec not realisable")
     N = net["N"]
     bold = seed % 2 == 1                               # BOLD read-out with a short count history: db_step lets it catch up
     if bold:
