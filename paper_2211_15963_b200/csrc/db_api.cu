@@ -43,6 +43,7 @@ struct db_sim {
     int32_t* ext_ids_dev = nullptr; // db_deliver_external: device copy of the id list
     uint64_t ext_ids_cap = 0;
     cudaEvent_t xchg_event = nullptr; // db_exchange_peer: orders this handle's stream after the source's
+    int xchg_event_dev = -1;          // device the event was created on (the source's)
     double list_rate_hz = 0.0;      // arrival lists: mean firing rate their capacity was sized for
     int update_sm = 0;              // two-kernel mode: SM count the update kernel is shaped for
     cudaGraphExec_t graph_exec = nullptr;
@@ -1019,8 +1020,13 @@ int32_t db_exchange_peer(db_sim* sim, db_sim* src, uint64_t step_begin, uint64_t
         else if (e != cudaSuccess) return fail(sim, DB_ECUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
     }
     if (src->stream != sim->stream) {                  // the kernel runs after the steps the source has launched so far
-        if (!sim->xchg_event) CK(cudaEventCreateWithFlags(&sim->xchg_event, cudaEventDisableTiming));
+        // the event is recorded on the source's stream, so it has to live on the source's device
         if (src->device != sim->device) CK(cudaSetDevice(src->device));
+        if (sim->xchg_event && sim->xchg_event_dev != src->device) { cudaEventDestroy(sim->xchg_event); sim->xchg_event = nullptr; }
+        if (!sim->xchg_event) {
+            CK(cudaEventCreateWithFlags(&sim->xchg_event, cudaEventDisableTiming));
+            sim->xchg_event_dev = src->device;
+        }
         CK(cudaEventRecord(sim->xchg_event, src->stream));
         if (src->device != sim->device) CK(cudaSetDevice(sim->device));
         CK(cudaStreamWaitEvent(sim->stream, sim->xchg_event, 0));

@@ -475,3 +475,43 @@ def test_long_run_past_the_wrap_of_the_step_log_and_the_raster_ring(db, oracle_m
     assert e.value.code == db.binding.DB_ERANGE
     cnt, first = g.db_region_counts()
     assert first > 0 and np.array_equal(cnt, o.region_counts()[first:first + len(cnt)])
+
+
+def test_device_to_device_exchange_between_handles_on_different_streams(db, oracle_mod):
+    # db_exchange_peer orders the receiver's stream after the sender's steps with an event when the two handles run on
+    # different streams (the handles of the other tests share torch's current stream).  Nothing here synchronises the
+    # host between the steps and the exchanges.
+    import torch
+    cfg = db_inputs.config(2, scale=0.004)
+    cfg["net"].update(n_regions=8, delay_intra_min=4, delay_inter_min=20)
+    t = db_inputs.type_params(bg_weight=0.02)
+    t.update(G=[0.5, 0.125, 0.5, 0.5])
+    cfg["sim"]["types"] = [t, dict(t)]
+    N = cfg["net"]["N"]
+    net = oracle_mod.generate(cfg["net"], db_inputs.GEN_SEED)
+    o = oracle_mod.OracleSim(cfg["sim"], net, db_inputs.DYN_SEED)
+    bounds = [0, 7 * 1024, 13 * 1024, N]
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    shards = []
+    for k in range(3):
+        with torch.cuda.stream(streams[k]):              # the handle keeps the stream that is current when it is created
+            shards.append(db.Sim.db_create(cfg["net"], cfg["sim"], seed=db_inputs.GEN_SEED, exec_mode=[2, 1, 3][k],
+                                           own=(bounds[k], bounds[k + 1] - bounds[k])))
+    from paper_2211_15963_b200 import sharded
+    sharded.run_local(shards, 240, 4)
+    torch.cuda.synchronize()
+    o.step(240)
+    so, io = o.spikes()
+    order = np.lexsort((io, so))
+    parts = [s.db_read_spikes(0, 240) for s in shards]
+    st, ids = np.concatenate([a for a, _ in parts]), np.concatenate([b for _, b in parts])
+    od = np.lexsort((ids, st))
+    assert np.array_equal(st[od], so[order]) and np.array_equal(ids[od], io[order]) and len(ids) > 300
+    Vo, go, ro = o.state()
+    ring = o.ring()
+    for k, s in enumerate(shards):
+        a, b = bounds[k], bounds[k + 1]
+        Vg, gg, rg = s.state()
+        assert np.array_equal(Vg, Vo[a:b].astype(np.float32)) and np.array_equal(gg, go[a:b].astype(np.float32)) and np.array_equal(rg, ro[a:b])
+        assert np.array_equal(s.db_read_state(db.FIELD_RING), ring[:, a:b, :])
+    assert sum(s.db_get_counters()["events"] for s in shards) == o.counters()["events"]
